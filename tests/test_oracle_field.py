@@ -1,0 +1,242 @@
+"""Pins for the oracle's rho reduction, Poisson/E solve, diagnostics and Strang step
+(pins p10, p11, p12 and the density / DFT special cases).
+
+Nothing here calls the CUDA path.  Independent references: closed forms, numpy's FFT
+(a library routine the oracle does not call), exact polynomial integrals, and the
+kinetic-theory Landau damping rate (value in BASELINE.json).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+import workloads as W
+
+
+def coords(orc):
+    return [orc.node_coords(a) for a in range(orc.d)]
+
+
+# --------------------------------------------------------------- O4 density
+
+def test_density_integrates_polynomials_in_v_exactly():
+    """rho = int f dv is the exact integral of the dG polynomial: for
+    f = g(x) * v1^p * v2^q with p, q <= 2k+1 the (k+1)-point GL rule is exact."""
+    k = 2
+    orc = O.Oracle(1, 2, [3, 4, 5], k, [0.0, 1.0, -1.0, 2.0, 0.5, 3.0])
+    x, v1, v2 = coords(orc)
+    g = 1.0 + x ** 2
+    for p, q in ((0, 0), (1, 0), (2, 3), (5, 5), (4, 1)):
+        f = (v2[:, None, None] ** q) * (v1[None, :, None] ** p) * g[None, None, :]
+        rho = orc.density(f)
+        i1 = (2.0 ** (p + 1) - (-1.0) ** (p + 1)) / (p + 1)
+        i2 = (3.0 ** (q + 1) - 0.5 ** (q + 1)) / (q + 1)
+        assert np.abs(rho - g * i1 * i2).max() < 1e-12 * abs(i1 * i2)
+
+
+def test_density_picks_the_right_weight_for_every_v_node():
+    """A unit spike at one v node gives rho = h_v1 w_j1 h_v2 w_j2 at that x node only (index / weight pin)."""
+    k = 1
+    orc = O.Oracle(2, 2, [2, 3, 2, 3], k, [0, 1.0, 0, 1.0, -1.0, 1.0, -3.0, 3.0])
+    _, w = np.polynomial.legendre.leggauss(k + 1)
+    w = w / 2
+    hv1, hv2 = 2.0 / 2, 6.0 / 3
+    for (n2, n1, m2, m1) in ((0, 0, 0, 0), (5, 3, 1, 2), (2, 1, 5, 3)):
+        f = np.zeros(orc.shape)
+        f[n2, n1, m2, m1] = 1.0
+        rho = orc.density(f)
+        want = np.zeros(orc.xshape)
+        want[m2, m1] = hv1 * w[n1 % 2] * hv2 * w[n2 % 2]
+        assert np.abs(rho - want).max() < 1e-16
+
+
+def test_p11_landau_density_is_one_plus_eps_cos():
+    """f0 = (1 + eps cos(k x1) + eps cos(k x2)) * Maxwellian -> rho = 1 + eps(...) up to
+    the e^{-18} tails and the GL error of the Gaussian (k=2, 24 cells on [-6,6]: < 1e-9)."""
+    cfg = W.scaled(W.CONFIGS[0], [4, 4, 24, 24])
+    cfg["degree"] = 2
+    orc = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    f = W.initial_data(cfg, coords(orc)).numpy()
+    rho = orc.density(f)
+    x1, x2 = orc.node_coords(0), orc.node_coords(1)
+    want = 1 + 0.01 * np.cos(0.5 * x1)[None, :] + 0.01 * np.cos(0.5 * x2)[:, None]
+    assert np.abs(rho - want).max() < 1e-8
+
+
+# --------------------------------------------------------------- O5 Poisson / E
+
+@pytest.mark.parametrize("k", [1, 2, 3])
+def test_p10_poisson_cos_half_x_closed_form_and_order(k):
+    """-phi'' = cos(0.5 x) on [0,4pi) periodic.  With -Laplace(phi) = 1 - rho that is
+    rho = 1 - cos(0.5x), phi = 4 cos(0.5 x), E = -phi' = 2 sin(0.5 x).  Error falls at order >= k+1
+    under cell doubling (reading P1: interpolation error of the equidistant transfer)."""
+    errs = []
+    for N in (8, 16, 32):
+        orc = O.Oracle(1, 1, [N, 2], k, [0, 4 * math.pi, -1, 1])
+        x = orc.node_coords(0)
+        E = orc.poisson(1 - np.cos(0.5 * x))[0]
+        errs.append(np.abs(E - 2 * np.sin(0.5 * x)).max())
+    assert errs[0] < 0.05
+    for a, b in zip(errs, errs[1:]):
+        if a > 1e-11:
+            assert math.log2(a / b) > k + 1 - 0.35
+
+
+def test_p10_sign_and_component_layout_2d():
+    """rho = 1 - cos(0.5 x1) - 0.5 cos(x2)  ->  E1 = 2 sin(0.5 x1), E2 = 0.5 sin(x2); E is [dx][X]
+    component-major with x1 fastest."""
+    orc = O.Oracle(2, 2, [24, 16, 2, 2], 3, [0, 4 * math.pi, 0, 2 * math.pi, -1, 1, -1, 1])
+    x1, x2 = orc.node_coords(0), orc.node_coords(1)
+    rho = 1 - np.cos(0.5 * x1)[None, :] - 0.5 * np.cos(x2)[:, None]
+    E = orc.poisson(rho)
+    assert E.shape == (2, 64, 96)
+    assert np.abs(E[0] - 2 * np.sin(0.5 * x1)[None, :]).max() < 2e-5
+    assert np.abs(E[1] - 0.5 * np.sin(x2)[:, None]).max() < 2e-5
+
+
+def test_poisson_ignores_mean_and_is_linear():
+    """Zero mode -> 0 (reading P1 (iii)): adding a constant to rho leaves E unchanged; E is linear in rho."""
+    orc = O.Oracle(2, 2, [5, 4, 2, 2], 2, [0, 3.0, 0, 2.0, -1, 1, -1, 1])
+    rng = np.random.default_rng(5)
+    r1, r2 = rng.uniform(0, 1, orc.xshape), rng.uniform(0, 1, orc.xshape)
+    E1, E2 = orc.poisson(r1), orc.poisson(r2)
+    assert np.abs(orc.poisson(r1 + 7.5) - E1).max() < 1e-13
+    assert np.abs(orc.poisson(2 * r1 - 3 * r2) - (2 * E1 - 3 * E2)).max() < 1e-13
+    assert np.abs(orc.poisson(np.full(orc.xshape, 3.0))).max() < 1e-15
+
+
+@pytest.mark.parametrize("dx,cells", [(1, [12]), (1, [7]), (2, [6, 5]), (3, [4, 3, 5])])
+def test_poisson_k0_reduces_to_numpy_fft_spectral_solve(dx, cells):
+    """k=0: one node per cell at the cell centre = the equidistant grid itself, P = P^-1 = 1, so reading P1
+    reduces to the textbook spectral solve E^_d = i kappa_d rho^/|kappa|^2, written here with numpy.fft
+    (a library routine the oracle does not call; the oracle uses a naive DFT).  Odd and even lengths."""
+    L = [3.0, 2.0, 5.0][:dx]
+    dom = []
+    for a in range(dx):
+        dom += [0.0, L[a]]
+    dom += [-1.0, 1.0] * dx
+    orc = O.Oracle(dx, dx, cells + [1] * dx, 0, dom)
+    rng = np.random.default_rng(21)
+    rho = rng.uniform(0, 1, orc.xshape)
+    E = orc.poisson(rho)
+    rh = np.fft.fftn(rho)
+    kap = []
+    for a in range(dx):
+        n = cells[a]
+        kk = 2 * math.pi * np.fft.fftfreq(n, d=L[a] / n)
+        shp = [1] * dx
+        shp[dx - 1 - a] = n
+        kap.append(kk.reshape(shp))
+    k2 = sum(kk ** 2 for kk in kap)
+    k2[(0,) * dx] = 1.0
+    for d in range(dx):
+        kd = kap[d].copy()
+        if cells[d] % 2 == 0:
+            idx = [slice(None)] * dx
+            idx[dx - 1 - d] = cells[d] // 2
+            kd = np.broadcast_to(kd, rho.shape).copy()
+            kd[tuple(idx)] = 0.0
+        Eh = 1j * kd * rh / k2
+        Eh[(0,) * dx] = 0.0
+        want = np.fft.ifftn(Eh).real
+        assert np.abs(E[d] - want).max() < 1e-13
+
+
+def test_poisson_satisfies_gauss_law_on_resolved_modes():
+    """div E = 1 - rho (from E = -grad phi, -Laplace phi = 1 - rho) for a resolved 2-d mode mix."""
+    orc = O.Oracle(2, 2, [20, 20, 2, 2], 3, [0, 2 * math.pi, 0, 2 * math.pi, -1, 1, -1, 1])
+    x1, x2 = orc.node_coords(0)[None, :], orc.node_coords(1)[:, None]
+    rho = 1 + 0.3 * np.cos(x1 + 2 * x2) + 0.2 * np.sin(3 * x1 - x2)
+    # rho-1 = cos(a x1 + b x2): E = -(a, b) sin(.)/(a^2+b^2);  rho-1 = sin(.): E = +(a, b) cos(.)/(a^2+b^2)
+    E1 = -0.3 * 1 * np.sin(x1 + 2 * x2) / 5 + 0.2 * 3 * np.cos(3 * x1 - x2) / 10
+    E2 = -0.3 * 2 * np.sin(x1 + 2 * x2) / 5 - 0.2 * 1 * np.cos(3 * x1 - x2) / 10
+    E = orc.poisson(rho)
+    assert np.abs(E[0] - E1).max() < 5e-5 and np.abs(E[1] - E2).max() < 5e-5   # O(h^4) interpolation error
+
+
+# --------------------------------------------------------------- O7 diagnostics
+
+def test_p11_landau_initial_field_and_electric_energy():
+    """Landau IC: rho = 1 + eps cos(k x) -> E = -(eps/k) sin(k x) (sign pin) and electric
+    energy 1/2 int E^2 = 1/4 (eps/k)^2 L = 1.2566e-3 for eps=.01, k=.5, L=4 pi (1-d)."""
+    orc = O.Oracle(1, 1, [32, 2], 2, [0, 4 * math.pi, -1, 1])
+    x = orc.node_coords(0)
+    E = orc.poisson(1 + 0.01 * np.cos(0.5 * x))
+    assert np.abs(E[0] + 0.02 * np.sin(0.5 * x)).max() < 1e-6       # O(h^3) transfer error, k=2
+    ee = orc.electric_energy(E)
+    assert abs(ee - 0.25 * 0.02 ** 2 * 4 * math.pi) < 1e-9
+    assert abs(ee - 1.2566e-3) < 1e-7
+
+
+def test_mass_is_exact_for_polynomials():
+    orc = O.Oracle(1, 1, [3, 4], 1, [0.0, 2.0, -1.0, 3.0])
+    x, v = coords(orc)
+    f = (x ** 3)[None, :] * (v ** 2)[:, None]
+    assert abs(orc.mass(f) - (2 ** 4 / 4) * ((27 + 1) / 3)) < 1e-12
+
+
+# --------------------------------------------------------------- O6 Strang step
+
+def test_step_is_the_composition_of_its_parts():
+    """x(dt/2) -> rho -> E -> v(dt) -> x(dt/2), built from the separately pinned calls."""
+    cfg = W.CONFIGS[0]
+    orc = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    f0 = W.initial_data(cfg, coords(orc)).numpy()
+    g, rho, E = orc.step(f0, 0.1)
+    h = orc.advect_x(f0, 0.05)
+    rho2 = orc.density(h)
+    E2 = orc.poisson(rho2)
+    h = orc.advect_x(orc.advect_v(h, E2, 0.1), 0.05)
+    assert np.array_equal(rho, rho2) and np.array_equal(E, E2) and np.array_equal(g, h)
+
+
+def test_free_streaming_full_period_converges_at_order_k_plus_1():
+    """BASELINE.json: 'free streaming over a full period returns the initial data' -- reading N: to
+    O(h^{k+1}); x-advection only, one v node moving exactly one period in 10 fractional steps."""
+    k = 2
+    errs = []
+    for N in (8, 16, 32):
+        orc = O.Oracle(1, 1, [N, 1], 0 if False else k, [0.0, 1.0, 0.5, 1.5])
+        x, v = coords(orc)
+        f = np.sin(2 * math.pi * x)[None, :] * np.ones_like(v)[:, None]
+        g = f.copy()
+        # every v node returns after time 1/v; use the middle node (v = 1) and 10 steps of tau = 0.1
+        for _ in range(10):
+            g = orc.advect_x(g, 0.1)
+        mid = k // 2 if k % 2 == 0 else None
+        errs.append(np.abs(g[mid] - f[mid]).max())
+    assert math.log2(errs[0] / errs[1]) > k + 1 - 0.4 and math.log2(errs[1] / errs[2]) > k + 1 - 0.4
+
+
+def test_p12_linear_landau_damping_rate():
+    """PAPER.md:175-181 with BASELINE.json's gamma = -0.1533 (k = 0.5, eps = 0.01): the log-peaks of the
+    electric energy decay with slope 2*gamma; oscillation frequency omega = 1.4156 (peaks of E^2 are pi/omega
+    apart).  1x1v, 16 x-cells x 48 v-cells, k=2, dt=0.1, t <= 15 (before the numerical recurrence)."""
+    cfg = dict(name="landau1x1v", dim_x=1, dim_v=1, cells=[16, 48], degree=2,
+               domain=[0, 4 * math.pi, -6, 6], dt=0.1, ic="landau", ic_args=dict(eps=0.01, k=0.5, axes=[0]))
+    orc = O.Oracle(1, 1, cfg["cells"], 2, cfg["domain"], threads=O.lib().orc_max_threads())
+    f = W.initial_data(cfg, coords(orc)).numpy()
+    dt, nsteps = 0.1, 150
+    t, ee = [], []
+    for n in range(nsteps):
+        f, rho, E = orc.step(f, dt)
+        t.append((n + 0.5) * dt)                       # rho, E are taken at the middle of the step
+        ee.append(orc.electric_energy(E))
+    t, ee = np.array(t), np.array(ee)
+    pk = [i for i in range(1, nsteps - 1) if ee[i] > ee[i - 1] and ee[i] > ee[i + 1]]
+    assert len(pk) >= 5
+    # refine each peak with a parabola through log(ee) at the three samples
+    tp, lp = [], []
+    for i in pk:
+        y0, y1, y2 = np.log(ee[i - 1:i + 2])
+        den = y0 - 2 * y1 + y2
+        off = 0.5 * (y0 - y2) / den
+        tp.append(t[i] + off * dt)
+        lp.append(y1 - 0.25 * (y0 - y2) * off)
+    tp, lp = np.array(tp), np.array(lp)
+    slope = np.polyfit(tp, lp, 1)[0]
+    gamma = slope / 2
+    omega = math.pi / np.mean(np.diff(tp))
+    assert abs(gamma - (-0.1533)) < 0.02 * 0.1533 * 2, gamma
+    assert abs(omega - 1.4156) < 0.02 * 1.4156, omega
