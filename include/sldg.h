@@ -1,0 +1,147 @@
+/*
+ * sldg.h -- C-ABI of the B200-native (sm_100a) hot path of the split-step semi-Lagrangian
+ * discontinuous Galerkin (SLDG) Vlasov-Poisson solver of Einkemmer & Moriggl,
+ * arXiv 2110.14557.  Citations "P:line" are lines of the paper text;
+ * "reading X" refers to the table of readings in DESIGN.md section 3.
+ *
+ * Problem (eq. (1),(2)):  d_t f + v.grad_x f - E.grad_v f = 0,  E = -grad phi,
+ * -Laplace phi = 1 - rho,  rho = int f dv,  on a periodic box in d_x + d_v dimensions.
+ *
+ * Discretisation: per axis, N_a cells of k+1 Gauss-Legendre nodes; f holds the
+ * VALUES of the piecewise polynomial at the tensor-product nodes.
+ *
+ * LAYOUT OF f (reading E).  One flat fp64 array of |f| = prod_a D_a values, D_a = N_a (k+1):
+ *     flat index  n = n_0 + D_0 (n_1 + D_1 (n_2 + ...)),   axes ordered x_1..x_dx, v_1..v_dv
+ *     (x_1 fastest);  per-axis node index n_a = i_a (k+1) + j_a (cell i_a, node j_a);
+ *     value stored = f at coordinate lo_a + (i_a + xi_{j_a}) h_a,  h_a = (hi_a - lo_a)/N_a.
+ * rho is [X] with X = prod_{a<dx} D_a (same order); E is [dx][X], component-major.
+ *
+ * POINTERS are DEVICE pointers unless the argument is marked "host".  f, rho, E and the
+ * workspace are owned by the caller, must be 16-byte aligned (256 recommended) and must not
+ * alias each other.  The library never allocates O(|f|) memory itself.
+ *
+ * STREAM / SYNC.  All device work is enqueued on the stream given to sldg_set_stream (default:
+ * the legacy default stream).  No call synchronises, except those marked "synchronises".
+ *
+ * ERRORS.  Every int-returning call returns SLDG_OK (0) or a negative code; nothing throws,
+ * aborts or prints.  A context is not thread-safe.  There is NO CPU fallback: without a CUDA
+ * device every compute call returns SLDG_ECUDA.
+ */
+#ifndef SLDG_H
+#define SLDG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SLDG_OK 0
+#define SLDG_EINVAL (-1)        /* bad argument (NULL, dimension, degree, alignment, ...) */
+#define SLDG_ENOMEM (-2)        /* host or small device allocation failed                  */
+#define SLDG_ECUDA (-3)         /* a CUDA runtime call failed; see sldg_last_cuda_error    */
+#define SLDG_ENOWORKSPACE (-4)  /* sldg_set_workspace not called or too small              */
+
+#define SLDG_MAX_DIM 6
+#define SLDG_MAX_DEGREE 4
+
+typedef struct sldg_ctx sldg_ctx;
+
+/* ---- lifetime --------------------------------------------------------------------------
+ * sldg_create: problem statement of P:50-58.  dim_x in 1..3, dim_x <= dim_v <= 3 (the paper
+ * uses 2x2v, 2x3v, 3x3v; 1x1v and 1x2v are accepted as cheap test vehicles).
+ *   cells  (host) [dim_x+dim_v]   cells per axis, x axes first, each >= 1
+ *   degree k in 0..SLDG_MAX_DEGREE, the same on every axis (order k+1)
+ *   domain (host) [2(dim_x+dim_v)] lo_a, hi_a per axis, hi_a > lo_a; every axis is periodic
+ *                                  (reading C)
+ * Builds host tables (GL nodes/weights, polynomial coefficients of A(alpha), B(alpha)) and
+ * small device tables (O(sum_a D_a) bytes).  *out is written only on success. */
+int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree,
+                const double* domain);
+int sldg_destroy(sldg_ctx* ctx);
+
+/* stream = a cudaStream_t passed as void*; NULL selects the legacy default stream. */
+int sldg_set_stream(sldg_ctx* ctx, void* stream);
+
+/* Workspace: the second f buffer (|f| values), per-x-node shift tables, rho/E and DFT scratch.
+ * Caller-owned device memory, >= sldg_workspace_bytes(ctx) bytes, 256-byte aligned. */
+size_t sldg_workspace_bytes(const sldg_ctx* ctx);
+int sldg_set_workspace(sldg_ctx* ctx, void* dev, size_t bytes);
+
+/* ---- the hot path ------------------------------------ */
+
+/* a1+a2, steps 1a-1c: for d = 1..dim_x, in that order, f(x_d - v_d dt) by the 1-D
+ * SLDG update, eq. (3)
+ *     u_i <- A(alpha) u_{(i-s) mod N} + B(alpha) u_{(i-s-1) mod N},
+ *     delta = (v_d * dt) / h_{x_d},  s = floor(delta),  alpha = delta - s   (reading B)
+ * on every line along x_d; v_d is the coordinate of the line's v_d node.  `dt` is the actual
+ * time increment (a Strang half step passes Delta t / 2; reading J).  Result in f. */
+int sldg_advect_x(sldg_ctx* ctx, double* f, double dt);
+
+/* a5+a6, steps 3a-3c: for d = 1..dim_x, f(x, v_d + E_d(x) dt), i.e. the same update
+ * along v_d with delta = ((-E_d(x)) * dt) / h_{v_d} per x node (sign from eq. (1), reading H).
+ * Velocity axes beyond dim_x are not advected (reading D).  E is [dim_x][X].  Result in f. */
+int sldg_advect_v(sldg_ctx* ctx, double* f, const double* E, double dt);
+
+/* a3: rho[x] = sum_v (prod_d h_{v_d} w_{j_d}) f[x,v]. */
+int sldg_density(sldg_ctx* ctx, const double* f, double* rho);
+
+/* a4 (reading P1): -Laplace phi = 1 - rho periodic, E = -grad phi at the x
+ * nodes, by interpolation to the equidistant grid, a spectral solve, and interpolation back. */
+int sldg_poisson(sldg_ctx* ctx, const double* rho, double* E);
+
+/* a7, Strang splitting: advect_x(dt/2); density; poisson; advect_v(dt);
+ * advect_x(dt/2).  rho and E of the step stay in the workspace (sldg_last_rho / sldg_last_E). */
+int sldg_step(sldg_ctx* ctx, double* f, double dt);
+
+/* Same path driven from HOST memory: copies f_host (|f| doubles, pinned memory recommended) to
+ * the device buffer f_dev, runs nsteps Strang steps, copies the result back into f_host and the
+ * last E ([dim_x][X]) into E_host if it is not NULL.  Synchronises. */
+int sldg_step_host(sldg_ctx* ctx, double* f_host, double* f_dev, double* E_host, double dt,
+                   int nsteps);
+
+/* ---- helpers ---------------------------------------------------------------------------- */
+long long sldg_field_elems(const sldg_ctx* ctx);                 /* |f|                     */
+long long sldg_rho_elems(const sldg_ctx* ctx);                   /* X                       */
+int sldg_nodes(const sldg_ctx* ctx, int axis);                   /* D_axis, or SLDG_EINVAL  */
+/* host_out (host) [D_axis]: coordinates lo + (i + xi_j) h of the nodes of `axis`. */
+int sldg_node_coords(const sldg_ctx* ctx, int axis, double* host_out);
+/* device pointers into the workspace, valid after sldg_step / until the workspace changes */
+const double* sldg_last_rho(const sldg_ctx* ctx);
+const double* sldg_last_E(const sldg_ctx* ctx);
+/* 1/2 sum_x W_x |E(x)|^2 and sum_n W_n f_n; host_out is one host double.  Synchronise. */
+int sldg_electric_energy(sldg_ctx* ctx, const double* E, double* host_out);
+int sldg_mass(sldg_ctx* ctx, const double* f, double* host_out);
+const char* sldg_strerror(int code);
+int sldg_last_cuda_error(const sldg_ctx* ctx);                   /* cudaError_t as int      */
+
+/* A(alpha), B(alpha) as the library evaluates them on the host (row-major (k+1)x(k+1)). */
+int sldg_AB(const sldg_ctx* ctx, double alpha, double* hostA, double* hostB);
+
+/* Test hook: one sweep along `axis` with a caller-given shift table (in cells), through the
+ * production kernels.  delta_host (host): for an x axis, D_{v axis dim_x+axis} entries indexed
+ * by that axis' node; for a v axis, X entries indexed by flat x node.  Result in f. */
+int sldg_advect_axis(sldg_ctx* ctx, double* f, int axis, const double* delta_host);
+
+/* ---- instrumentation --------------------------------------------------------------------
+ * With timing on, every kernel launch is bracketed by CUDA events on the context's stream.
+ * Kinds: 0 = sweep along axis 0 (TMA/SMEM kernel), 1 = sweep along a slow axis, 2 = rho,
+ * 3 = Poisson/E, 4 = shift tables, 5 = copies.  sldg_timing_read synchronises, adds the elapsed
+ * times of all events recorded since the last read, and returns per kind the number of launches
+ * and the total milliseconds (arrays of SLDG_NKINDS entries, host). */
+#define SLDG_NKINDS 6
+int sldg_timing_enable(sldg_ctx* ctx, int on);
+int sldg_timing_read(sldg_ctx* ctx, long long* launches, double* ms);
+/* total kernel launches enqueued by this context since creation */
+long long sldg_launch_count(const sldg_ctx* ctx);
+/* Per-axis sweep time (ms) and launches accumulated since the last sldg_timing_read; arrays of
+ * SLDG_MAX_DIM entries (host).  Filled by sldg_timing_read; this call does not synchronise. */
+int sldg_timing_axis(const sldg_ctx* ctx, long long* launches, double* ms);
+
+/* Tuning knob (affects speed only, never results): see DESIGN.md section 5. */
+int sldg_set_option(sldg_ctx* ctx, const char* name, long long value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLDG_H */

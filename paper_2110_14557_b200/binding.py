@@ -1,0 +1,236 @@
+"""ctypes binding with the same names as include/sldg.h (argument marshalling only).
+
+PyTorch supplies device memory and the stream; nothing here computes.  This module never
+imports anything under oracle/.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBNAME = "libsldg_b200.so"
+
+NKINDS = 6
+MAX_DIM = 6
+KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies"]
+
+_vp, _dp, _ip, _ll = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_longlong
+_llp = C.POINTER(C.c_longlong)
+
+# name -> (restype, argtypes); every symbol include/sldg.h declares
+EXPORTS = {
+    "sldg_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, _ip, C.c_int, _dp]),
+    "sldg_destroy": (C.c_int, [_vp]),
+    "sldg_set_stream": (C.c_int, [_vp, _vp]),
+    "sldg_workspace_bytes": (C.c_size_t, [_vp]),
+    "sldg_set_workspace": (C.c_int, [_vp, _vp, C.c_size_t]),
+    "sldg_advect_x": (C.c_int, [_vp, _vp, C.c_double]),
+    "sldg_advect_v": (C.c_int, [_vp, _vp, _vp, C.c_double]),
+    "sldg_density": (C.c_int, [_vp, _vp, _vp]),
+    "sldg_poisson": (C.c_int, [_vp, _vp, _vp]),
+    "sldg_step": (C.c_int, [_vp, _vp, C.c_double]),
+    "sldg_step_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int]),
+    "sldg_field_elems": (_ll, [_vp]),
+    "sldg_rho_elems": (_ll, [_vp]),
+    "sldg_nodes": (C.c_int, [_vp, C.c_int]),
+    "sldg_node_coords": (C.c_int, [_vp, C.c_int, _dp]),
+    "sldg_last_rho": (_vp, [_vp]),
+    "sldg_last_E": (_vp, [_vp]),
+    "sldg_electric_energy": (C.c_int, [_vp, _vp, _dp]),
+    "sldg_mass": (C.c_int, [_vp, _vp, _dp]),
+    "sldg_strerror": (C.c_char_p, [C.c_int]),
+    "sldg_last_cuda_error": (C.c_int, [_vp]),
+    "sldg_AB": (C.c_int, [_vp, C.c_double, _dp, _dp]),
+    "sldg_advect_axis": (C.c_int, [_vp, _vp, C.c_int, _dp]),
+    "sldg_timing_enable": (C.c_int, [_vp, C.c_int]),
+    "sldg_timing_read": (C.c_int, [_vp, _llp, _dp]),
+    "sldg_launch_count": (_ll, [_vp]),
+    "sldg_timing_axis": (C.c_int, [_vp, _llp, _dp]),
+    "sldg_set_option": (C.c_int, [_vp, C.c_char_p, _ll]),
+}
+
+_lib = None
+
+
+class SldgError(RuntimeError):
+    pass
+
+
+def library_path():
+    return os.path.join(_HERE, _LIBNAME)
+
+
+def lib():
+    """Load the in-tree CUDA library.  Fails loudly if it was not built (no fallback)."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise SldgError(f"{path} is missing: run `python -m paper_2110_14557_b200.build` "
+                            "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(path)
+        for name, (res, args) in EXPORTS.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(code, ctx=None):
+    if code != 0:
+        msg = lib().sldg_strerror(code).decode()
+        if ctx is not None and code == -3:
+            msg += f" [cudaError {lib().sldg_last_cuda_error(ctx)}]"
+        raise SldgError(f"sldg error {code}: {msg}")
+
+
+def _ptr(t):
+    """Device (or pinned host) pointer of a contiguous float64 torch tensor."""
+    import torch
+    assert isinstance(t, torch.Tensor) and t.dtype == torch.float64 and t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+class Sldg:
+    """One solver context: sldg_create(dim_x, dim_v, cells, degree, domain) plus a torch-owned workspace."""
+
+    def __init__(self, dim_x, dim_v, cells, degree, domain, device="cuda:0", stream=None):
+        import torch
+        self._h = None
+        L = lib()
+        if not torch.cuda.is_available():
+            raise SldgError("no CUDA device: the SLDG path has no CPU fallback")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.dx, self.dv, self.d, self.k = dim_x, dim_v, dim_x + dim_v, degree
+        self.cells = [int(c) for c in cells]
+        dom = [float(v) for v in domain]
+        assert len(self.cells) == self.d and len(dom) == 2 * self.d
+        h = _vp()
+        _check(L.sldg_create(C.byref(h), dim_x, dim_v, (C.c_int * self.d)(*self.cells), degree,
+                             (C.c_double * (2 * self.d))(*dom)))
+        self._h = h
+        self.D = [L.sldg_nodes(h, a) for a in range(self.d)]
+        self.nf = L.sldg_field_elems(h)
+        self.X = L.sldg_rho_elems(h)
+        self.shape = tuple(reversed(self.D))
+        self.xshape = tuple(reversed(self.D[:dim_x]))
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.stream = st
+        _check(L.sldg_set_stream(h, C.c_void_p(st.cuda_stream)))
+        nbytes = L.sldg_workspace_bytes(h)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 256
+        _check(L.sldg_set_workspace(h, C.c_void_p(self.workspace.data_ptr() + off), nbytes), h)
+
+    def close(self):
+        if self._h is not None:
+            lib().sldg_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- helpers
+    def node_coords(self, axis):
+        import numpy as np
+        out = np.empty(self.D[axis])
+        _check(lib().sldg_node_coords(self._h, axis, out.ctypes.data_as(_dp)))
+        return out
+
+    def empty_field(self):
+        import torch
+        return torch.empty(self.shape, dtype=torch.float64, device=self.device)
+
+    def AB(self, alpha):
+        import numpy as np
+        n = self.k + 1
+        A, B = np.empty((n, n)), np.empty((n, n))
+        _check(lib().sldg_AB(self._h, float(alpha), A.ctypes.data_as(_dp), B.ctypes.data_as(_dp)))
+        return A, B
+
+    # ---- hot path (names as in include/sldg.h)
+    def advect_x(self, f, dt):
+        _check(lib().sldg_advect_x(self._h, _ptr(f), float(dt)), self._h)
+
+    def advect_v(self, f, E, dt):
+        _check(lib().sldg_advect_v(self._h, _ptr(f), _ptr(E), float(dt)), self._h)
+
+    def density(self, f, rho=None):
+        import torch
+        if rho is None:
+            rho = torch.empty(self.xshape, dtype=torch.float64, device=self.device)
+        _check(lib().sldg_density(self._h, _ptr(f), _ptr(rho)), self._h)
+        return rho
+
+    def poisson(self, rho, E=None):
+        import torch
+        if E is None:
+            E = torch.empty((self.dx,) + self.xshape, dtype=torch.float64, device=self.device)
+        _check(lib().sldg_poisson(self._h, _ptr(rho), _ptr(E)), self._h)
+        return E
+
+    def step(self, f, dt):
+        _check(lib().sldg_step(self._h, _ptr(f), float(dt)), self._h)
+
+    def step_host(self, f_host, f_dev, dt, nsteps=1, E_host=None):
+        _check(lib().sldg_step_host(self._h, _ptr(f_host), _ptr(f_dev),
+                                    _ptr(E_host) if E_host is not None else None, float(dt), int(nsteps)), self._h)
+
+    def advect_axis(self, f, axis, delta):
+        import numpy as np
+        d = np.ascontiguousarray(np.asarray(delta, dtype=np.float64))
+        want = self.D[self.dx + axis] if axis < self.dx else self.X
+        assert d.size == want, (d.size, want)
+        _check(lib().sldg_advect_axis(self._h, _ptr(f), int(axis), d.ctypes.data_as(_dp)), self._h)
+
+    def last_rho(self):
+        return self._view(lib().sldg_last_rho(self._h), self.xshape)
+
+    def last_E(self):
+        return self._view(lib().sldg_last_E(self._h), (self.dx,) + self.xshape)
+
+    def _view(self, ptr, shape):
+        """Copy of a workspace region as a torch tensor (device)."""
+        import torch
+        base = self.workspace.data_ptr()
+        off = ptr - base
+        n = 1
+        for s in shape:
+            n *= s
+        return self.workspace[off:off + 8 * n].view(torch.float64).reshape(shape).clone()
+
+    def electric_energy(self, E):
+        out = C.c_double()
+        _check(lib().sldg_electric_energy(self._h, _ptr(E), C.byref(out)), self._h)
+        return out.value
+
+    def mass(self, f):
+        out = C.c_double()
+        _check(lib().sldg_mass(self._h, _ptr(f), C.byref(out)), self._h)
+        return out.value
+
+    # ---- instrumentation
+    def timing_enable(self, on=True):
+        _check(lib().sldg_timing_enable(self._h, 1 if on else 0))
+
+    def timing_read(self):
+        """-> (per kind {name: (launches, ms)}, per axis [(launches, ms)])  since the last read; synchronises."""
+        n = (C.c_longlong * NKINDS)()
+        ms = (C.c_double * NKINDS)()
+        _check(lib().sldg_timing_read(self._h, n, ms), self._h)
+        an = (C.c_longlong * MAX_DIM)()
+        ams = (C.c_double * MAX_DIM)()
+        _check(lib().sldg_timing_axis(self._h, an, ams))
+        kinds = {KIND_NAMES[i]: (int(n[i]), float(ms[i])) for i in range(NKINDS)}
+        axes = [(int(an[i]), float(ams[i])) for i in range(self.d)]
+        return kinds, axes
+
+    def launch_count(self):
+        return int(lib().sldg_launch_count(self._h))
+
+    def set_option(self, name, value):
+        _check(lib().sldg_set_option(self._h, name.encode(), int(value)))

@@ -1,0 +1,42 @@
+"""Build the sm_100a SLDG library in-tree: paper_2110_14557_b200/libsldg_b200.so.
+
+nvcc cross-compiles without a GPU.  -lineinfo so ncu's source page maps to csrc/; static cudart so the
+library loads (and exports its symbols) on a box without a CUDA driver.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libsldg_b200.so")
+SOURCES = ["sldg_api.cu", "sldg_sweep_walk.cu", "sldg_sweep_tma.cu", "sldg_field.cu", "sldg_tables.cpp"]
+HEADERS = [os.path.join(CSRC, "sldg_internal.h"), os.path.join(HERE, "..", "include", "sldg.h")]
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+         "-Xcompiler", "-fPIC,-ffp-contract=off", "-cudart", "static"]
+
+
+def _stale(target, deps):
+    if not os.path.exists(target):
+        return True
+    t = os.path.getmtime(target)
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def build(force=False, verbose=False):
+    objs = []
+    extra = ["-Xptxas", "-v"] if verbose else []
+    for s in SOURCES:
+        src = os.path.join(CSRC, s)
+        obj = os.path.join(CSRC, os.path.splitext(s)[0] + ".o")
+        if force or _stale(obj, [src] + HEADERS):
+            subprocess.check_call([NVCC] + FLAGS + extra + ["-c", src, "-o", obj])
+        objs.append(obj)
+    if force or _stale(LIB, objs):
+        subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-o", LIB] + objs)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,559 @@
+// sldg_api.cu -- the C-ABI of include/sldg.h: context, host tables, launch sequencing.
+// No CPU fallback anywhere: every compute entry point enqueues sm_100a kernels or returns an error.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "sldg_internal.h"
+
+#define CK(call)                                                      \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) { c->last_cuda = (int)e_; return SLDG_ECUDA; } \
+    } while (0)
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------ instrumentation
+void sldg_ev_begin(sldg_ctx* c, int kind, int axis)
+{
+    if (!c->timing) return;
+    EventRec r;
+    if (!c->ev_free.empty()) { r = c->ev_free.back(); c->ev_free.pop_back(); }
+    else {
+        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+    }
+    r.kind = kind; r.axis = axis;
+    cudaEventRecord(r.a, c->stream);
+    c->ev.push_back(r);
+}
+void sldg_ev_end(sldg_ctx* c)
+{
+    if (!c->timing || c->ev.empty()) return;
+    cudaEventRecord(c->ev.back().b, c->stream);
+}
+
+// ------------------------------------------------------------------ layout of the workspace
+struct WsLayout { size_t f2, vS, vAB, Wv, rho, E, part, cplx[6], red, total; long long part_cap; };
+
+static WsLayout ws_layout(const sldg_ctx* c)
+{
+    WsLayout L;
+    size_t off = 0;
+    const size_t X = (size_t)c->X, NN2 = 2 * (size_t)c->K1 * c->K1;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    L.f2 = take((size_t)c->nf * 8);
+    L.vS = take(X * 4);
+    L.vAB = take(X * NN2 * 8);
+    L.Wv = take((size_t)c->V * 8);
+    L.rho = take(X * 8);
+    L.E = take(X * 8 * c->dx);
+    // rho partial sums: enough chunks to fill the GPU (see sldg_launch_density), at least 1
+    long long xtiles = (c->X + 255) / 256;
+    long long nchunk = ((long long)148 * 16 + xtiles - 1) / xtiles;
+    if (nchunk > c->V / 16) nchunk = c->V / 16;
+    if (nchunk < 1) nchunk = 1;
+    nchunk += 1;
+    L.part_cap = nchunk * c->X;
+    L.part = take((size_t)L.part_cap * 8);
+    for (int i = 0; i < 6; i++) L.cplx[i] = take(X * 8);
+    L.red = take(4096 * 8);
+    L.total = off;
+    return L;
+}
+
+// ------------------------------------------------------------------ lifetime
+extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree, const double* domain)
+{
+    if (!out || !cells || !domain) return SLDG_EINVAL;
+    if (dim_x < 1 || dim_x > 3 || dim_v < dim_x || dim_v > 3) return SLDG_EINVAL;
+    if (degree < 0 || degree > SLDG_MAX_DEGREE) return SLDG_EINVAL;
+    const int d = dim_x + dim_v;
+    for (int a = 0; a < d; a++) {
+        if (cells[a] < 1 || cells[a] >= (1 << 24)) return SLDG_EINVAL;
+        if (!(domain[2 * a + 1] > domain[2 * a])) return SLDG_EINVAL;
+    }
+    sldg_ctx* c = new (std::nothrow) sldg_ctx();
+    if (!c) return SLDG_ENOMEM;
+    c->dx = dim_x; c->dv = dim_v; c->d = d; c->k = degree; c->K1 = degree + 1;
+    c->nf = 1; c->X = 1; c->V = 1;
+    for (int a = 0; a < d; a++) {
+        c->cells[a] = cells[a];
+        c->D[a] = (long long)cells[a] * c->K1;
+        c->lo[a] = domain[2 * a]; c->hi[a] = domain[2 * a + 1];
+        c->h[a] = (c->hi[a] - c->lo[a]) / (double)cells[a];
+        c->nf *= c->D[a];
+        if (a < dim_x) c->X *= c->D[a]; else c->V *= c->D[a];
+    }
+    sldg_gl_rule(c->K1, c->xi, c->w);
+    sldg_build_poly(c->k, c->xi, c->w, &c->poly);
+    c->stream = 0; c->last_cuda = 0; c->sm_count = 148;
+    c->ws = nullptr; c->ws_bytes = 0; c->ws_ready = false;
+    c->timing = false; c->launches = 0;
+    memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
+    memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
+    c->opt_tile_bytes = 16384; c->opt_walk_block = 256; c->opt_walk_vec = 0;
+    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->dWx[a] = nullptr; }
+    for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
+    c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
+    c->dScalar = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
+
+    // device side: needs a CUDA device.  Without one the context is unusable -> fail loudly.
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) {
+        int sm = 0;
+        if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sm > 0) c->sm_count = sm;
+        e = sldg_upload_poly(&c->poly);
+    }
+    const size_t NN2 = 2 * (size_t)c->K1 * c->K1;
+    long long maxD = 0;
+    for (int a = 0; a < d; a++) if (c->D[a] > maxD) maxD = c->D[a];
+    c->hcap = maxD;
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->hS, (size_t)maxD * 4);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->hAB, (size_t)maxD * NN2 * 8);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->dScalar, 8);
+    for (int a = 0; a < dim_x && e == cudaSuccess; a++) {
+        long long Ds = c->D[dim_x + a];
+        e = cudaMalloc((void**)&c->dS[a], (size_t)Ds * 4);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&c->dAB[a], (size_t)Ds * NN2 * 8);
+    }
+    if (e == cudaSuccess) { e = cudaMalloc((void**)&c->dS_hook, (size_t)maxD * 4); }
+    if (e == cudaSuccess) { e = cudaMalloc((void**)&c->dAB_hook, (size_t)maxD * NN2 * 8); c->hook_cap = maxD; }
+    // per-axis quadrature weights h_a w_j
+    for (int a = 0; a < d && e == cudaSuccess; a++) {
+        std::vector<double> wa((size_t)c->D[a]);
+        for (long long n = 0; n < c->D[a]; n++) wa[(size_t)n] = c->h[a] * c->w[n % c->K1];
+        e = cudaMalloc((void**)&c->dWx[a], (size_t)c->D[a] * 8);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dWx[a], wa.data(), (size_t)c->D[a] * 8, cudaMemcpyHostToDevice);
+    }
+    // Poisson tables
+    for (int a = 0; a < dim_x && e == cudaSuccess; a++) {
+        const long long D = c->D[a];
+        std::vector<double> fw((size_t)(2 * D * D)), iv((size_t)(2 * D * D)), kap((size_t)D);
+        sldg_build_dft(c->k, c->xi, c->cells[a], fw.data(), iv.data());
+        const long double twopi = 6.28318530717958647692528676655900577L;
+        for (long long m = 0; m < D; m++) {
+            long long mm = (2 * m < D) ? m : m - D;
+            kap[(size_t)m] = (double)(twopi * (long double)mm / (long double)(c->hi[a] - c->lo[a]));
+        }
+        e = cudaMalloc((void**)&c->dFwdT[a], (size_t)(2 * D * D) * 8);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&c->dInvT[a], (size_t)(2 * D * D) * 8);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&c->dKap[a], (size_t)D * 8);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dFwdT[a], fw.data(), (size_t)(2 * D * D) * 8, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dInvT[a], iv.data(), (size_t)(2 * D * D) * 8, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(c->dKap[a], kap.data(), (size_t)D * 8, cudaMemcpyHostToDevice);
+    }
+    if (e != cudaSuccess) {
+        c->last_cuda = (int)e;
+        sldg_destroy(c);
+        return (e == cudaErrorMemoryAllocation) ? SLDG_ENOMEM : SLDG_ECUDA;
+    }
+    *out = c;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_destroy(sldg_ctx* c)
+{
+    if (!c) return SLDG_EINVAL;
+    for (int a = 0; a < SLDG_MAX_DIM; a++) {
+        if (c->dS[a]) cudaFree(c->dS[a]);
+        if (c->dAB[a]) cudaFree(c->dAB[a]);
+        if (c->dWx[a]) cudaFree(c->dWx[a]);
+    }
+    for (int a = 0; a < 3; a++) {
+        if (c->dFwdT[a]) cudaFree(c->dFwdT[a]);
+        if (c->dInvT[a]) cudaFree(c->dInvT[a]);
+        if (c->dKap[a]) cudaFree(c->dKap[a]);
+    }
+    if (c->dS_hook) cudaFree(c->dS_hook);
+    if (c->dAB_hook) cudaFree(c->dAB_hook);
+    if (c->dScalar) cudaFree(c->dScalar);
+    if (c->hS) cudaFreeHost(c->hS);
+    if (c->hAB) cudaFreeHost(c->hAB);
+    for (auto& r : c->ev) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto& r : c->ev_free) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    delete c;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_set_stream(sldg_ctx* c, void* stream)
+{
+    if (!c) return SLDG_EINVAL;
+    c->stream = (cudaStream_t)stream;
+    return SLDG_OK;
+}
+
+extern "C" size_t sldg_workspace_bytes(const sldg_ctx* c) { return c ? ws_layout(c).total : 0; }
+
+extern "C" int sldg_set_workspace(sldg_ctx* c, void* dev, size_t bytes)
+{
+    if (!c || !dev) return SLDG_EINVAL;
+    if (((uintptr_t)dev) & 255) return SLDG_EINVAL;
+    WsLayout L = ws_layout(c);
+    if (bytes < L.total) return SLDG_ENOWORKSPACE;
+    char* b = (char*)dev;
+    c->ws = b; c->ws_bytes = bytes;
+    c->f2 = (double*)(b + L.f2); c->vS = (int*)(b + L.vS); c->vAB = (double*)(b + L.vAB);
+    c->Wv = (double*)(b + L.Wv); c->rho = (double*)(b + L.rho); c->E = (double*)(b + L.E);
+    c->part = (double*)(b + L.part); c->part_cap = L.part_cap;
+    for (int i = 0; i < 6; i++) c->cplx[i] = (double*)(b + L.cplx[i]);
+    c->red = (double*)(b + L.red);
+    sldg_ev_begin(c, KIND_TABLE, -1);
+    cudaError_t e = sldg_launch_wv(c);
+    sldg_ev_end(c);
+    c->launches++;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; c->ws_ready = false; return SLDG_ECUDA; }
+    c->ws_ready = true;
+    return SLDG_OK;
+}
+
+// ------------------------------------------------------------------ geometry / tables
+static SweepGeom geom_of(const sldg_ctx* c, int axis)
+{
+    SweepGeom g;
+    g.inner = 1; g.outer = 1;
+    for (int b = 0; b < axis; b++) g.inner *= c->D[b];
+    for (int b = axis + 1; b < c->d; b++) g.outer *= c->D[b];
+    g.N = c->cells[axis]; g.K1 = c->K1;
+    if (axis < c->dx) {
+        g.mode = 0;
+        int sa = c->dx + axis;
+        g.sdiv = 1;
+        for (int b = axis + 1; b < sa; b++) g.sdiv *= c->D[b];
+        g.smod = c->D[sa];
+    } else {
+        g.mode = 1; g.sdiv = 1; g.smod = c->X;
+    }
+    return g;
+}
+
+// host: split delta into (s mod N | copy bit) and A(alpha), B(alpha)   (reading B, O)
+static void host_entry(const sldg_ctx* c, double delta, int N, int* S, double* AB)
+{
+    const int NN = c->K1 * c->K1;
+    double sd = floor(delta);
+    double alpha = delta - sd;
+    int s = (int)fmod(sd, (double)N);
+    if (s < 0) s += N;
+    if (alpha == 0.0) {
+        *S = s | SLDG_COPY_BIT;
+        for (int m = 0; m < NN; m++) { AB[m] = (m % (c->K1 + 1) == 0) ? 1.0 : 0.0; AB[NN + m] = 0.0; }
+    } else {
+        *S = s;
+        sldg_eval_AB_host(&c->poly, c->k, alpha, AB, AB + NN);
+    }
+}
+
+static int upload_table(sldg_ctx* c, const double* delta, long long n, int N, int* dS, double* dAB)
+{
+    const size_t NN2 = 2 * (size_t)c->K1 * c->K1;
+    if (n > c->hcap) return SLDG_EINVAL;
+    // the pinned staging buffers may still be in flight from a previous upload on this stream
+    CK(cudaStreamSynchronize(c->stream));
+    for (long long i = 0; i < n; i++) host_entry(c, delta[i], N, c->hS + i, c->hAB + (size_t)i * NN2);
+    sldg_ev_begin(c, KIND_COPY, -1);
+    CK(cudaMemcpyAsync(dS, c->hS, (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(dAB, c->hAB, (size_t)n * NN2 * 8, cudaMemcpyHostToDevice, c->stream));
+    sldg_ev_end(c);
+    return SLDG_OK;
+}
+
+static int run_sweep(sldg_ctx* c, const double* fin, double* fout, int axis, const ShiftTable& t)
+{
+    SweepGeom g = geom_of(c, axis);
+    cudaError_t e;
+    if (g.inner == 1) {
+        sldg_ev_begin(c, KIND_SWEEP0, axis);
+        e = sldg_launch_sweep_tma(c, fin, fout, g, t);
+    } else {
+        if (fin == fout) return SLDG_EINVAL;
+        sldg_ev_begin(c, KIND_SWEEP, axis);
+        e = sldg_launch_sweep_walk(c, fin, fout, g, t);
+    }
+    sldg_ev_end(c);
+    c->launches++;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    return SLDG_OK;
+}
+
+static int copy_back(sldg_ctx* c, double* dst, const double* src)
+{
+    sldg_ev_begin(c, KIND_COPY, -1);
+    cudaError_t e = cudaMemcpyAsync(dst, src, (size_t)c->nf * 8, cudaMemcpyDeviceToDevice, c->stream);
+    sldg_ev_end(c);
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    return SLDG_OK;
+}
+
+static int check_f(const sldg_ctx* c, const void* f)
+{
+    if (!c || !f) return SLDG_EINVAL;
+    if (((uintptr_t)f) & 15) return SLDG_EINVAL;
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    return SLDG_OK;
+}
+
+// Run sweeps along axes[0..n) in order, result in f.  The sweep along axis 0 (if present) runs in place; the
+// others ping-pong f <-> f2; an odd number of ping-pong sweeps ends with a device copy back into f.
+static int run_sweeps(sldg_ctx* c, double* f, const int* axes, const ShiftTable* tabs, int n,
+                      int (*prep)(sldg_ctx*, int, void*), void* prep_arg)
+{
+    double* cur = f;
+    double* oth = c->f2;
+    for (int i = 0; i < n; i++) {
+        if (prep) { int r = prep(c, i, prep_arg); if (r) return r; }
+        SweepGeom g = geom_of(c, axes[i]);
+        if (g.inner == 1) {
+            int r = run_sweep(c, cur, cur, axes[i], tabs[i]);
+            if (r) return r;
+        } else {
+            int r = run_sweep(c, cur, oth, axes[i], tabs[i]);
+            if (r) return r;
+            double* t = cur; cur = oth; oth = t;
+        }
+    }
+    if (cur != f) return copy_back(c, f, cur);
+    return SLDG_OK;
+}
+
+// ------------------------------------------------------------------ hot path
+extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    int axes[3];
+    ShiftTable tabs[3];
+    const long long NN2 = 2LL * c->K1 * c->K1;
+    for (int a = 0; a < c->dx; a++) {
+        const int b = c->dx + a;
+        if (!c->tab_valid[a] || c->tab_tau[a] != dt) {
+            std::vector<double> delta((size_t)c->D[b]);
+            for (long long n = 0; n < c->D[b]; n++) {
+                // node coordinate lo + (i + xi_j) h, then delta = (v * dt) / h_x   (reading O3)
+                volatile double cell = (double)(n / c->K1) + c->xi[n % c->K1];
+                volatile double off = cell * c->h[b];
+                volatile double v = c->lo[b] + off;
+                volatile double vt = v * dt;
+                delta[(size_t)n] = vt / c->h[a];
+            }
+            r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
+            if (r) return r;
+            c->tab_valid[a] = true; c->tab_tau[a] = dt;
+        }
+        axes[a] = a;
+        tabs[a].S = c->dS[a]; tabs[a].AB = c->dAB[a]; tabs[a].strideIdx = NN2; tabs[a].strideM = 1;
+    }
+    return run_sweeps(c, f, axes, tabs, c->dx, nullptr, nullptr);
+}
+
+struct VPrep { const double* E; double dt; };
+static int vprep(sldg_ctx* c, int i, void* arg)
+{
+    VPrep* p = (VPrep*)arg;
+    const int a = c->dx + i;
+    sldg_ev_begin(c, KIND_TABLE, a);
+    cudaError_t e = sldg_launch_vtable(c, p->E + (long long)i * c->X, p->dt, c->h[a], c->cells[a], c->vS, c->vAB);
+    sldg_ev_end(c);
+    c->launches++;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    return SLDG_OK;
+}
+
+extern "C" int sldg_advect_v(sldg_ctx* c, double* f, const double* E, double dt)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    if (!E) return SLDG_EINVAL;
+    int axes[3];
+    ShiftTable tabs[3];
+    for (int i = 0; i < c->dx; i++) {
+        axes[i] = c->dx + i;
+        tabs[i].S = c->vS; tabs[i].AB = c->vAB; tabs[i].strideIdx = 1; tabs[i].strideM = c->X;
+    }
+    VPrep p = {E, dt};
+    return run_sweeps(c, f, axes, tabs, c->dx, vprep, &p);
+}
+
+extern "C" int sldg_density(sldg_ctx* c, const double* f, double* rho)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    if (!rho) return SLDG_EINVAL;
+    sldg_ev_begin(c, KIND_RHO, -1);
+    cudaError_t e = sldg_launch_density(c, f, rho);
+    sldg_ev_end(c);
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    return SLDG_OK;
+}
+
+extern "C" int sldg_poisson(sldg_ctx* c, const double* rho, double* E)
+{
+    if (!c || !rho || !E) return SLDG_EINVAL;
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    sldg_ev_begin(c, KIND_POISSON, -1);
+    cudaError_t e = sldg_launch_poisson(c, rho, E);
+    sldg_ev_end(c);
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    return SLDG_OK;
+}
+
+extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    if ((r = sldg_advect_x(c, f, dt / 2.0))) return r;
+    if ((r = sldg_density(c, f, c->rho))) return r;
+    if ((r = sldg_poisson(c, c->rho, c->E))) return r;
+    if ((r = sldg_advect_v(c, f, c->E, dt))) return r;
+    return sldg_advect_x(c, f, dt / 2.0);
+}
+
+extern "C" int sldg_step_host(sldg_ctx* c, double* f_host, double* f_dev, double* E_host, double dt, int nsteps)
+{
+    int r = check_f(c, f_dev);
+    if (r) return r;
+    if (!f_host || nsteps < 0) return SLDG_EINVAL;
+    CK(cudaMemcpyAsync(f_dev, f_host, (size_t)c->nf * 8, cudaMemcpyHostToDevice, c->stream));
+    for (int s = 0; s < nsteps; s++)
+        if ((r = sldg_step(c, f_dev, dt))) return r;
+    CK(cudaMemcpyAsync(f_host, f_dev, (size_t)c->nf * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (E_host) CK(cudaMemcpyAsync(E_host, c->E, (size_t)c->X * 8 * c->dx, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return SLDG_OK;
+}
+
+extern "C" int sldg_advect_axis(sldg_ctx* c, double* f, int axis, const double* delta_host)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    if (!delta_host || axis < 0 || axis >= c->d) return SLDG_EINVAL;
+    ShiftTable t;
+    const long long NN2 = 2LL * c->K1 * c->K1;
+    if (axis < c->dx) {
+        const int b = c->dx + axis;
+        r = upload_table(c, delta_host, c->D[b], c->cells[axis], c->dS_hook, c->dAB_hook);
+        if (r) return r;
+        t.S = c->dS_hook; t.AB = c->dAB_hook; t.strideIdx = NN2; t.strideM = 1;
+    } else {
+        // per-x-node table, built on the host with the same host routine, stored SoA like the device-built one
+        const long long X = c->X;
+        const int NN = c->K1 * c->K1;
+        std::vector<int> S((size_t)X);
+        std::vector<double> AB((size_t)(X * NN2)), ent((size_t)NN2);
+        for (long long x = 0; x < X; x++) {
+            host_entry(c, delta_host[x], c->cells[axis], &S[(size_t)x], ent.data());
+            for (int m = 0; m < 2 * NN; m++) AB[(size_t)((long long)m * X + x)] = ent[(size_t)m];
+        }
+        CK(cudaStreamSynchronize(c->stream));
+        CK(cudaMemcpy(c->vS, S.data(), (size_t)X * 4, cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(c->vAB, AB.data(), (size_t)(X * NN2) * 8, cudaMemcpyHostToDevice));
+        t.S = c->vS; t.AB = c->vAB; t.strideIdx = 1; t.strideM = X;
+    }
+    int axes[1] = {axis};
+    return run_sweeps(c, f, axes, &t, 1, nullptr, nullptr);
+}
+
+// ------------------------------------------------------------------ helpers
+extern "C" long long sldg_field_elems(const sldg_ctx* c) { return c ? c->nf : 0; }
+extern "C" long long sldg_rho_elems(const sldg_ctx* c) { return c ? c->X : 0; }
+extern "C" int sldg_nodes(const sldg_ctx* c, int axis)
+{
+    if (!c || axis < 0 || axis >= c->d) return SLDG_EINVAL;
+    return (int)c->D[axis];
+}
+extern "C" int sldg_node_coords(const sldg_ctx* c, int axis, double* host_out)
+{
+    if (!c || !host_out || axis < 0 || axis >= c->d) return SLDG_EINVAL;
+    for (long long n = 0; n < c->D[axis]; n++) {
+        volatile double cell = (double)(n / c->K1) + c->xi[n % c->K1];
+        volatile double off = cell * c->h[axis];
+        host_out[n] = c->lo[axis] + off;
+    }
+    return SLDG_OK;
+}
+extern "C" const double* sldg_last_rho(const sldg_ctx* c) { return (c && c->ws_ready) ? c->rho : nullptr; }
+extern "C" const double* sldg_last_E(const sldg_ctx* c) { return (c && c->ws_ready) ? c->E : nullptr; }
+
+static int scalar_out(sldg_ctx* c, cudaError_t e, double* host_out)
+{
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    CK(cudaMemcpyAsync(host_out, c->dScalar, 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return SLDG_OK;
+}
+extern "C" int sldg_electric_energy(sldg_ctx* c, const double* E, double* host_out)
+{
+    if (!c || !E || !host_out) return SLDG_EINVAL;
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    return scalar_out(c, sldg_launch_energy(c, E, c->dScalar), host_out);
+}
+extern "C" int sldg_mass(sldg_ctx* c, const double* f, double* host_out)
+{
+    if (!c || !f || !host_out) return SLDG_EINVAL;
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    return scalar_out(c, sldg_launch_mass(c, f, c->dScalar), host_out);
+}
+extern "C" const char* sldg_strerror(int code)
+{
+    switch (code) {
+    case SLDG_OK: return "ok";
+    case SLDG_EINVAL: return "invalid argument";
+    case SLDG_ENOMEM: return "out of memory";
+    case SLDG_ECUDA: return "CUDA runtime error (see sldg_last_cuda_error); no CPU fallback exists";
+    case SLDG_ENOWORKSPACE: return "workspace missing or too small";
+    }
+    return "unknown error";
+}
+extern "C" int sldg_last_cuda_error(const sldg_ctx* c) { return c ? c->last_cuda : 0; }
+
+extern "C" int sldg_AB(const sldg_ctx* c, double alpha, double* A, double* B)
+{
+    if (!c || !A || !B || !(alpha >= 0.0 && alpha <= 1.0)) return SLDG_EINVAL;
+    sldg_eval_AB_host(&c->poly, c->k, alpha, A, B);
+    return SLDG_OK;
+}
+
+// ------------------------------------------------------------------ instrumentation API
+extern "C" int sldg_timing_enable(sldg_ctx* c, int on)
+{
+    if (!c) return SLDG_EINVAL;
+    c->timing = on != 0;
+    return SLDG_OK;
+}
+extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
+{
+    if (!c || !launches || !ms) return SLDG_EINVAL;
+    CK(cudaStreamSynchronize(c->stream));
+    memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
+    memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
+    for (auto& r : c->ev) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
+            c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
+            if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
+        }
+        c->ev_free.push_back(r);
+    }
+    c->ev.clear();
+    for (int i = 0; i < SLDG_NKINDS; i++) { launches[i] = c->t_launch[i]; ms[i] = c->t_ms[i]; }
+    return SLDG_OK;
+}
+extern "C" int sldg_timing_axis(const sldg_ctx* c, long long* launches, double* ms)
+{
+    if (!c || !launches || !ms) return SLDG_EINVAL;
+    for (int i = 0; i < SLDG_MAX_DIM; i++) { launches[i] = c->a_launch[i]; ms[i] = c->a_ms[i]; }
+    return SLDG_OK;
+}
+extern "C" long long sldg_launch_count(const sldg_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
+{
+    if (!c || !name) return SLDG_EINVAL;
+    if (!strcmp(name, "tile_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_tile_bytes = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "walk_block")) { if (value < 32 || value > 256 || (value & 31)) return SLDG_EINVAL; c->opt_walk_block = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "walk_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_walk_vec = (int)value; return SLDG_OK; }
+    return SLDG_EINVAL;
+}

@@ -1,0 +1,311 @@
+// sldg_field.cu -- rho reduction, Poisson/E solve, v-sweep shift tables and diagnostics, sm_100a.
+//
+//  rho[x] = sum_v W_v f[x,v]   HBM-bound: one read of f
+//  -Laplace phi = 1 - rho, E = -grad phi  (reading P1)     tiny, latency-bound
+//  per-x-node shift tables of the v-sweeps
+#include "sldg_internal.h"
+
+__constant__ ABPoly c_poly;
+
+cudaError_t sldg_upload_poly(const ABPoly* p) { return cudaMemcpyToSymbol(c_poly, p, sizeof(ABPoly)); }
+
+namespace {
+
+// ------------------------------------------------------------------ v-sweep shift table (row a5)
+// delta = ((-E) * tau) / h_v in exactly this operation order (reading O3); s = floor(delta), alpha = delta - s.
+// A(alpha), B(alpha) by Horner on the polynomial coefficients.  Output SoA: AB[m][X].
+template <int K1>
+__global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double hv, int N, long long X,
+                              int* __restrict__ S, double* __restrict__ AB)
+{
+    long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= X) return;
+    constexpr int NN = K1 * K1, DEG = 2 * K1 - 1;
+    double delta = __ddiv_rn(__dmul_rn(-Ed[x], tau), hv);
+    double sd = floor(delta);
+    double alpha = delta - sd;
+    double sm = fmod(sd, (double)N);
+    int s = (int)sm;
+    if (s < 0) s += N;
+    bool cp = (alpha == 0.0);
+    S[x] = s | (cp ? SLDG_COPY_BIT : 0);
+#pragma unroll
+    for (int m = 0; m < NN; m++) {
+        double a = c_poly.c[0][m][DEG], b = c_poly.c[1][m][DEG];
+#pragma unroll
+        for (int t = DEG - 1; t >= 0; t--) {
+            a = fma(a, alpha, c_poly.c[0][m][t]);
+            b = fma(b, alpha, c_poly.c[1][m][t]);
+        }
+        if (cp) { a = (m % (K1 + 1) == 0) ? 1.0 : 0.0; b = 0.0; }
+        AB[(long long)m * X + x] = a;
+        AB[(long long)(NN + m) * X + x] = b;
+    }
+}
+
+// ------------------------------------------------------------------ velocity quadrature weights W_v
+struct WvParams { int dv; long long Dv[3]; const double* w[3]; long long V; };
+__global__ void wv_kernel(WvParams P, double* __restrict__ Wv)
+{
+    long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= P.V) return;
+    long long r = v;
+    double wv = 1.0;
+    for (int a = 0; a < P.dv; a++) {
+        long long n = r % P.Dv[a]; r /= P.Dv[a];
+        wv *= P.w[a][n];
+    }
+    Wv[v] = wv;
+}
+
+// ------------------------------------------------------------------ rho (row a3)
+// f seen as [V][X] (X contiguous).  Block = 128 threads x 2 values along x; grid.y splits V into chunks.
+// Each chunk writes a partial sum; a second kernel adds the partials in a fixed order (deterministic).
+template <int VEC>
+__global__ void __launch_bounds__(128) rho_partial_kernel(const double* __restrict__ f, const double* __restrict__ Wv,
+                                                          long long X, long long V, long long vchunk,
+                                                          double* __restrict__ part)
+{
+    long long x = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+    if (x >= X) return;
+    long long v0 = (long long)blockIdx.y * vchunk;
+    long long v1 = v0 + vchunk; if (v1 > V) v1 = V;
+    double acc[VEC] = {0};
+    constexpr int U = 8;
+    long long v = v0;
+    for (; v + U <= v1; v += U) {
+        double t[U][VEC];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const double* p = f + (v + u) * X + x;
+            if (VEC == 2) { double2 d = __ldcs(reinterpret_cast<const double2*>(p)); t[u][0] = d.x; t[u][VEC - 1] = d.y; }
+            else t[u][0] = __ldcs(p);
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            double wv = __ldg(Wv + v + u);
+#pragma unroll
+            for (int e = 0; e < VEC; e++) acc[e] = fma(wv, t[u][e], acc[e]);
+        }
+    }
+    for (; v < v1; v++) {
+        double wv = __ldg(Wv + v);
+#pragma unroll
+        for (int e = 0; e < VEC; e++) acc[e] = fma(wv, __ldcs(f + v * X + x + e), acc[e]);
+    }
+#pragma unroll
+    for (int e = 0; e < VEC; e++) part[(long long)blockIdx.y * X + x + e] = acc[e];
+}
+
+__global__ void rho_final_kernel(const double* __restrict__ part, long long X, int nchunk, double* __restrict__ rho)
+{
+    long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= X) return;
+    double acc = 0.0;
+    for (int c = 0; c < nchunk; c++) acc += part[(long long)c * X + x];
+    rho[x] = acc;
+}
+
+// ------------------------------------------------------------------ Poisson / E (row a4)
+// out[q][m][p] = sum_n M[m][n] in[q][n][p], complex; M stored transposed MT[n][m] (re block, then im block).
+// HAS_IM = 0: the input is real.
+template <int HAS_IM>
+__global__ void apply_axis_kernel(const double* __restrict__ inr, const double* __restrict__ ini,
+                                  const double* __restrict__ MT, long long D, long long inner, long long total,
+                                  double* __restrict__ outr, double* __restrict__ outi)
+{
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= total) return;
+    long long p = t % inner, m = (t / inner) % D, q = t / (inner * D);
+    const double* Mr = MT + m; const double* Mi = MT + D * D + m;
+    const double* xr = inr + q * D * inner + p;
+    const double* xi = HAS_IM ? ini + q * D * inner + p : nullptr;
+    double ar = 0.0, ai = 0.0;
+    for (long long n = 0; n < D; n++) {
+        double mr = __ldg(Mr + n * D), mi = __ldg(Mi + n * D);
+        double vr = xr[n * inner];
+        ar = fma(mr, vr, ar); ai = fma(mi, vr, ai);
+        if (HAS_IM) {
+            double vi = xi[n * inner];
+            ar = fma(-mi, vi, ar); ai = fma(mr, vi, ai);
+        }
+    }
+    outr[t] = ar;
+    if (outi) outi[t] = ai;
+}
+
+// E^_d = i kappa_d rho^ / |kappa|^2 (kappa != 0), 0 at kappa = 0; kappa_d := 0 at the Nyquist index of an even axis.
+struct SpecParams { int dx; long long D[3]; const double* kap[3]; long long X; };
+__global__ void spectral_kernel(SpecParams P, int d, const double* __restrict__ rr, const double* __restrict__ ri,
+                                double* __restrict__ er, double* __restrict__ ei)
+{
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= P.X) return;
+    long long r = t;
+    double k2 = 0.0, kd = 0.0;
+    for (int a = 0; a < P.dx; a++) {
+        long long m = r % P.D[a]; r /= P.D[a];
+        double kap = P.kap[a][m];
+        k2 += kap * kap;
+        if (a == d) kd = (2 * m == P.D[a]) ? 0.0 : kap;
+    }
+    if (k2 == 0.0) { er[t] = 0.0; ei[t] = 0.0; }
+    else { er[t] = -kd * ri[t] / k2; ei[t] = kd * rr[t] / k2; }
+}
+
+// ------------------------------------------------------------------ diagnostics
+struct WgtParams { int nd; long long D[SLDG_MAX_DIM]; const double* w[SLDG_MAX_DIM]; long long total; };
+
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double sh[32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        v = (lane < (blockDim.x >> 5)) ? sh[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    }
+    return v;
+}
+
+// partial[b] = sum over a grid-stride slice of  W_n * g(n);  NCOMP = 0: g = f[n];  NCOMP > 0: g = sum_d E_d[n]^2
+__global__ void __launch_bounds__(256) weighted_sum_kernel(WgtParams P, const double* __restrict__ a, int ncomp,
+                                                           double* __restrict__ partial)
+{
+    double acc = 0.0;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < P.total;
+         t += (long long)gridDim.x * blockDim.x) {
+        long long r = t;
+        double wn = 1.0;
+        for (int d = 0; d < P.nd; d++) { long long n = r % P.D[d]; r /= P.D[d]; wn *= P.w[d][n]; }
+        double g;
+        if (ncomp == 0) g = a[t];
+        else { g = 0.0; for (int d = 0; d < ncomp; d++) { double e = a[(long long)d * P.total + t]; g = fma(e, e, g); } }
+        acc = fma(wn, g, acc);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+}
+__global__ void __launch_bounds__(256) final_sum_kernel(const double* __restrict__ partial, int n, double scale,
+                                                        double* __restrict__ out)
+{
+    double acc = 0.0;
+    for (int t = threadIdx.x; t < n; t += blockDim.x) acc += partial[t];
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) out[0] = acc * scale;
+}
+
+}  // namespace
+
+cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB)
+{
+    int block = 128;
+    unsigned grid = (unsigned)((c->X + block - 1) / block);
+    switch (c->K1) {
+    case 1: vtable_kernel<1><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 2: vtable_kernel<2><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 3: vtable_kernel<3><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 4: vtable_kernel<4><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 5: vtable_kernel<5><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t sldg_launch_wv(sldg_ctx* c)
+{
+    WvParams P;
+    P.dv = c->dv; P.V = c->V;
+    for (int a = 0; a < c->dv; a++) { P.Dv[a] = c->D[c->dx + a]; P.w[a] = c->dWx[c->dx + a]; }
+    int block = 256;
+    wv_kernel<<<(unsigned)((c->V + block - 1) / block), block, 0, c->stream>>>(P, c->Wv);
+    return cudaGetLastError();
+}
+
+cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho)
+{
+    const long long X = c->X, V = c->V;
+    int vec = ((X & 1) == 0 && (((uintptr_t)f) & 15) == 0) ? 2 : 1;
+    long long xtiles = (X + 128LL * vec - 1) / (128LL * vec);
+    long long want = (long long)c->sm_count * 16;
+    long long nchunk = (want + xtiles - 1) / xtiles;
+    if (nchunk > V / 16) nchunk = V / 16;
+    if (nchunk > c->part_cap / X) nchunk = c->part_cap / X;
+    if (nchunk > 65535) nchunk = 65535;
+    if (nchunk < 1) nchunk = 1;
+    long long vchunk = (V + nchunk - 1) / nchunk;
+    nchunk = (V + vchunk - 1) / vchunk;
+    dim3 grid((unsigned)xtiles, (unsigned)nchunk);
+    if (vec == 2) rho_partial_kernel<2><<<grid, 128, 0, c->stream>>>(f, c->Wv, X, V, vchunk, c->part);
+    else rho_partial_kernel<1><<<grid, 128, 0, c->stream>>>(f, c->Wv, X, V, vchunk, c->part);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    rho_final_kernel<<<(unsigned)((X + 255) / 256), 256, 0, c->stream>>>(c->part, X, (int)nchunk, rho);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E)
+{
+    const long long X = c->X;
+    const int block = 128;
+    const unsigned grid = (unsigned)((X + block - 1) / block);
+    double *ar = c->cplx[0], *ai = c->cplx[1], *br = c->cplx[2], *bi = c->cplx[3], *rr = c->cplx[4], *ri = c->cplx[5];
+    // forward: transfer to the equidistant grid + DFT, axis by axis
+    const double* sr = rho; const double* si = nullptr;
+    long long inner = 1;
+    for (int a = 0; a < c->dx; a++) {
+        bool last = (a == c->dx - 1);
+        double* dr = last ? rr : ((a & 1) ? br : ar);
+        double* di = last ? ri : ((a & 1) ? bi : ai);
+        if (si) apply_axis_kernel<1><<<grid, block, 0, c->stream>>>(sr, si, c->dFwdT[a], c->D[a], inner, X, dr, di);
+        else apply_axis_kernel<0><<<grid, block, 0, c->stream>>>(sr, si, c->dFwdT[a], c->D[a], inner, X, dr, di);
+        c->launches++;
+        sr = dr; si = di; inner *= c->D[a];
+    }
+    SpecParams S;
+    S.dx = c->dx; S.X = X;
+    for (int a = 0; a < c->dx; a++) { S.D[a] = c->D[a]; S.kap[a] = c->dKap[a]; }
+    for (int d = 0; d < c->dx; d++) {
+        spectral_kernel<<<grid, block, 0, c->stream>>>(S, d, rr, ri, ar, ai);
+        c->launches++;
+        double *pr = ar, *pi = ai, *qr = br, *qi = bi;
+        inner = 1;
+        for (int a = 0; a < c->dx; a++) {
+            bool last = (a == c->dx - 1);
+            apply_axis_kernel<1><<<grid, block, 0, c->stream>>>(pr, pi, c->dInvT[a], c->D[a], inner, X,
+                                                                last ? E + (long long)d * X : qr, last ? nullptr : qi);
+            c->launches++;
+            double* t;
+            t = pr; pr = qr; qr = t;
+            t = pi; pi = qi; qi = t;
+            inner *= c->D[a];
+        }
+    }
+    return cudaGetLastError();
+}
+
+static cudaError_t weighted_sum(sldg_ctx* c, const double* a, int nd, int axis0, int ncomp, long long total,
+                                double scale, double* out1)
+{
+    WgtParams P;
+    P.nd = nd; P.total = total;
+    for (int d = 0; d < nd; d++) { P.D[d] = c->D[axis0 + d]; P.w[d] = c->dWx[axis0 + d]; }
+    long long nb = (total + 255) / 256;
+    if (nb > 2048) nb = 2048;
+    weighted_sum_kernel<<<(unsigned)nb, 256, 0, c->stream>>>(P, a, ncomp, c->red);
+    final_sum_kernel<<<1, 256, 0, c->stream>>>(c->red, (int)nb, scale, out1);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t sldg_launch_energy(sldg_ctx* c, const double* E, double* out1)
+{
+    return weighted_sum(c, E, c->dx, 0, c->dx, c->X, 0.5, out1);
+}
+
+cudaError_t sldg_launch_mass(sldg_ctx* c, const double* f, double* out1)
+{
+    return weighted_sum(c, f, c->d, 0, 0, c->nf, 1.0, out1);
+}

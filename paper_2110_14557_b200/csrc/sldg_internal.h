@@ -1,0 +1,121 @@
+// sldg_internal.h -- private declarations of the sm_100a SLDG library (see include/sldg.h).
+// Nothing in this directory includes, links or calls anything under oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/sldg.h"
+
+#define SLDG_MAXK1 (SLDG_MAX_DEGREE + 1)
+#define SLDG_MAXNN (SLDG_MAXK1 * SLDG_MAXK1)
+#define SLDG_MAXPOLY (2 * SLDG_MAX_DEGREE + 2)   // A_jl(alpha) has degree <= 2k+1
+
+// bit 30 of a table's s-entry marks alpha == 0 (pure copy, exact permutation)
+#define SLDG_COPY_BIT (1 << 30)
+#define SLDG_S_MASK (SLDG_COPY_BIT - 1)
+
+enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5 };
+
+// Polynomial coefficients of A_jl(alpha), B_jl(alpha) (monomials in alpha, ascending), row-major
+// [2][K1*K1][SLDG_MAXPOLY]; held in __constant__ memory for the device-side table kernel.
+struct ABPoly {
+    double c[2][SLDG_MAXNN][SLDG_MAXPOLY];
+};
+
+struct ShiftTable {          // device-resident shift table of one sweep
+    const int* S;            // [n]  (s mod N) | copy bit
+    const double* AB;        // A then B, element m of index i at AB[i*strideIdx + m*strideM]
+    long long strideIdx, strideM;
+};
+
+struct SweepGeom {
+    long long inner, outer;  // prod of D_b below / above the axis
+    int N, K1;               // cells along the axis, nodes per cell
+    // shift index of the line at (inner p, outer q):
+    //   mode 0: (q / sdiv) % smod      (x-sweeps: node of the matching v axis)
+    //   mode 1: p % smod               (v-sweeps: flat x node, smod = X)
+    int mode;
+    long long sdiv, smod;
+};
+
+struct EventRec { cudaEvent_t a, b; int kind, axis; };
+
+struct sldg_ctx {
+    int dx, dv, d, k, K1;
+    int cells[SLDG_MAX_DIM];
+    long long D[SLDG_MAX_DIM];
+    double lo[SLDG_MAX_DIM], hi[SLDG_MAX_DIM], h[SLDG_MAX_DIM];
+    long long nf, X, V;
+    double xi[SLDG_MAXK1], w[SLDG_MAXK1];
+    ABPoly poly;
+
+    cudaStream_t stream;
+    int last_cuda;
+    int sm_count;
+
+    // ctx-owned small device tables
+    int* dS[SLDG_MAX_DIM];          // x-sweep shift tables, one per x axis: [D_{dx+a}]
+    double* dAB[SLDG_MAX_DIM];      //                                       [D_{dx+a}][2 K1^2]
+    double tab_tau[SLDG_MAX_DIM];   // dt the cached table of x axis a was built for
+    bool tab_valid[SLDG_MAX_DIM];
+    int* dS_hook; double* dAB_hook; long long hook_cap;   // test-hook tables (x axes)
+    double* dFwdT[3];               // forward transfer+DFT matrices, transposed [n][m], re then im
+    double* dInvT[3];               // inverse DFT+transfer matrices, transposed
+    double* dKap[3];                // signed wave numbers per x axis [D_a], Nyquist kept (zeroed in-kernel)
+    double* dWx[SLDG_MAX_DIM];      // per-axis quadrature weights h_a w_j  [D_a]
+    double* dScalar;                // 1 double result of mass / energy
+    int* hS; double* hAB;           // pinned host staging for table uploads
+    long long hcap;
+
+    // caller-owned workspace
+    char* ws; size_t ws_bytes;
+    double* f2;                     // second f buffer
+    int* vS; double* vAB;           // v-sweep tables [X], [2 K1^2][X]
+    double* Wv;                     // [V]
+    double* rho; double* E;         // [X], [dx][X]
+    double* part; long long part_cap;   // rho partial sums
+    double* cplx[6];                // complex scratch, X doubles each
+    double* red;                    // reduction partials [4096]
+    bool ws_ready;
+
+    // instrumentation
+    bool timing;
+    std::vector<EventRec> ev;       // recorded since last read
+    std::vector<EventRec> ev_free;
+    long long launches;
+    long long t_launch[SLDG_NKINDS]; double t_ms[SLDG_NKINDS];
+    long long a_launch[SLDG_MAX_DIM]; double a_ms[SLDG_MAX_DIM];
+
+    // tuning
+    int opt_tile_bytes;             // axis-0 kernel tile size
+    int opt_walk_block;             // slow-axis kernel block size
+    int opt_walk_vec;               // 0 = auto, 1, 2
+};
+
+// ---- host tables (sldg_tables.cpp)
+void sldg_gl_rule(int n, double* xi, double* w);
+void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out);
+void sldg_eval_AB_host(const ABPoly* p, int k, double alpha, double* A, double* B);
+// forward: G = F (I (x) P), inverse: H = (I (x) P^-1) F^-1 / D ; transposed storage [n][m], re block then im block
+void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* invT);
+
+// ---- kernel launchers (each returns cudaError_t of the launch)
+cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
+                                   const ShiftTable& t);
+cudaError_t sldg_launch_sweep_tma(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
+                                  const ShiftTable& t);
+cudaError_t sldg_upload_poly(const ABPoly* p);
+cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB);
+cudaError_t sldg_launch_wv(sldg_ctx* c);
+cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho);
+cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E);
+cudaError_t sldg_launch_energy(sldg_ctx* c, const double* E, double* out1);
+cudaError_t sldg_launch_mass(sldg_ctx* c, const double* f, double* out1);
+
+// instrumentation helpers (sldg_api.cu)
+void sldg_ev_begin(sldg_ctx* c, int kind, int axis);
+void sldg_ev_end(sldg_ctx* c);

@@ -1,0 +1,235 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the ctypes binding) against the CPU oracle, element by
+element on the same seeded inputs.  Bars (BASELINE.json north_star): max|g-o|/max|o| <= 1e-12 per sweep,
+<= 1e-10 after 10 Strang steps, bit-exact for integer shifts.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from oracle import oracle as O
+
+pytestmark = pytest.mark.gpu
+
+TOL_SWEEP = 1e-12
+TOL_STEPS = 1e-10
+
+
+def rel_inf(g, o):
+    return float(np.abs(g - o).max() / np.abs(o).max())
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2110_14557_b200 as pkg
+    if not torch.cuda.is_available():
+        pytest.fail("gpu test without a CUDA device")
+    return pkg
+
+
+def make_pair(P, dx, dv, cells, k, dom=None):
+    if dom is None:
+        dom = []
+        for a in range(dx + dv):
+            dom += [0.0, 1.0 + a] if a < dx else [-2.0 - a, 2.0 + a]
+    return P.Sldg(dx, dv, cells, k, dom), O.Oracle(dx, dv, cells, k, dom, threads=O.lib().orc_max_threads())
+
+
+def pair_of_cfg(P, cfg):
+    return make_pair(P, cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+
+
+# --------------------------------------------------------------- constants
+
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
+def test_AB_and_nodes_match_oracle(P, k):
+    g, o = make_pair(P, 1, 1, [3, 2], k)
+    for a in range(2):
+        assert np.abs(g.node_coords(a) - o.node_coords(a)).max() <= 4e-16 * 5
+    for alpha in [0.0, 1e-12, 1e-3, 0.123, 0.3, 0.5, 0.77, 0.999, 1 - 1e-12]:
+        A, B = g.AB(alpha)
+        Ao, Bo = O.AB(k, alpha)
+        assert np.abs(A - Ao).max() < 5e-14 and np.abs(B - Bo).max() < 5e-14, (k, alpha)
+
+
+# --------------------------------------------------------------- single sweeps through the test hook
+
+GEOMS = [
+    # dx, dv, cells, k      (several tiles, ragged tails, odd sizes, all degrees)
+    (1, 1, [37, 23], 1),
+    (1, 2, [16, 5, 7], 2),
+    (2, 2, [8, 8, 16, 16], 1),        # BASELINE config 1
+    (2, 2, [7, 5, 6, 9], 2),          # odd D everywhere: scalar / non-TMA paths
+    (2, 2, [5, 3, 4, 3], 0),
+    (2, 2, [6, 4, 5, 3], 3),
+    (2, 2, [4, 3, 3, 2], 4),
+    (2, 3, [6, 4, 5, 4, 3], 1),
+    (3, 3, [4, 3, 5, 3, 4, 2], 1),
+    (3, 3, [3, 2, 2, 3, 2, 2], 2),
+    (2, 2, [1, 2, 1, 3], 1),          # single-cell axes
+    (2, 2, [40, 33, 6, 5], 1),        # many lines per TMA tile + ragged last tile
+]
+KINDS_FRAC = ["small", "cfl", "edge"]
+KINDS_INT = ["int0", "int+1", "int-1", "int+3", "int-3", "intwrap", "intmix"]
+
+
+@pytest.mark.parametrize("geom", GEOMS, ids=lambda g: f"{g[0]}x{g[1]}v-{'x'.join(map(str, g[2]))}-k{g[3]}")
+def test_every_axis_every_shift_kind(P, geom):
+    dx, dv, cells, k = geom
+    g, o = make_pair(P, dx, dv, cells, k)
+    f0 = W.random_field(o.shape, seed=W.SEED + k)
+    for axis in range(dx + dv):
+        n = o.D[dx + axis] if axis < dx else o.X
+        for kind in KINDS_FRAC + KINDS_INT:
+            delta = W.delta_table(n, kind, seed=W.SEED + axis, ncells=cells[axis]).numpy()
+            want = o.sweep_axis(f0.numpy(), axis, delta)
+            fg = f0.to(g.device).contiguous()
+            g.advect_axis(fg, axis, delta)
+            got = fg.cpu().numpy()
+            if kind in KINDS_INT:
+                assert np.array_equal(got, want), (axis, kind)
+            else:
+                assert rel_inf(got, want) <= TOL_SWEEP, (axis, kind, rel_inf(got, want))
+
+
+def test_integer_shift_keeps_negative_zero_nan_and_inf(P):
+    """alpha == 0 is a copy, not A=I,B=0 arithmetic: -0.0, inf and NaN payloads survive bit for bit."""
+    g, o = make_pair(P, 2, 2, [6, 4, 4, 4], 1)
+    f0 = W.random_field(o.shape, seed=5)
+    f0.view(-1)[::7] = -0.0
+    f0.view(-1)[3::11] = float("inf")
+    f0.view(-1)[5::13] = float("nan")
+    for axis in range(4):
+        n = o.D[2 + axis] if axis < 2 else o.X
+        delta = W.delta_table(n, "intmix", seed=3 + axis).numpy()
+        want = o.sweep_axis(f0.numpy(), axis, delta)
+        fg = f0.to(g.device).contiguous()
+        g.advect_axis(fg, axis, delta)
+        assert np.array_equal(fg.cpu().numpy().view(np.int64), want.view(np.int64))
+
+
+def test_tile_size_option_does_not_change_results(P):
+    g, o = make_pair(P, 2, 2, [9, 31, 4, 5], 1)
+    f0 = W.random_field(o.shape, seed=9)
+    delta = W.delta_table(o.D[2], "cfl", seed=1).numpy()
+    outs = []
+    for tb in (256, 1024, 16384, 65536):
+        g.set_option("tile_bytes", tb)
+        fg = f0.to(g.device).contiguous()
+        g.advect_axis(fg, 0, delta)
+        outs.append(fg.cpu().numpy())
+    for x in outs[1:]:
+        assert np.array_equal(outs[0], x)
+    assert rel_inf(outs[0], o.sweep_axis(f0.numpy(), 0, delta)) <= TOL_SWEEP
+
+
+# --------------------------------------------------------------- the named calls
+
+def small_cfgs():
+    c = W.CONFIGS
+    return [c[0],
+            W.scaled(c[1], [12, 10, 8, 8]),
+            W.scaled(c[2], [8, 8, 6, 6, 4]),
+            W.scaled(c[3], [6, 4, 4, 6, 4, 4]),
+            W.scaled(c[4], [6, 4, 6, 4, 6, 4])]
+
+
+@pytest.mark.parametrize("cfg", small_cfgs(), ids=lambda c: c["name"])
+def test_advect_x_advect_v_density_poisson(P, cfg):
+    g, o = pair_of_cfg(P, cfg)
+    coords = [o.node_coords(a) for a in range(o.d)]
+    f0 = W.random_field(o.shape, kind="perturbed", base=W.initial_data(cfg, coords))
+    dt = cfg["dt"]
+    # advect_x
+    fg = f0.to(g.device).contiguous()
+    g.advect_x(fg, dt / 2)
+    want = o.advect_x(f0.numpy(), dt / 2)
+    assert rel_inf(fg.cpu().numpy(), want) <= TOL_SWEEP * cfg["dim_x"]
+    # density
+    rho_g = g.density(fg).cpu().numpy()
+    rho_o = o.density(want)
+    assert rel_inf(rho_g, rho_o) <= 1e-12
+    # poisson on the oracle's rho (same input both sides)
+    E_g = g.poisson(torch.from_numpy(rho_o).to(g.device)).cpu().numpy()
+    E_o = o.poisson(rho_o)
+    assert rel_inf(E_g, E_o) <= 1e-12
+    # advect_v with the physical field and with a strong random field (|delta| up to ~3 cells)
+    hv = (cfg["domain"][2 * cfg["dim_x"] + 1] - cfg["domain"][2 * cfg["dim_x"]]) / cfg["cells"][cfg["dim_x"]]
+    for E in (E_o, W.random_E(o.dx, o.xshape, amplitude=3.0 * hv / dt).numpy()):
+        fg = f0.to(g.device).contiguous()
+        g.advect_v(fg, torch.from_numpy(E).to(g.device), dt)
+        want = o.advect_v(f0.numpy(), E, dt)
+        assert rel_inf(fg.cpu().numpy(), want) <= TOL_SWEEP * cfg["dim_x"]
+
+
+def test_advect_v_constant_dyadic_field_is_exact_integer_shift(P):
+    """E = m h_v / dt with dyadic h_v, dt: delta = -m exactly -> bit-exact permutation through advect_v
+    (the device-built shift table takes the same floor() decision as the oracle, in fp64)."""
+    dom = [0, 1.0, 0, 1.0, -3.0, 3.0, -1.5, 1.5]
+    g, o = make_pair(P, 2, 2, [4, 6, 8, 4], 1, dom)            # h_v = 0.75
+    f0 = W.random_field(o.shape, seed=11)
+    dt = 0.25
+    E = np.empty((2,) + o.xshape)
+    E[0] = 2 * 0.75 / dt
+    E[1] = -1 * 0.75 / dt
+    fg = f0.to(g.device).contiguous()
+    g.advect_v(fg, torch.from_numpy(E).to(g.device), dt)
+    want = o.advect_v(f0.numpy(), E, dt)
+    assert np.array_equal(fg.cpu().numpy(), want)
+    assert np.array_equal(want, np.roll(np.roll(f0.numpy(), -2 * 2, axis=1), 1 * 2, axis=0))
+
+
+@pytest.mark.parametrize("cfg", small_cfgs(), ids=lambda c: c["name"])
+def test_ten_strang_steps(P, cfg):
+    g, o = pair_of_cfg(P, cfg)
+    coords = [o.node_coords(a) for a in range(o.d)]
+    f0 = W.initial_data(cfg, coords)
+    fg = f0.to(g.device).contiguous()
+    fo = f0.numpy()
+    m0 = g.mass(fg)
+    for _ in range(10):
+        g.step(fg, cfg["dt"])
+        fo, rho_o, E_o = o.step(fo, cfg["dt"])
+    assert rel_inf(fg.cpu().numpy(), fo) <= TOL_STEPS
+    assert rel_inf(g.last_rho().cpu().numpy(), rho_o) <= TOL_STEPS
+    # E is a difference quantity (rho - 1 ~ 1e-2..1e-3): relative to max|E| it inherits rho's absolute error
+    assert np.abs(g.last_E().cpu().numpy() - E_o).max() <= TOL_STEPS * max(1.0, np.abs(E_o).max())
+    assert abs(g.mass(fg) - m0) <= 1e-12 * abs(m0)
+    assert abs(g.mass(fg) - o.mass(fo)) <= 1e-12 * abs(m0)
+    Eg = g.last_E()
+    assert abs(g.electric_energy(Eg) - o.electric_energy(Eg.cpu().numpy())) <= 1e-12 * o.electric_energy(E_o) + 1e-30
+
+
+def test_step_host_matches_step(P):
+    cfg = W.CONFIGS[0]
+    g, o = pair_of_cfg(P, cfg)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    fd = f0.to(g.device).contiguous()
+    for _ in range(3):
+        g.step(fd, cfg["dt"])
+    fh = f0.clone().pin_memory()
+    fdev = g.empty_field()
+    Eh = torch.empty((2,) + o.xshape, dtype=torch.float64).pin_memory()
+    g.step_host(fh, fdev, cfg["dt"], nsteps=3, E_host=Eh)
+    assert torch.equal(fh, fd.cpu())
+    assert torch.equal(Eh, g.last_E().cpu())
+
+
+def test_errors_are_reported_not_swallowed(P):
+    import ctypes as C
+    L = P.lib()
+    h = C.c_void_p()
+    bad = L.sldg_create(C.byref(h), 3, 2, (C.c_int * 5)(2, 2, 2, 2, 2), 1, (C.c_double * 10)(*([0, 1] * 5)))
+    assert bad == -1
+    g, o = make_pair(P, 1, 1, [4, 4], 1)
+    f = g.empty_field()
+    assert L.sldg_step(None, C.c_void_p(f.data_ptr()), 0.1) == -1
+    assert L.sldg_advect_x(g._h, None, 0.1) == -1
+    assert L.sldg_advect_x(g._h, C.c_void_p(f.data_ptr() + 8), 0.1) == -1      # misaligned
+    # a context without workspace refuses to run
+    h2 = C.c_void_p()
+    assert L.sldg_create(C.byref(h2), 1, 1, (C.c_int * 2)(4, 4), 1, (C.c_double * 4)(0, 1, 0, 1)) == 0
+    assert L.sldg_step(h2, C.c_void_p(f.data_ptr()), 0.1) == -4
+    L.sldg_destroy(h2)
