@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the driver.
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--config I]
+
+A "step" is one Strang step (3*d_x sweeps + rho + Poisson + shift tables) of the
+SLDG Vlasov-Poisson path on synthetic data of BASELINE.json configs[I] (default I=1: 4-d two-stream,
+64^4 cells, k=2, 192^4 values = 10.9 GB fp64).  Metric: effective HBM GB/s per 1-D advection sweep,
+2*|f|*8 B per sweep / time (BASELINE.json `metric`); `value` uses the WHOLE step time (rho, Poisson and
+table kernels included), `sweeps` lists the pure per-axis kernel figures from CUDA events on the launching
+stream.  Multi-GPU: the path does not shard in this build ("replicas only"): every rank
+runs an independent replica, value = total bytes of all ranks / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "effective HBM GB/s per 1D advection sweep (2*|f|*8 B / time), whole Strang step"
+UNIT = "GB/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star "~8 TB/s"
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy burst)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def sweeps_per_step(cfg):
+    return 3 * cfg["dim_x"]
+
+
+def sweep_bytes(cfg):
+    import workloads as W
+    return 2 * W.field_elems(cfg) * 8
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                if out.returncode == 0 and out.stdout.strip():
+                    self.rows.append([c.strip() for c in out.stdout.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def stop(self):
+        self._stop.set()
+        self.join(timeout=10)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------- distributed plumbing
+def dist_setup(n_gpus):
+    """-> (rank, world, local_rank).  Under torchrun: init the process group (nccl on GPU, gloo otherwise)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        if torch.cuda.is_available():
+            torch.cuda.set_device(local)
+        dist.init_process_group(backend=backend)
+    return rank, world, local
+
+
+def aggregate(ms_local, bytes_local, device="cpu"):
+    """Replicas-only aggregation: (max over ranks of the timed region [ms], sum over ranks of the bytes).
+    Works with gloo (CPU tests) and nccl."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms_local), float(bytes_local)
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    b = torch.tensor([float(bytes_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(b, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(b.item())
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+# ----------------------------------------------------------------------------- the oracle as CPU baseline
+def oracle_sample_cfg(cfg, target_values=2.0e7):
+    """A bounded sample of the workload: same dimensions, degree, domain, dt and initial data, fewer cells
+    (a 'scaled replica'), sized so that one oracle Strang step takes seconds."""
+    import workloads as W
+    d = cfg["dim_x"] + cfg["dim_v"]
+    k1 = cfg["degree"] + 1
+    per_axis = max(2, int(round(target_values ** (1.0 / d) / k1)))
+    cells = [min(c, per_axis) for c in cfg["cells"]]
+    return W.scaled(cfg, cells)
+
+
+def time_oracle(cfg, steps, warmup, budget_s=25.0):
+    """Time the oracle AS IT STANDS (oracle/sldg_oracle.c, all host threads) on a bounded sample.
+    -> dict(value [GB/s effective per sweep], ms_per_step, cores, sample, steps)."""
+    import workloads as W
+    from oracle import oracle as O
+    s = oracle_sample_cfg(cfg)
+    cores = O.lib().orc_max_threads()
+    o = O.Oracle(s["dim_x"], s["dim_v"], s["cells"], s["degree"], s["domain"], threads=cores)
+    f = W.initial_data(s, [o.node_coords(a) for a in range(o.d)]).numpy()
+    for _ in range(max(0, warmup)):
+        f, _, _ = o.step(f, s["dt"])
+    done, t0 = 0, time.perf_counter()
+    while done < steps:
+        f, _, _ = o.step(f, s["dt"])
+        done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    ms = 1e3 * dt / done
+    value = sweeps_per_step(s) * sweep_bytes(s) / (ms * 1e-3) / 1e9
+    return {"value": value, "unit": UNIT, "ms_per_step": ms, "cores": cores, "kind": "oracle", "steps": done,
+            "sample": f"scaled replica of {cfg['name']}: cells {s['cells']} ({W.field_elems(s)} values), "
+                      f"{done} Strang step(s), all {cores} host threads"}
+
+
+def run_reference(args, cfg, rank, world):
+    """--impl reference: for this tier the reference arm IS the oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return None
+    r = time_oracle(cfg, args.steps, args.warmup, budget_s=120.0)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": r["steps"], "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "note": "CPU oracle on a bounded sample; " + r["sample"]},
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    return line
+
+
+# ----------------------------------------------------------------------------- the CUDA path
+def ncu_traffic(cfg_name):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.txt")
+    try:
+        with open(p) as fh:
+            for ln in fh:
+                if ln.startswith("{"):
+                    d = json.loads(ln)
+                    if d.get("workload") == cfg_name:
+                        return d
+    except Exception:
+        pass
+    return None
+
+
+def run_ours(args, cfg, rank, world, local):
+    import torch
+    import workloads as W
+    import paper_2110_14557_b200 as P
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SLDG path has no CPU fallback (use --impl reference "
+                         "to time the CPU oracle)")
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], device=dev)
+    coords = [g.node_coords(a) for a in range(g.d)]
+    f = g.empty_field()
+    W.initial_data(cfg, coords, device=dev, out=f)
+    dt = cfg["dt"]
+    nf = W.field_elems(cfg)
+    nsweeps = sweeps_per_step(cfg)
+    bytes_step = nsweeps * sweep_bytes(cfg)
+
+    for _ in range(max(args.warmup, 3)):
+        g.step(f, dt)
+    torch.cuda.synchronize(dev)
+    g.timing_enable(True)
+    g.timing_read()
+    launches0 = g.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    for _ in range(args.steps):
+        g.step(f, dt)
+    e1.record(g.stream)
+    torch.cuda.synchronize(dev)
+    barrier()
+    ms_total_local = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = g.launch_count() - launches0
+    kinds, axes = g.timing_read()
+    g.timing_enable(False)
+    ms_total, bytes_all = aggregate(ms_total_local, bytes_step * args.steps, device=dev)
+    ms_step = ms_total / args.steps
+    value = bytes_all / (ms_total * 1e-3) / 1e9
+
+    peak, peak_src = measured_peak()
+    # per-axis pure kernel figures (CUDA events around every sweep launch, on the launching stream)
+    sweeps = {}
+    names = [f"x{a + 1}" for a in range(cfg["dim_x"])] + [f"v{a + 1}" for a in range(cfg["dim_v"])]
+    for a, (n, ms) in enumerate(axes):
+        if n:
+            gbs = sweep_bytes(cfg) / (ms / n * 1e-3) / 1e9
+            sweeps[names[a]] = {"launches": n, "ms": ms / n, "gbs": gbs, "pct_of_measured_peak": 100 * gbs / peak,
+                                "pct_of_nominal_8TBs": 100 * gbs / NOMINAL_HBM_GBS}
+    # dominant kernel = the one with the largest share of the step
+    kn, (kl, kms) = max(((k, v) for k, v in kinds.items() if k.startswith("sweep")), key=lambda kv: kv[1][1])
+    achieved = sweep_bytes(cfg) / (kms / kl * 1e-3) / 1e9
+    tr = ncu_traffic(cfg["name"])
+    roofline = {"bound": "hbm", "kernel": kn, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": tr.get("traffic_bytes_per_launch") if tr else None,
+                "algorithmic_bytes_per_launch": sweep_bytes(cfg), "peak_source": peak_src,
+                "launches": kl, "avg_ms": kms / kl, "share_of_step": kms / (ms_total_local)}
+    parts = {k: {"launches": n, "ms_per_step": ms / args.steps} for k, (n, ms) in kinds.items() if n}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": cfg["name"], "values": nf, "bytes_f": nf * 8, "sweeps_per_step": nsweeps,
+                   "dt": dt, "l2": "inputs larger than L2 (no flush needed)" if nf * 8 > 2 * 126e6 else
+                   "array fits in L2: numbers are L2-resident, launch-bound",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "pct_of_measured_peak": 100 * value / world / peak, "pct_of_nominal_8TBs": 100 * value / world / NOMINAL_HBM_GBS,
+        "sweeps": sweeps, "parts": parts, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
+    }
+
+    # end to end through the C-ABI with HOST buffers (sldg_step_host): H2D of f, one Strang step, D2H of f, per step
+    if rank == 0 or world > 1:
+        try:
+            fh = torch.empty(g.shape, dtype=torch.float64, pin_memory=True)
+            fh.copy_(f)
+            nrep = max(1, min(args.steps, 3))
+            g.step_host(fh, f, dt, nsteps=1)                    # warm-up
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            for _ in range(nrep):
+                g.step_host(fh, f, dt, nsteps=1)
+            torch.cuda.synchronize(dev)
+            e2e_ms_local = 1e3 * (time.perf_counter() - t0)
+            e2e_ms, e2e_bytes = aggregate(e2e_ms_local, bytes_step * nrep, device=dev)
+            line["e2e"] = {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": nf * 8,
+                           "d2h_bytes_per_step": nf * 8, "ms_per_step": e2e_ms / nrep, "steps": nrep,
+                           "api": "sldg_step_host (pinned host f -> device, 1 Strang step, device -> host)"}
+            del fh
+        except Exception as ex:                                  # e.g. not enough pinned host memory
+            line["e2e"] = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = time_oracle(cfg, steps=1000, warmup=1, budget_s=15.0)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "ms_per_step")}
+    return line if rank == 0 else None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--cells", type=str, default=None, help="override cells, e.g. 16,16,16,16 (debug only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    import workloads as W
+    cfg = W.CONFIGS[args.config]
+    if args.cells:
+        cfg = W.scaled(cfg, [int(c) for c in args.cells.split(",")])
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        line = run_reference(args, cfg, rank, int(os.environ.get("WORLD_SIZE", "1")))
+    else:
+        rank, world, local = dist_setup(args.gpus)
+        line = run_ours(args, cfg, rank, world, local)
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -88,7 +88,7 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
         if (a < dim_x) c->X *= c->D[a]; else c->V *= c->D[a];
     }
     sldg_gl_rule(c->K1, c->xi, c->w);
-    sldg_build_poly(c->k, c->xi, c->w, &c->poly);
+    sldg_build_poly(c->k, c->xi, c->w, &c->poly, &c->poly_ld);
     c->stream = 0; c->last_cuda = 0; c->sm_count = 148;
     c->ws = nullptr; c->ws_bytes = 0; c->ws_ready = false;
     c->timing = false; c->launches = 0;
@@ -243,7 +243,7 @@ static void host_entry(const sldg_ctx* c, double delta, int N, int* S, double* A
         for (int m = 0; m < NN; m++) { AB[m] = (m % (c->K1 + 1) == 0) ? 1.0 : 0.0; AB[NN + m] = 0.0; }
     } else {
         *S = s;
-        sldg_eval_AB_host(&c->poly, c->k, alpha, AB, AB + NN);
+        sldg_eval_AB_host(&c->poly_ld, c->k, alpha, AB, AB + NN);
     }
 }
 
@@ -512,7 +512,7 @@ extern "C" int sldg_last_cuda_error(const sldg_ctx* c) { return c ? c->last_cuda
 extern "C" int sldg_AB(const sldg_ctx* c, double alpha, double* A, double* B)
 {
     if (!c || !A || !B || !(alpha >= 0.0 && alpha <= 1.0)) return SLDG_EINVAL;
-    sldg_eval_AB_host(&c->poly, c->k, alpha, A, B);
+    sldg_eval_AB_host(&c->poly_ld, c->k, alpha, A, B);
     return SLDG_OK;
 }
 

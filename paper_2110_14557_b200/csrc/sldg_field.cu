@@ -29,13 +29,14 @@ __global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double 
     if (s < 0) s += N;
     bool cp = (alpha == 0.0);
     S[x] = s | (cp ? SLDG_COPY_BIT : 0);
+    const double xc = alpha - 0.5;              // coefficients are in powers of (alpha - 1/2)
 #pragma unroll
     for (int m = 0; m < NN; m++) {
         double a = c_poly.c[0][m][DEG], b = c_poly.c[1][m][DEG];
 #pragma unroll
         for (int t = DEG - 1; t >= 0; t--) {
-            a = fma(a, alpha, c_poly.c[0][m][t]);
-            b = fma(b, alpha, c_poly.c[1][m][t]);
+            a = fma(a, xc, c_poly.c[0][m][t]);
+            b = fma(b, xc, c_poly.c[1][m][t]);
         }
         if (cp) { a = (m % (K1 + 1) == 0) ? 1.0 : 0.0; b = 0.0; }
         AB[(long long)m * X + x] = a;

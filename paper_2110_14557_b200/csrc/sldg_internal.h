@@ -20,10 +20,13 @@
 
 enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5 };
 
-// Polynomial coefficients of A_jl(alpha), B_jl(alpha) (monomials in alpha, ascending), row-major
-// [2][K1*K1][SLDG_MAXPOLY]; held in __constant__ memory for the device-side table kernel.
+// Polynomial coefficients of A_jl(alpha), B_jl(alpha) in powers of (alpha - 1/2), ascending, row-major
+// [2][K1*K1][SLDG_MAXPOLY]; the fp64 copy sits in __constant__ memory for the device-side table kernel.
 struct ABPoly {
     double c[2][SLDG_MAXNN][SLDG_MAXPOLY];
+};
+struct ABPolyLD {
+    long double c[2][SLDG_MAXNN][SLDG_MAXPOLY];
 };
 
 struct ShiftTable {          // device-resident shift table of one sweep
@@ -52,6 +55,7 @@ struct sldg_ctx {
     long long nf, X, V;
     double xi[SLDG_MAXK1], w[SLDG_MAXK1];
     ABPoly poly;
+    ABPolyLD poly_ld;
 
     cudaStream_t stream;
     int last_cuda;
@@ -98,8 +102,8 @@ struct sldg_ctx {
 
 // ---- host tables (sldg_tables.cpp)
 void sldg_gl_rule(int n, double* xi, double* w);
-void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out);
-void sldg_eval_AB_host(const ABPoly* p, int k, double alpha, double* A, double* B);
+void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out, ABPolyLD* outld);
+void sldg_eval_AB_host(const ABPolyLD* p, int k, double alpha, double* A, double* B);
 // forward: G = F (I (x) P), inverse: H = (I (x) P^-1) F^-1 / D ; transposed storage [n][m], re block then im block
 void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* invT);
 

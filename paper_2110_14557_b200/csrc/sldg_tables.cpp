@@ -6,7 +6,8 @@
 //    (Fig. 1) with the diagonal GL-Lagrange mass matrix (reading A):
 //        A_jl = 1/w_j int_alpha^1 l_j(x) l_l(x - alpha) dx,   B_jl = 1/w_j int_0^alpha l_j(x) l_l(x - alpha + 1) dx.
 //    Here the integrals are done in closed form on the monomial expansion of the Lagrange basis (long double),
-//    which gives every entry as a polynomial of degree <= 2k+1 in alpha; the kernels evaluate it by Horner.
+//    which gives every entry as a polynomial of degree <= 2k+1 in alpha (stored re-expanded around alpha = 1/2);
+//    the host evaluates it by Horner in long double, the device in fp64.
 //  * fused transfer + DFT matrices of the Poisson solve (reading P1).
 #include <math.h>
 #include <string.h>
@@ -74,12 +75,13 @@ static ld binom(int n, int r)
     return b;
 }
 
-void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out)
+void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out, ABPolyLD* outld)
 {
     int n = k + 1;
     ld c[SLDG_MAXK1][SLDG_MAXK1];
     lagrange_monomials(n, xi, c);
     memset(out, 0, sizeof(*out));
+    memset(outld, 0, sizeof(*outld));
     for (int j = 0; j < n; j++)
         for (int l = 0; l < n; l++) {
             ld pa[SLDG_MAXPOLY] = {0}, pb[SLDG_MAXPOLY] = {0};
@@ -101,21 +103,32 @@ void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out)
                             pb[m + r + 1 + t] += f * binom(p, t) * ((t & 1) ? -1.0L : 1.0L);
                     }
                 }
-            for (int t = 0; t < SLDG_MAXPOLY; t++) {
-                out->c[0][j * n + l][t] = (double)(pa[t] / (ld)w[j]);
-                out->c[1][j * n + l][t] = (double)(pb[t] / (ld)w[j]);
+            // re-expand around alpha = 1/2 (t = alpha - 1/2, |t| <= 1/2): sum |c_i| |t|^i drops from ~380 to ~20
+            // for k = 4, which keeps the fp64 Horner evaluation on the device within a few 1e-15.
+            const int deg = 2 * k + 1;
+            for (int m = 0; m <= deg; m++) {
+                ld sa = 0, sb = 0, half = 1;
+                for (int i = m; i <= deg; i++) {
+                    sa += pa[i] * binom(i, m) * half;
+                    sb += pb[i] * binom(i, m) * half;
+                    half *= 0.5L;
+                }
+                ld ca = sa / (ld)w[j], cb = sb / (ld)w[j];
+                outld->c[0][j * n + l][m] = ca; outld->c[1][j * n + l][m] = cb;
+                out->c[0][j * n + l][m] = (double)ca; out->c[1][j * n + l][m] = (double)cb;
             }
         }
 }
 
-void sldg_eval_AB_host(const ABPoly* p, int k, double alpha, double* A, double* B)
+void sldg_eval_AB_host(const ABPolyLD* p, int k, double alpha, double* A, double* B)
 {
     int n = k + 1, deg = 2 * k + 1;
+    const ld x = (ld)alpha - 0.5L;
     for (int e = 0; e < n * n; e++) {
         ld a = p->c[0][e][deg], b = p->c[1][e][deg];
         for (int t = deg - 1; t >= 0; t--) {
-            a = a * (ld)alpha + (ld)p->c[0][e][t];
-            b = b * (ld)alpha + (ld)p->c[1][e][t];
+            a = a * x + p->c[0][e][t];
+            b = b * x + p->c[1][e][t];
         }
         A[e] = (double)a; B[e] = (double)b;
     }
