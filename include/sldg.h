@@ -115,8 +115,14 @@ int sldg_mass(sldg_ctx* ctx, const double* f, double* host_out);
 const char* sldg_strerror(int code);
 int sldg_last_cuda_error(const sldg_ctx* ctx);                   /* cudaError_t as int      */
 
-/* A(alpha), B(alpha) as the library evaluates them on the host (row-major (k+1)x(k+1)). */
-int sldg_AB(const sldg_ctx* ctx, double alpha, double* hostA, double* hostB);
+/* A(alpha), B(alpha) of eq. (3) (reading A) as the library evaluates them, row-major
+ * (k+1)x(k+1), 0 <= alpha <= 1, degree in 0..SLDG_MAX_DEGREE.  Host-only, needs no context or device.
+ *   device_arith = 0: the host route of the x-sweep tables (Horner in long double, rounded to fp64);
+ *   device_arith = 1: the exact arithmetic of the device-side v-sweep table kernel (fp64 Horner with
+ *                     fused multiply-add on the fp64 coefficients), reproduced on the host. */
+int sldg_AB(int degree, double alpha, int device_arith, double* hostA, double* hostB);
+/* (degree+1)-point Gauss-Legendre nodes and weights on [0,1] as the library uses them. Host-only. */
+int sldg_gauss_legendre(int degree, double* host_xi, double* host_w);
 
 /* Test hook: one sweep along `axis` with a caller-given shift table (in cells), through the
  * production kernels.  delta_host (host): for an x axis, D_{v axis dim_x+axis} entries indexed

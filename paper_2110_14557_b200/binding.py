@@ -39,7 +39,8 @@ EXPORTS = {
     "sldg_mass": (C.c_int, [_vp, _vp, _dp]),
     "sldg_strerror": (C.c_char_p, [C.c_int]),
     "sldg_last_cuda_error": (C.c_int, [_vp]),
-    "sldg_AB": (C.c_int, [_vp, C.c_double, _dp, _dp]),
+    "sldg_AB": (C.c_int, [C.c_int, C.c_double, C.c_int, _dp, _dp]),
+    "sldg_gauss_legendre": (C.c_int, [C.c_int, _dp, _dp]),
     "sldg_advect_axis": (C.c_int, [_vp, _vp, C.c_int, _dp]),
     "sldg_timing_enable": (C.c_int, [_vp, C.c_int]),
     "sldg_timing_read": (C.c_int, [_vp, _llp, _dp]),
@@ -88,6 +89,24 @@ def _ptr(t):
     import torch
     assert isinstance(t, torch.Tensor) and t.dtype == torch.float64 and t.is_contiguous()
     return C.c_void_p(t.data_ptr())
+
+
+def AB(degree, alpha, device_arith=False):
+    """sldg_AB: the library's A(alpha), B(alpha) (host-only call; no device needed)."""
+    import numpy as np
+    n = degree + 1
+    A, B = np.empty((n, n)), np.empty((n, n))
+    _check(lib().sldg_AB(int(degree), float(alpha), 1 if device_arith else 0,
+                         A.ctypes.data_as(_dp), B.ctypes.data_as(_dp)))
+    return A, B
+
+
+def gauss_legendre(degree):
+    """sldg_gauss_legendre: the library's nodes and weights on [0,1] (host-only call)."""
+    import numpy as np
+    xi, w = np.empty(degree + 1), np.empty(degree + 1)
+    _check(lib().sldg_gauss_legendre(int(degree), xi.ctypes.data_as(_dp), w.ctypes.data_as(_dp)))
+    return xi, w
 
 
 class Sldg:
@@ -145,12 +164,8 @@ class Sldg:
         import torch
         return torch.empty(self.shape, dtype=torch.float64, device=self.device)
 
-    def AB(self, alpha):
-        import numpy as np
-        n = self.k + 1
-        A, B = np.empty((n, n)), np.empty((n, n))
-        _check(lib().sldg_AB(self._h, float(alpha), A.ctypes.data_as(_dp), B.ctypes.data_as(_dp)))
-        return A, B
+    def AB(self, alpha, device_arith=False):
+        return AB(self.k, alpha, device_arith)
 
     # ---- hot path (names as in include/sldg.h)
     def advect_x(self, f, dt):

@@ -509,10 +509,38 @@ extern "C" const char* sldg_strerror(int code)
 }
 extern "C" int sldg_last_cuda_error(const sldg_ctx* c) { return c ? c->last_cuda : 0; }
 
-extern "C" int sldg_AB(const sldg_ctx* c, double alpha, double* A, double* B)
+template <int K1>
+static void ab_device_arith(const ABPoly& p, double alpha, double* A, double* B)
 {
-    if (!c || !A || !B || !(alpha >= 0.0 && alpha <= 1.0)) return SLDG_EINVAL;
-    sldg_eval_AB_host(&c->poly_ld, c->k, alpha, A, B);
+    const double xc = alpha - 0.5;
+    for (int m = 0; m < K1 * K1; m++) { A[m] = sldg_horner<K1>(p, 0, m, xc); B[m] = sldg_horner<K1>(p, 1, m, xc); }
+}
+
+extern "C" int sldg_AB(int degree, double alpha, int device_arith, double* A, double* B)
+{
+    if (degree < 0 || degree > SLDG_MAX_DEGREE || !A || !B || !(alpha >= 0.0 && alpha <= 1.0)) return SLDG_EINVAL;
+    double xi[SLDG_MAXK1], w[SLDG_MAXK1];
+    sldg_gl_rule(degree + 1, xi, w);
+    ABPoly* p = new (std::nothrow) ABPoly;
+    ABPolyLD* pl = new (std::nothrow) ABPolyLD;
+    if (!p || !pl) { delete p; delete pl; return SLDG_ENOMEM; }
+    sldg_build_poly(degree, xi, w, p, pl);
+    if (!device_arith) sldg_eval_AB_host(pl, degree, alpha, A, B);
+    else switch (degree) {
+        case 0: ab_device_arith<1>(*p, alpha, A, B); break;
+        case 1: ab_device_arith<2>(*p, alpha, A, B); break;
+        case 2: ab_device_arith<3>(*p, alpha, A, B); break;
+        case 3: ab_device_arith<4>(*p, alpha, A, B); break;
+        default: ab_device_arith<5>(*p, alpha, A, B); break;
+    }
+    delete p; delete pl;
+    return SLDG_OK;
+}
+
+extern "C" int sldg_gauss_legendre(int degree, double* xi, double* w)
+{
+    if (degree < 0 || degree > SLDG_MAX_DEGREE || !xi || !w) return SLDG_EINVAL;
+    sldg_gl_rule(degree + 1, xi, w);
     return SLDG_OK;
 }
 

@@ -20,7 +20,7 @@ __global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double 
 {
     long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (x >= X) return;
-    constexpr int NN = K1 * K1, DEG = 2 * K1 - 1;
+    constexpr int NN = K1 * K1;
     double delta = __ddiv_rn(__dmul_rn(-Ed[x], tau), hv);
     double sd = floor(delta);
     double alpha = delta - sd;
@@ -32,12 +32,7 @@ __global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double 
     const double xc = alpha - 0.5;              // coefficients are in powers of (alpha - 1/2)
 #pragma unroll
     for (int m = 0; m < NN; m++) {
-        double a = c_poly.c[0][m][DEG], b = c_poly.c[1][m][DEG];
-#pragma unroll
-        for (int t = DEG - 1; t >= 0; t--) {
-            a = fma(a, xc, c_poly.c[0][m][t]);
-            b = fma(b, xc, c_poly.c[1][m][t]);
-        }
+        double a = sldg_horner<K1>(c_poly, 0, m, xc), b = sldg_horner<K1>(c_poly, 1, m, xc);
         if (cp) { a = (m % (K1 + 1) == 0) ? 1.0 : 0.0; b = 0.0; }
         AB[(long long)m * X + x] = a;
         AB[(long long)(NN + m) * X + x] = b;

@@ -29,6 +29,23 @@ struct ABPolyLD {
     long double c[2][SLDG_MAXNN][SLDG_MAXPOLY];
 };
 
+// fp64 Horner evaluation of entry m of A (which = 0) or B (which = 1) at xc = alpha - 1/2: the arithmetic of the
+// device-side table kernel; also compiled for the host so that CPU tests can check it (sldg_AB, device_arith = 1).
+#ifdef __CUDACC__
+#define SLDG_HD __host__ __device__ __forceinline__
+#else
+#define SLDG_HD inline
+#endif
+template <int K1, class Coef>
+SLDG_HD double sldg_horner(const Coef& c, int which, int m, double xc)
+{
+    constexpr int DEG = 2 * K1 - 1;
+    double a = c.c[which][m][DEG];
+#pragma unroll
+    for (int t = DEG - 1; t >= 0; t--) a = fma(a, xc, c.c[which][m][t]);
+    return a;
+}
+
 struct ShiftTable {          // device-resident shift table of one sweep
     const int* S;            // [n]  (s mod N) | copy bit
     const double* AB;        // A then B, element m of index i at AB[i*strideIdx + m*strideM]

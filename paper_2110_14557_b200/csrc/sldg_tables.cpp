@@ -15,6 +15,7 @@
 #include "sldg_internal.h"
 
 typedef long double ld;
+typedef __float128 qd;   // coefficient construction only: the monomial route cancels ~1e5, harmless at 1e-34
 
 void sldg_gl_rule(int n, double* xi, double* w)
 {
@@ -47,19 +48,20 @@ void sldg_gl_rule(int n, double* xi, double* w)
 }
 
 // monomial coefficients (ascending) of the Lagrange basis on the nodes xi
-static void lagrange_monomials(int n, const double* xi, ld c[SLDG_MAXK1][SLDG_MAXK1])
+static void lagrange_monomials(int n, const double* xi, qd c[SLDG_MAXK1][SLDG_MAXK1])
 {
     for (int l = 0; l < n; l++) {
-        ld p[SLDG_MAXK1 + 1] = {0};
+        qd p[SLDG_MAXK1 + 1];
+        for (int q = 0; q <= SLDG_MAXK1; q++) p[q] = 0;
         p[0] = 1;
         int deg = 0;
         for (int m = 0; m < n; m++) {
             if (m == l) continue;
-            ld den = (ld)xi[l] - (ld)xi[m], r = (ld)xi[m];
+            qd den = (qd)xi[l] - (qd)xi[m], r = (qd)xi[m];
             // p <- p * (z - r) / den
             for (int q = deg + 1; q >= 0; q--) {
-                ld lower = (q > 0) ? p[q - 1] : 0;
-                ld same = (q <= deg) ? p[q] : 0;
+                qd lower = (q > 0) ? p[q - 1] : (qd)0;
+                qd same = (q <= deg) ? p[q] : (qd)0;
                 p[q] = (lower - r * same) / den;
             }
             deg++;
@@ -68,53 +70,54 @@ static void lagrange_monomials(int n, const double* xi, ld c[SLDG_MAXK1][SLDG_MA
     }
 }
 
-static ld binom(int n, int r)
+static qd binom(int n, int r)
 {
-    ld b = 1;
-    for (int i = 1; i <= r; i++) b = b * (ld)(n - r + i) / (ld)i;
+    qd b = 1;
+    for (int i = 1; i <= r; i++) b = b * (qd)(n - r + i) / (qd)i;
     return b;
 }
 
 void sldg_build_poly(int k, const double* xi, const double* w, ABPoly* out, ABPolyLD* outld)
 {
     int n = k + 1;
-    ld c[SLDG_MAXK1][SLDG_MAXK1];
+    qd c[SLDG_MAXK1][SLDG_MAXK1];
     lagrange_monomials(n, xi, c);
     memset(out, 0, sizeof(*out));
     memset(outld, 0, sizeof(*outld));
     for (int j = 0; j < n; j++)
         for (int l = 0; l < n; l++) {
-            ld pa[SLDG_MAXPOLY] = {0}, pb[SLDG_MAXPOLY] = {0};
+            qd pa[SLDG_MAXPOLY], pb[SLDG_MAXPOLY];
+            for (int i = 0; i < SLDG_MAXPOLY; i++) { pa[i] = 0; pb[i] = 0; }
             for (int m = 0; m < n; m++)
                 for (int q = 0; q < n; q++) {
-                    ld cc = c[j][m] * c[l][q];
-                    // A: sum_r C(m,r) alpha^(m-r) (1-alpha)^(r+q+1) / (r+q+1)
+                    qd cc = c[j][m] * c[l][q];
+                    // A: int_alpha^1 x^m (x-alpha)^q dx = sum_r C(m,r) alpha^(m-r) (1-alpha)^(r+q+1) / (r+q+1)
                     for (int r = 0; r <= m; r++) {
                         int p = r + q + 1;
-                        ld f = cc * binom(m, r) / (ld)p;
+                        qd f = cc * binom(m, r) / (qd)p;
                         for (int t = 0; t <= p; t++)
-                            pa[m - r + t] += f * binom(p, t) * ((t & 1) ? -1.0L : 1.0L);
+                            pa[m - r + t] += f * binom(p, t) * ((t & 1) ? (qd)-1 : (qd)1);
                     }
-                    // B: sum_r C(q,r) (1-alpha)^(q-r) alpha^(m+r+1) / (m+r+1)
+                    // B: int_0^alpha x^m (x+1-alpha)^q dx = sum_r C(q,r) (1-alpha)^(q-r) alpha^(m+r+1) / (m+r+1)
                     for (int r = 0; r <= q; r++) {
                         int p = q - r;
-                        ld f = cc * binom(q, r) / (ld)(m + r + 1);
+                        qd f = cc * binom(q, r) / (qd)(m + r + 1);
                         for (int t = 0; t <= p; t++)
-                            pb[m + r + 1 + t] += f * binom(p, t) * ((t & 1) ? -1.0L : 1.0L);
+                            pb[m + r + 1 + t] += f * binom(p, t) * ((t & 1) ? (qd)-1 : (qd)1);
                     }
                 }
             // re-expand around alpha = 1/2 (t = alpha - 1/2, |t| <= 1/2): sum |c_i| |t|^i drops from ~380 to ~20
             // for k = 4, which keeps the fp64 Horner evaluation on the device within a few 1e-15.
             const int deg = 2 * k + 1;
             for (int m = 0; m <= deg; m++) {
-                ld sa = 0, sb = 0, half = 1;
+                qd sa = 0, sb = 0, half = 1;
                 for (int i = m; i <= deg; i++) {
                     sa += pa[i] * binom(i, m) * half;
                     sb += pb[i] * binom(i, m) * half;
-                    half *= 0.5L;
+                    half *= (qd)0.5;
                 }
-                ld ca = sa / (ld)w[j], cb = sb / (ld)w[j];
-                outld->c[0][j * n + l][m] = ca; outld->c[1][j * n + l][m] = cb;
+                qd ca = sa / (qd)w[j], cb = sb / (qd)w[j];
+                outld->c[0][j * n + l][m] = (ld)ca; outld->c[1][j * n + l][m] = (ld)cb;
                 out->c[0][j * n + l][m] = (double)ca; out->c[1][j * n + l][m] = (double)cb;
             }
         }
