@@ -296,34 +296,29 @@ static int check_f(const sldg_ctx* c, const void* f)
     return SLDG_OK;
 }
 
-// Run sweeps along axes[0..n) in order, result in f.  The sweep along axis 0 (if present) runs in place; the
-// others ping-pong f <-> f2; an odd number of ping-pong sweeps ends with a device copy back into f.
-static int run_sweeps(sldg_ctx* c, double* f, const int* axes, const ShiftTable* tabs, int n,
-                      int (*prep)(sldg_ctx*, int, void*), void* prep_arg)
+// Run sweeps along axes[0..n) in order on the buffer pair (*cur, *oth); on return *cur holds the result.
+// A sweep along a slow axis is out of place (it flips cur/oth).  The sweep along axis 0 stages whole lines in
+// shared memory, so it may run in place or out of place: `flip0` selects out of place, which lets the caller fix
+// the parity of the flips so that a sequence ends in the caller's buffer without a device copy.
+static int run_sweeps(sldg_ctx* c, double** cur, double** oth, const int* axes, const ShiftTable* tabs, int n,
+                      bool flip0, int (*prep)(sldg_ctx*, int, void*), void* prep_arg)
 {
-    double* cur = f;
-    double* oth = c->f2;
     for (int i = 0; i < n; i++) {
         if (prep) { int r = prep(c, i, prep_arg); if (r) return r; }
         SweepGeom g = geom_of(c, axes[i]);
-        if (g.inner == 1) {
-            int r = run_sweep(c, cur, cur, axes[i], tabs[i]);
-            if (r) return r;
-        } else {
-            int r = run_sweep(c, cur, oth, axes[i], tabs[i]);
-            if (r) return r;
-            double* t = cur; cur = oth; oth = t;
-        }
+        const bool oop = (g.inner != 1) || flip0;
+        int r = run_sweep(c, *cur, oop ? *oth : *cur, axes[i], tabs[i]);
+        if (r) return r;
+        if (oop) { double* t = *cur; *cur = *oth; *oth = t; }
     }
-    if (cur != f) return copy_back(c, f, cur);
     return SLDG_OK;
 }
 
 // ------------------------------------------------------------------ hot path
-extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
+// x-sweeps on (*cur, *oth).  The dx-1 slow-axis sweeps flip the pair; the axis-0 sweep flips too iff that makes
+// the total number of flips even (`flip` = false: result in the buffer it started in) or odd (`flip` = true).
+static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, bool flip)
 {
-    int r = check_f(c, f);
-    if (r) return r;
     int axes[3];
     ShiftTable tabs[3];
     const long long NN2 = 2LL * c->K1 * c->K1;
@@ -339,14 +334,23 @@ extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
                 volatile double vt = v * dt;
                 delta[(size_t)n] = vt / c->h[a];
             }
-            r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
+            int r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
             if (r) return r;
             c->tab_valid[a] = true; c->tab_tau[a] = dt;
         }
         axes[a] = a;
         tabs[a].S = c->dS[a]; tabs[a].AB = c->dAB[a]; tabs[a].strideIdx = NN2; tabs[a].strideM = 1;
     }
-    return run_sweeps(c, f, axes, tabs, c->dx, nullptr, nullptr);
+    const bool flip0 = (((c->dx - 1) & 1) != 0) != flip;
+    return run_sweeps(c, cur, oth, axes, tabs, c->dx, flip0, nullptr, nullptr);
+}
+
+extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    double *cur = f, *oth = c->f2;
+    return advect_x_impl(c, &cur, &oth, dt, false);     // ends in f: no copy
 }
 
 struct VPrep { const double* E; double dt; };
@@ -362,11 +366,9 @@ static int vprep(sldg_ctx* c, int i, void* arg)
     return SLDG_OK;
 }
 
-extern "C" int sldg_advect_v(sldg_ctx* c, double* f, const double* E, double dt)
+// v-sweeps on (*cur, *oth): dx slow-axis sweeps, each flips the pair.
+static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt)
 {
-    int r = check_f(c, f);
-    if (r) return r;
-    if (!E) return SLDG_EINVAL;
     int axes[3];
     ShiftTable tabs[3];
     for (int i = 0; i < c->dx; i++) {
@@ -374,7 +376,20 @@ extern "C" int sldg_advect_v(sldg_ctx* c, double* f, const double* E, double dt)
         tabs[i].S = c->vS; tabs[i].AB = c->vAB; tabs[i].strideIdx = 1; tabs[i].strideM = c->X;
     }
     VPrep p = {E, dt};
-    return run_sweeps(c, f, axes, tabs, c->dx, vprep, &p);
+    return run_sweeps(c, cur, oth, axes, tabs, c->dx, false, vprep, &p);
+}
+
+extern "C" int sldg_advect_v(sldg_ctx* c, double* f, const double* E, double dt)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    if (!E) return SLDG_EINVAL;
+    double *cur = f, *oth = c->f2;
+    if ((r = advect_v_impl(c, &cur, &oth, E, dt))) return r;
+    // an odd number of v-sweeps (dim_x = 1 or 3) leaves the result in the workspace: one device copy.
+    // sldg_step avoids it by fixing the parity in its second x half step.
+    if (cur != f) return copy_back(c, f, cur);
+    return SLDG_OK;
 }
 
 extern "C" int sldg_density(sldg_ctx* c, const double* f, double* rho)
@@ -404,11 +419,14 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
 {
     int r = check_f(c, f);
     if (r) return r;
-    if ((r = sldg_advect_x(c, f, dt / 2.0))) return r;
-    if ((r = sldg_density(c, f, c->rho))) return r;
+    double *cur = f, *oth = c->f2;
+    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, false))) return r;          // ends in f
+    if ((r = sldg_density(c, cur, c->rho))) return r;
     if ((r = sldg_poisson(c, c->rho, c->E))) return r;
-    if ((r = sldg_advect_v(c, f, c->E, dt))) return r;
-    return sldg_advect_x(c, f, dt / 2.0);
+    if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;                 // ends in f2 iff dim_x is odd
+    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f))) return r;       // ... then flip back: ends in f
+    if (cur != f) return copy_back(c, f, cur);                                  // unreachable by construction
+    return SLDG_OK;
 }
 
 extern "C" int sldg_step_host(sldg_ctx* c, double* f_host, double* f_dev, double* E_host, double dt, int nsteps)
@@ -453,7 +471,10 @@ extern "C" int sldg_advect_axis(sldg_ctx* c, double* f, int axis, const double* 
         t.S = c->vS; t.AB = c->vAB; t.strideIdx = 1; t.strideM = X;
     }
     int axes[1] = {axis};
-    return run_sweeps(c, f, axes, &t, 1, nullptr, nullptr);
+    double *cur = f, *oth = c->f2;
+    if ((r = run_sweeps(c, &cur, &oth, axes, &t, 1, false, nullptr, nullptr))) return r;
+    if (cur != f) return copy_back(c, f, cur);
+    return SLDG_OK;
 }
 
 // ------------------------------------------------------------------ helpers
