@@ -113,6 +113,7 @@ struct sldg_ctx {
 
     // tuning
     int opt_tile_bytes;             // axis-0 kernel tile size
+    int opt_tile_stages;            // axis-0 kernel input ring depth (4, 2 or 1)
     int opt_walk_block;             // slow-axis kernel block size
     int opt_walk_vec;               // 0 = auto, 1, 2
 };
