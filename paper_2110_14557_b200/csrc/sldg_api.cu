@@ -94,11 +94,11 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
     c->timing = false; c->launches = 0;
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
-    c->opt_tile_bytes = 16384; c->opt_tile_stages = 4; c->opt_walk_block = 256; c->opt_walk_vec = 0;
+    c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 256; c->opt_walk_vec = 0;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
-    c->dScalar = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
+    c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
 
     // device side: needs a CUDA device.  Without one the context is unusable -> fail loudly.
     int dev = 0;
@@ -115,6 +115,8 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->hS, (size_t)maxD * 4);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->hAB, (size_t)maxD * NN2 * 8);
     if (e == cudaSuccess) e = cudaMalloc((void**)&c->dScalar, 8);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->dCounter, 16);
+    if (e == cudaSuccess) e = cudaMemset(c->dCounter, 0, 16);
     for (int a = 0; a < dim_x && e == cudaSuccess; a++) {
         long long Ds = c->D[dim_x + a];
         e = cudaMalloc((void**)&c->dS[a], (size_t)Ds * 4);
@@ -171,6 +173,7 @@ extern "C" int sldg_destroy(sldg_ctx* c)
     if (c->dS_hook) cudaFree(c->dS_hook);
     if (c->dAB_hook) cudaFree(c->dAB_hook);
     if (c->dScalar) cudaFree(c->dScalar);
+    if (c->dCounter) cudaFree(c->dCounter);
     if (c->hS) cudaFreeHost(c->hS);
     if (c->hAB) cudaFreeHost(c->hAB);
     for (auto& r : c->ev) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -261,13 +264,35 @@ static int upload_table(sldg_ctx* c, const double* delta, long long n, int N, in
     return SLDG_OK;
 }
 
-static int run_sweep(sldg_ctx* c, const double* fin, double* fout, int axis, const ShiftTable& t)
+static int copy_back(sldg_ctx* c, double* dst, const double* src);
+
+// `scratch`: the buffer of the pair that is neither read nor written (used only if an in-place request has to be
+// served by an out-of-place kernel).
+static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scratch, int axis, const ShiftTable& t)
 {
     SweepGeom g = geom_of(c, axis);
     cudaError_t e;
     if (g.inner == 1) {
+        // contiguous lines: per-warp TMA pipelines; block-wide tiles when a line is too long for a warp's ring;
+        // the (uncoalesced) register walk when it does not even fit a block's shared memory
         sldg_ev_begin(c, KIND_SWEEP0, axis);
-        e = sldg_launch_sweep_tma(c, fin, fout, g, t);
+        e = cudaErrorNotSupported;
+        if (c->opt_axis0_impl == 0 || c->opt_axis0_impl == 1) e = sldg_launch_sweep_line(c, fin, fout, g, t);
+        if (e == cudaErrorNotSupported && c->opt_axis0_impl != 3) {
+            e = sldg_launch_sweep_tma(c, fin, fout, g, t);
+            if (e == cudaErrorInvalidConfiguration) e = cudaErrorNotSupported;
+        }
+        if (e == cudaErrorNotSupported) {
+            if (fin == fout) {
+                if (!scratch || scratch == fin) { sldg_ev_end(c); return SLDG_EINVAL; }
+                e = sldg_launch_sweep_walk(c, fin, scratch, g, t);
+                sldg_ev_end(c);
+                c->launches++;
+                if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+                return copy_back(c, fout, scratch);
+            }
+            e = sldg_launch_sweep_walk(c, fin, fout, g, t);
+        }
     } else {
         if (fin == fout) return SLDG_EINVAL;
         sldg_ev_begin(c, KIND_SWEEP, axis);
@@ -307,7 +332,7 @@ static int run_sweeps(sldg_ctx* c, double** cur, double** oth, const int* axes, 
         if (prep) { int r = prep(c, i, prep_arg); if (r) return r; }
         SweepGeom g = geom_of(c, axes[i]);
         const bool oop = (g.inner != 1) || flip0;
-        int r = run_sweep(c, *cur, oop ? *oth : *cur, axes[i], tabs[i]);
+        int r = run_sweep(c, *cur, oop ? *oth : *cur, oop ? nullptr : *oth, axes[i], tabs[i]);
         if (r) return r;
         if (oop) { double* t = *cur; *cur = *oth; *oth = t; }
     }
@@ -602,7 +627,8 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
 {
     if (!c || !name) return SLDG_EINVAL;
     if (!strcmp(name, "tile_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_tile_bytes = (int)value; return SLDG_OK; }
-    if (!strcmp(name, "tile_stages")) { if (value != 1 && value != 2 && value != 4) return SLDG_EINVAL; c->opt_tile_stages = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "axis0_impl")) { if (value < 0 || value > 3) return SLDG_EINVAL; c->opt_axis0_impl = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "tile_stages")) { if (value < 1 || value > 4) return SLDG_EINVAL; c->opt_tile_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_block")) { if (value < 32 || value > 256 || (value & 31)) return SLDG_EINVAL; c->opt_walk_block = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_walk_vec = (int)value; return SLDG_OK; }
     return SLDG_EINVAL;

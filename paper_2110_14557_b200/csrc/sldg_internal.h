@@ -89,6 +89,7 @@ struct sldg_ctx {
     double* dKap[3];                // signed wave numbers per x axis [D_a], Nyquist kept (zeroed in-kernel)
     double* dWx[SLDG_MAX_DIM];      // per-axis quadrature weights h_a w_j  [D_a]
     double* dScalar;                // 1 double result of mass / energy
+    unsigned long long* dCounter;   // [2] work counter of the persistent axis-0 kernel (self-resetting)
     int* hS; double* hAB;           // pinned host staging for table uploads
     long long hcap;
 
@@ -112,8 +113,9 @@ struct sldg_ctx {
     long long a_launch[SLDG_MAX_DIM]; double a_ms[SLDG_MAX_DIM];
 
     // tuning
-    int opt_tile_bytes;             // axis-0 kernel tile size
-    int opt_tile_stages;            // axis-0 kernel input ring depth (4, 2 or 1)
+    int opt_tile_bytes;             // axis-0 kernels: bytes per chunk (per warp) / per tile (block-wide kernel)
+    int opt_tile_stages;            // axis-0 line kernel: input ring depth per warp (1..4)
+    int opt_axis0_impl;             // 0 = auto, 1 = per-warp pipelines, 2 = block-wide tiles, 3 = register walk
     int opt_walk_block;             // slow-axis kernel block size
     int opt_walk_vec;               // 0 = auto, 1, 2
 };
@@ -127,6 +129,8 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
 
 // ---- kernel launchers (each returns cudaError_t of the launch)
 cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
+                                   const ShiftTable& t);
+cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
                                    const ShiftTable& t);
 cudaError_t sldg_launch_sweep_tma(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
                                   const ShiftTable& t);

@@ -110,16 +110,23 @@ def test_integer_shift_keeps_negative_zero_nan_and_inf(P):
         assert np.array_equal(fg.cpu().numpy().view(np.int64), want.view(np.int64))
 
 
-def test_tile_size_option_does_not_change_results(P):
-    g, o = make_pair(P, 2, 2, [9, 31, 4, 5], 1)
+@pytest.mark.parametrize("cells,k", [([9, 31, 4, 5], 1), ([7, 33, 3, 5], 2), ([64, 40, 3, 4], 2), ([5, 37, 2, 3], 0),
+                                     ([1, 9, 2, 3], 1), ([3, 50, 3, 3], 4), ([700, 3, 2, 2], 3)])
+def test_axis0_implementations_and_tilings_agree_bitwise(P, cells, k):
+    """Every axis-0 kernel (per-warp TMA pipelines at every ring depth, block-wide TMA tiles, register walk) and
+    every chunk size gives the same bits (same per-cell arithmetic), and matches the oracle."""
+    g, o = make_pair(P, 2, 2, cells, k)
     f0 = W.random_field(o.shape, seed=9)
-    delta = W.delta_table(o.D[2], "cfl", seed=1).numpy()
+    delta = W.delta_table(o.D[2], "cfl", seed=1, ncells=cells[0]).numpy()
     outs = []
-    for tb in (256, 1024, 16384, 65536):
-        g.set_option("tile_bytes", tb)
-        fg = f0.to(g.device).contiguous()
-        g.advect_axis(fg, 0, delta)
-        outs.append(fg.cpu().numpy())
+    for impl, stages in ((1, 1), (1, 2), (1, 3), (1, 4), (2, 1), (3, 1)):
+        g.set_option("axis0_impl", impl)
+        g.set_option("tile_stages", stages)
+        for tb in (256, 1024, 4096, 16384, 65536):
+            g.set_option("tile_bytes", tb)
+            fg = f0.to(g.device).contiguous()
+            g.advect_axis(fg, 0, delta)
+            outs.append(fg.cpu().numpy())
     for x in outs[1:]:
         assert np.array_equal(outs[0], x)
     assert rel_inf(outs[0], o.sweep_axis(f0.numpy(), 0, delta)) <= TOL_SWEEP
