@@ -27,6 +27,7 @@ def _stale(target, deps):
 def build(force=False, verbose=False):
     objs = []
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("SLDG_NVCC_EXTRA", "").split()      # experiments only (e.g. -DSLDG_WALK_U2=6)
     for s in SOURCES:
         src = os.path.join(CSRC, s)
         obj = os.path.join(CSRC, os.path.splitext(s)[0] + ".o")

@@ -40,7 +40,19 @@ template <> struct Vec<2> {
     }
 };
 
-template <int K1> struct Unroll { static constexpr int U = (K1 == 1) ? 8 : (K1 == 2) ? 4 : (K1 == 3) ? 3 : 2; };
+#ifndef SLDG_WALK_U1
+#define SLDG_WALK_U1 8
+#endif
+#ifndef SLDG_WALK_U2
+#define SLDG_WALK_U2 4
+#endif
+#ifndef SLDG_WALK_U3
+#define SLDG_WALK_U3 4
+#endif
+// cells loaded ahead of the one being computed (loads in flight per thread = U * K1 * VEC values)
+template <int K1> struct Unroll {
+    static constexpr int U = (K1 == 1) ? SLDG_WALK_U1 : (K1 == 2) ? SLDG_WALK_U2 : (K1 == 3) ? SLDG_WALK_U3 : 2;
+};
 
 // MODE 0: one shift per thread (x-sweep, shift indexed by a digit of the outer index)
 // MODE 1: one shift per VALUE (v-sweep, shift indexed by the x node = inner index mod X)
@@ -169,10 +181,11 @@ cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout,
     P.fin = fin; P.fout = fout;
     P.inner = g.inner; P.N = g.N;
     P.sdiv = g.sdiv; P.smod = g.smod; P.t = t;
-    int vec = 2;
-    if (c->opt_walk_vec == 1) vec = 1;
+    // Measured on B200: one value per thread (64-bit loads, more threads, more loads in
+    // flight) beats 128-bit loads except for x-sweeps of degree >= 2, where the thread count is ample either way.
+    int vec = (g.mode == 0 && g.K1 >= 3) ? 2 : 1;
+    if (c->opt_walk_vec) vec = c->opt_walk_vec;
     if ((g.inner & 1) || (((uintptr_t)fin | (uintptr_t)fout) & 15)) vec = 1;
-    if (g.mode == 1 && c->opt_walk_vec == 0 && g.K1 >= 3) vec = 1;   // two matrix sets per thread: registers
     P.innerV = g.inner / vec;
     P.nwork = P.innerV * g.outer;
     if (P.nwork == 0) return cudaSuccess;
