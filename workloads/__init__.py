@@ -129,6 +129,19 @@ def random_field(shape, seed=SEED, kind="uniform", base=None, device="cpu"):
     raise ValueError(kind)
 
 
+def perturb_inplace(f, seed=SEED, amplitude=1e-3, slab_elems=1 << 27):
+    """f *= 1 + amplitude * U(-1,1), slab by slab along the slowest axis (no |f|-sized temporary: usable on a
+    57 GB device array).  The draw depends on the slab size, so callers that compare must share it."""
+    g = generator(seed, f.device)
+    flat = f.view(-1)
+    n = flat.numel()
+    for a in range(0, n, slab_elems):
+        b = min(n, a + slab_elems)
+        u = torch.rand(b - a, dtype=torch.float64, device=f.device, generator=g)
+        flat[a:b].mul_(1.0 + amplitude * (2.0 * u - 1.0))
+    return f
+
+
 def delta_table(n, kind, seed=SEED, ncells=None):
     """Shift tables (in cells) for the single-sweep test hook; returns float64 CPU tensor of length n.
       'int0', 'int+1', 'int-1', 'int+3', 'int-3', 'intwrap' (= ncells+2), 'intmix' (seeded integers in [-6,6])
