@@ -52,7 +52,7 @@ static WsLayout ws_layout(const sldg_ctx* c)
     L.E = take(X * 8 * c->dx);
     // rho partial sums: enough chunks to fill the GPU (see sldg_launch_density), at least 1
     long long xtiles = (c->X + 255) / 256;
-    long long nchunk = ((long long)148 * 16 + xtiles - 1) / xtiles;
+    long long nchunk = ((long long)148 * 64 + xtiles - 1) / xtiles;
     if (nchunk > c->V / 16) nchunk = c->V / 16;
     if (nchunk < 1) nchunk = 1;
     nchunk += 1;
@@ -94,8 +94,8 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
     c->timing = false; c->launches = 0;
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
-    c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0;
-    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->dWx[a] = nullptr; }
+    c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
+    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
     c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
@@ -268,7 +268,8 @@ static int copy_back(sldg_ctx* c, double* dst, const double* src);
 
 // `scratch`: the buffer of the pair that is neither read nor written (used only if an in-place request has to be
 // served by an out-of-place kernel).
-static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scratch, int axis, const ShiftTable& t)
+static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scratch, int axis, const ShiftTable& t,
+                     bool inplace_walk_ok = false)
 {
     SweepGeom g = geom_of(c, axis);
     cudaError_t e;
@@ -294,7 +295,8 @@ static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scrat
             e = sldg_launch_sweep_walk(c, fin, fout, g, t);
         }
     } else {
-        if (fin == fout) return SLDG_EINVAL;
+        // a slow-axis walk may run in place only when every shift of its table is s in {0, -1} (see x_plan)
+        if (fin == fout && !inplace_walk_ok) return SLDG_EINVAL;
         sldg_ev_begin(c, KIND_SWEEP, axis);
         e = sldg_launch_sweep_walk(c, fin, fout, g, t);
     }
@@ -340,12 +342,11 @@ static int run_sweeps(sldg_ctx* c, double** cur, double** oth, const int* axes, 
 }
 
 // ------------------------------------------------------------------ hot path
-// x-sweeps on (*cur, *oth).  The dx-1 slow-axis sweeps flip the pair; the axis-0 sweep flips too iff that makes
-// the total number of flips even (`flip` = false: result in the buffer it started in) or odd (`flip` = true).
-static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, bool flip)
+// Host-built x-sweep tables for time increment dt (cached per axis).  Also records whether a slow-axis walk with
+// this table may run IN PLACE: the walk writes output cell (j + s + 1) mod N after reading cells j and j+1, which
+// never overtakes its own reads iff every entry has s mod N in {0, N-1} (|delta| < 1, the BASELINE regime).
+static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
 {
-    int axes[3];
-    ShiftTable tabs[3];
     const long long NN2 = 2LL * c->K1 * c->K1;
     for (int a = 0; a < c->dx; a++) {
         const int b = c->dx + a;
@@ -361,13 +362,83 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
             }
             int r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
             if (r) return r;
+            bool safe = true;
+            for (long long n = 0; n < c->D[b]; n++) {
+                const int sv = c->hS[n] & SLDG_S_MASK;
+                if (sv != 0 && sv != c->cells[a] - 1) safe = false;
+            }
+            c->tab_safe[a] = safe;
             c->tab_valid[a] = true; c->tab_tau[a] = dt;
         }
-        axes[a] = a;
         tabs[a].S = c->dS[a]; tabs[a].AB = c->dAB[a]; tabs[a].strideIdx = NN2; tabs[a].strideM = 1;
     }
-    const bool flip0 = (((c->dx - 1) & 1) != 0) != flip;
-    return run_sweeps(c, cur, oth, axes, tabs, c->dx, flip0, nullptr, nullptr);
+    return SLDG_OK;
+}
+
+// Plan of one x advection: x_1 and x_2 in one fused pass or separately, which sweeps run in place, such that the
+// number of buffer flips has the requested parity.  Fewest passes over f wins; ties go to fewer in-place walks.
+struct XPlan { bool ok, fused, x1_oop; bool inplace[3]; int passes, flips; };
+
+static bool fused_possible(const sldg_ctx* c)
+{
+    return c->opt_fuse_x && c->dx >= 2 && c->D[0] <= c->opt_fused_threads;
+}
+
+static XPlan x_plan(const sldg_ctx* c, bool flip)
+{
+    XPlan best; best.ok = false; best.passes = 1 << 30; best.flips = 0;
+    const int dx = c->dx;
+    for (int fused = fused_possible(c) ? 1 : 0; fused >= 0; fused--) {
+        const int first_slow = fused ? 2 : 1;
+        const int nslow = dx > first_slow ? dx - first_slow : 0;
+        for (int x1oop = fused ? 1 : 0; x1oop <= 1; x1oop++) {
+            for (int mask = 0; mask < (1 << nslow); mask++) {
+                bool legal = true;
+                int nin = 0;
+                for (int i = 0; i < nslow; i++)
+                    if (mask >> i & 1) { nin++; if (!c->tab_safe[first_slow + i] || !c->opt_inplace_walk) legal = false; }
+                if (!legal) continue;
+                const int flips = x1oop + nslow - nin, passes = 1 + nslow;
+                if ((flips & 1) != (flip ? 1 : 0)) continue;
+                const int score = passes * 16 + nin;
+                if (!best.ok || score < best.passes) {
+                    best.ok = true; best.passes = score; best.fused = fused != 0; best.x1_oop = x1oop != 0;
+                    best.flips = flips;
+                    for (int i = 0; i < 3; i++) best.inplace[i] = false;
+                    for (int i = 0; i < nslow; i++) best.inplace[first_slow + i] = (mask >> i & 1) != 0;
+                }
+            }
+        }
+    }
+    best.passes /= 16;
+    return best;
+}
+
+// x-sweeps on (*cur, *oth); `flip` = false: the result ends in the buffer it started in, true: in the other one.
+static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, bool flip)
+{
+    ShiftTable tabs[3];
+    int r = build_x_tables(c, dt, tabs);
+    if (r) return r;
+    XPlan p = x_plan(c, flip);
+    if (!p.ok) return SLDG_EINVAL;          // cannot happen: the unfused plan reaches either parity
+    int a = 0;
+    if (p.fused) {
+        sldg_ev_begin(c, KIND_FUSED, 0);
+        cudaError_t e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        sldg_ev_end(c);
+        c->launches++;
+        if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+        double* t = *cur; *cur = *oth; *oth = t;
+        a = 2;
+    }
+    for (; a < c->dx; a++) {
+        const bool oop = (a == 0) ? p.x1_oop : !p.inplace[a];
+        r = run_sweep(c, *cur, oop ? *oth : *cur, oop ? nullptr : *oth, a, tabs[a], /*inplace_walk_ok=*/!oop);
+        if (r) return r;
+        if (oop) { double* t = *cur; *cur = *oth; *oth = t; }
+    }
+    return SLDG_OK;
 }
 
 extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
@@ -445,11 +516,21 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
     int r = check_f(c, f);
     if (r) return r;
     double *cur = f, *oth = c->f2;
-    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, false))) return r;          // ends in f
+    // The dx v-sweeps flip the buffer pair dx times; the two x half steps choose their flip parities (p1, p2) so
+    // that the step ends in f with no device copy, at the fewest passes over f.
+    ShiftTable tabs[3];
+    if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;
+    int best = 1 << 30, p1 = 0;
+    for (int q1 = 0; q1 < 2; q1++) {
+        const int q2 = (q1 + c->dx) & 1;
+        XPlan a = x_plan(c, q1 != 0), b = x_plan(c, q2 != 0);
+        if (a.ok && b.ok && a.passes + b.passes < best) { best = a.passes + b.passes; p1 = q1; }
+    }
+    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, p1 != 0))) return r;
     if ((r = sldg_density(c, cur, c->rho))) return r;
     if ((r = sldg_poisson(c, c->rho, c->E))) return r;
-    if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;                 // ends in f2 iff dim_x is odd
-    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f))) return r;       // ... then flip back: ends in f
+    if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;
+    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f))) return r;       // ... ends in f
     if (cur != f) return copy_back(c, f, cur);                                  // unreachable by construction
     return SLDG_OK;
 }
@@ -608,6 +689,7 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
         if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
             c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
+            if (r.kind == KIND_FUSED) { for (int a = 0; a < 2; a++) { c->a_launch[a]++; c->a_ms[a] += 0.5 * t; } }
         }
         c->ev_free.push_back(r);
     }
@@ -630,6 +712,11 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "axis0_impl")) { if (value < 0 || value > 3) return SLDG_EINVAL; c->opt_axis0_impl = (int)value; return SLDG_OK; }
     if (!strcmp(name, "tile_stages")) { if (value < 1 || value > 4) return SLDG_EINVAL; c->opt_tile_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_block")) { if (value < 32 || value > 256 || (value & 31)) return SLDG_EINVAL; c->opt_walk_block = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fuse_x")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse_x = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "inplace_walk")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_inplace_walk = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fused_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_fused_threads = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "rho_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_rho_vec = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "rho_blocks")) { if (value < 1 || value > 64) return SLDG_EINVAL; c->opt_rho_blocks = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_walk_vec = (int)value; return SLDG_OK; }
     return SLDG_EINVAL;
 }

@@ -9,6 +9,10 @@ __constant__ ABPoly c_poly;
 
 cudaError_t sldg_upload_poly(const ABPoly* p) { return cudaMemcpyToSymbol(c_poly, p, sizeof(ABPoly)); }
 
+#ifndef SLDG_RHO_U
+#define SLDG_RHO_U 8
+#endif
+
 namespace {
 
 // ------------------------------------------------------------------ v-sweep shift table (row a5)
@@ -67,7 +71,7 @@ __global__ void __launch_bounds__(128) rho_partial_kernel(const double* __restri
     long long v0 = (long long)blockIdx.y * vchunk;
     long long v1 = v0 + vchunk; if (v1 > V) v1 = V;
     double acc[VEC] = {0};
-    constexpr int U = 8;
+    constexpr int U = SLDG_RHO_U;
     long long v = v0;
     for (; v + U <= v1; v += U) {
         double t[U][VEC];
@@ -223,9 +227,12 @@ cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho)
 {
     const long long X = c->X, V = c->V;
     int vec = ((X & 1) == 0 && (((uintptr_t)f) & 15) == 0) ? 2 : 1;
+    if (c->opt_rho_vec == 1) vec = 1;
     long long xtiles = (X + 128LL * vec - 1) / (128LL * vec);
-    long long want = (long long)c->sm_count * 16;
-    long long nchunk = (want + xtiles - 1) / xtiles;
+    // ONE wave of equal blocks: at most opt_rho_blocks (8) blocks per SM, rounded DOWN so that no second, partial
+    // wave forms (measured on B200: 1.2x between a grid of 1.03 waves and one of 0.5 or 4.0 waves)
+    long long want = (long long)c->sm_count * c->opt_rho_blocks;
+    long long nchunk = want / xtiles;
     if (nchunk > V / 16) nchunk = V / 16;
     if (nchunk > c->part_cap / X) nchunk = c->part_cap / X;
     if (nchunk > 65535) nchunk = 65535;

@@ -18,7 +18,7 @@
 #define SLDG_COPY_BIT (1 << 30)
 #define SLDG_S_MASK (SLDG_COPY_BIT - 1)
 
-enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5 };
+enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5, KIND_FUSED = 6 };
 
 // Polynomial coefficients of A_jl(alpha), B_jl(alpha) in powers of (alpha - 1/2), ascending, row-major
 // [2][K1*K1][SLDG_MAXPOLY]; the fp64 copy sits in __constant__ memory for the device-side table kernel.
@@ -83,6 +83,7 @@ struct sldg_ctx {
     double* dAB[SLDG_MAX_DIM];      //                                       [D_{dx+a}][2 K1^2]
     double tab_tau[SLDG_MAX_DIM];   // dt the cached table of x axis a was built for
     bool tab_valid[SLDG_MAX_DIM];
+    bool tab_safe[SLDG_MAX_DIM];    // every shift of the cached table is 0 or -1: a walk may run in place
     int* dS_hook; double* dAB_hook; long long hook_cap;   // test-hook tables (x axes)
     double* dFwdT[3];               // forward transfer+DFT matrices, transposed [n][m], re then im
     double* dInvT[3];               // inverse DFT+transfer matrices, transposed
@@ -118,6 +119,11 @@ struct sldg_ctx {
     int opt_axis0_impl;             // 0 = auto, 1 = per-warp pipelines, 2 = block-wide tiles, 3 = register walk
     int opt_walk_block;             // slow-axis kernel block size
     int opt_walk_vec;               // 0 = auto, 1, 2
+    int opt_fuse_x;                 // 1: x_1 and x_2 sweeps in one pass when the shape allows
+    int opt_fused_threads;          // fused kernel: threads per block (<= 256) = planes per block * D_0
+    int opt_inplace_walk;           // 1: slow-axis x sweeps may run in place when their table allows
+    int opt_rho_vec;                // 0 = auto (2 when aligned), 1
+    int opt_rho_blocks;             // rho kernel: 128-thread blocks per SM to aim for
 };
 
 // ---- host tables (sldg_tables.cpp)
@@ -134,6 +140,8 @@ cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout,
                                    const ShiftTable& t);
 cudaError_t sldg_launch_sweep_tma(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
                                   const ShiftTable& t);
+cudaError_t sldg_launch_sweep_fused(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
+                                    const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
 cudaError_t sldg_upload_poly(const ABPoly* p);
 cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB);
 cudaError_t sldg_launch_wv(sldg_ctx* c);

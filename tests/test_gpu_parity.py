@@ -240,3 +240,70 @@ def test_errors_are_reported_not_swallowed(P):
     assert L.sldg_create(C.byref(h2), 1, 1, (C.c_int * 2)(4, 4), 1, (C.c_double * 4)(0, 1, 0, 1)) == 0
     assert L.sldg_step(h2, C.c_void_p(f.data_ptr()), 0.1) == -4
     L.sldg_destroy(h2)
+
+
+# --------------------------------------------------------------- fused x1+x2 pass, in-place walks, step plans
+
+FUSE_GEOMS = [
+    (2, 2, [8, 8, 16, 16], 1),
+    (2, 2, [7, 5, 6, 9], 2),
+    (2, 2, [64, 9, 3, 4], 2),          # D_0 = 192: one plane per block
+    (2, 2, [5, 37, 4, 3], 0),
+    (2, 2, [3, 4, 3, 2], 4),
+    (2, 2, [6, 5, 2, 3], 3),
+    (2, 3, [6, 4, 5, 4, 3], 1),
+    (3, 3, [4, 3, 5, 3, 4, 2], 1),
+    (3, 3, [20, 7, 3, 2, 2, 2], 1),    # D_0 = 40: blocks straddle planes, ragged last block
+    (2, 2, [1, 1, 2, 3], 1),
+    (2, 2, [100, 3, 2, 2], 2),         # D_0 = 300 > 256 threads: falls back to separate sweeps
+]
+
+
+@pytest.mark.parametrize("geom", FUSE_GEOMS, ids=lambda g: f"{g[0]}x{g[1]}v-{'x'.join(map(str, g[2]))}-k{g[3]}")
+@pytest.mark.parametrize("tau", [0.013, 0.4, 7.7])
+def test_advect_x_plans_agree_bitwise_and_match_oracle(P, geom, tau):
+    """advect_x with the fused x1+x2 pass / separate sweeps, with and without in-place walks, and with fewer
+    planes per block: identical bits (same per-value arithmetic in the same order), and parity with the oracle.
+    tau = 0.013: |delta| < 1 everywhere (in-place walks allowed); 7.7: CFL > 1 (they are not)."""
+    dx, dv, cells, k = geom
+    g, o = make_pair(P, dx, dv, cells, k)
+    f0 = W.random_field(o.shape, seed=21 + k)
+    outs = []
+    for fuse, inplace, threads in ((1, 1, 256), (1, 0, 256), (0, 1, 256), (0, 0, 256), (1, 1, 64)):
+        g.set_option("fuse_x", fuse); g.set_option("inplace_walk", inplace); g.set_option("fused_threads", threads)
+        fg = f0.to(g.device).contiguous()
+        g.advect_x(fg, tau)
+        outs.append(fg.cpu().numpy())
+    for x in outs[1:]:
+        assert np.array_equal(outs[0], x)
+    assert rel_inf(outs[0], o.advect_x(f0.numpy(), tau)) <= TOL_SWEEP * dx
+
+
+def test_advect_x_integer_shifts_are_exact_in_every_plan(P):
+    """v nodes chosen so that v*tau/h_x is an integer on every line: the fused pass copies, bit for bit."""
+    # h_x = 0.25 on both x axes; v nodes of a k=0 grid on [-4,4] with 8 cells: -3.5..3.5; tau = 0.5 -> delta = 2 v
+    dom = [0, 1.0, 0, 1.5, -4.0, 4.0, -4.0, 4.0]
+    g, o = make_pair(P, 2, 2, [4, 6, 8, 8], 0, dom)
+    f0 = W.random_field(o.shape, seed=4)
+    f0.view(-1)[::5] = -0.0
+    want = o.advect_x(f0.numpy(), 0.5)
+    for fuse in (1, 0):
+        g.set_option("fuse_x", fuse)
+        fg = f0.to(g.device).contiguous()
+        g.advect_x(fg, 0.5)
+        assert np.array_equal(fg.cpu().numpy().view(np.int64), want.view(np.int64))
+
+
+@pytest.mark.parametrize("cfg", small_cfgs()[1:], ids=lambda c: c["name"])
+def test_step_plans_agree_bitwise(P, cfg):
+    g, o = pair_of_cfg(P, cfg)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    outs = []
+    for fuse, inplace in ((1, 1), (1, 0), (0, 1), (0, 0)):
+        g.set_option("fuse_x", fuse); g.set_option("inplace_walk", inplace)
+        fg = f0.to(g.device).contiguous()
+        for _ in range(3):
+            g.step(fg, cfg["dt"])
+        outs.append(fg.cpu().numpy())
+    for x in outs[1:]:
+        assert np.array_equal(outs[0], x)
