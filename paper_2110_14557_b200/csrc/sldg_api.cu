@@ -95,6 +95,7 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
+    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
@@ -425,7 +426,9 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     int a = 0;
     if (p.fused) {
         sldg_ev_begin(c, KIND_FUSED, 0);
-        cudaError_t e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        cudaError_t e = cudaErrorNotSupported;
+        if (c->opt_fused_impl != 2) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        if (e == cudaErrorNotSupported) e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
         sldg_ev_end(c);
         c->launches++;
         if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
@@ -446,6 +449,10 @@ extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
     int r = check_f(c, f);
     if (r) return r;
     double *cur = f, *oth = c->f2;
+    if (c->opt_x_copy) {                                // testing knob: the odd-parity plan (for dim_x = 2 the only
+        if ((r = advect_x_impl(c, &cur, &oth, dt, true))) return r;   // one with the fused pass) plus one device copy
+        return copy_back(c, f, cur);
+    }
     return advect_x_impl(c, &cur, &oth, dt, false);     // ends in f: no copy
 }
 
@@ -715,6 +722,12 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "fuse_x")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse_x = (int)value; return SLDG_OK; }
     if (!strcmp(name, "inplace_walk")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_inplace_walk = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fused_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_fused_threads = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "x_copy")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_copy = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fused_impl")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fused_impl = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "cell_threads")) { if (value < 1 || value > 128) return SLDG_EINVAL; c->opt_cell_threads = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "cell_rows")) { if (value < 0 || value > 1024) return SLDG_EINVAL; c->opt_cell_rows = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "cell_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_cell_bytes = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "cell_stages")) { if (value < 2 || value > 6) return SLDG_EINVAL; c->opt_cell_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "rho_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_rho_vec = (int)value; return SLDG_OK; }
     if (!strcmp(name, "rho_blocks")) { if (value < 1 || value > 64) return SLDG_EINVAL; c->opt_rho_blocks = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_walk_vec = (int)value; return SLDG_OK; }

@@ -122,6 +122,12 @@ struct sldg_ctx {
     int opt_fuse_x;                 // 1: x_1 and x_2 sweeps in one pass when the shape allows
     int opt_fused_threads;          // fused kernel: threads per block (<= 256) = planes per block * D_0
     int opt_inplace_walk;           // 1: slow-axis x sweeps may run in place when their table allows
+    int opt_fused_impl;             // 0 = auto (cell kernel, else node kernel), 1 = cell-per-thread TMA kernel, 2 = node-per-thread kernel
+    int opt_x_copy;                 // 1: sldg_advect_x runs the plan that ends in the workspace, then copies back (tests)
+    int opt_cell_threads;           // fused cell kernel: threads per block (<= 128) = planes per block * N_0
+    int opt_cell_rows;              // fused cell kernel: x_2 cells per chunk (0 = from opt_cell_bytes)
+    int opt_cell_bytes;             // fused cell kernel: target bytes of one input stage (all planes of the block)
+    int opt_cell_stages;            // fused cell kernel: input stages (2..6)
     int opt_rho_vec;                // 0 = auto (2 when aligned), 1
     int opt_rho_blocks;             // rho kernel: 128-thread blocks per SM to aim for
 };
@@ -142,6 +148,8 @@ cudaError_t sldg_launch_sweep_tma(sldg_ctx* c, const double* fin, double* fout, 
                                   const ShiftTable& t);
 cudaError_t sldg_launch_sweep_fused(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
                                     const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
+cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
+                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
 cudaError_t sldg_upload_poly(const ABPoly* p);
 cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB);
 cudaError_t sldg_launch_wv(sldg_ctx* c);

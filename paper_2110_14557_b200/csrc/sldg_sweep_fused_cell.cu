@@ -1,0 +1,287 @@
+// sldg_sweep_fused_cell.cu -- the x_1 and x_2 sweeps of an x advection in ONE pass over f, sm_100a: the production
+// kernel of the fused pass (sldg_sweep_fused.cu keeps the node-per-thread variant as the fallback).
+//
+// eq. (3), reading B, applied twice: first along x_1 (axis 0, contiguous), then along x_2 (axis 1).  The x
+// sweeps commute and act on different axes, so both are applied while a value passes through the SM once:
+// 16 B of HBM traffic per value for TWO sweeps.
+//
+// The array is seen as [planes q][N_1 cells][k+1 rows][D_0] with a row = one contiguous x_1 line, so the k+1 rows
+// of CR consecutive x_2 cells of one plane are ONE contiguous chunk.  A block owns PB planes:
+//
+//   plane leader:  cp.async.bulk global -> shared (1-D TMA, mbarrier complete_tx) of its plane's chunks into a
+//                  ring of input stages, issued `stages` chunks ahead: the HBM latency is covered by bytes in
+//                  flight, not by occupancy or registers;
+//   every thread:  owns ONE x_1 CELL of one plane.  Per x_2 cell it reads its two x_1 donor cells of each of the
+//                  k+1 rows from shared memory (2 shared loads per value instead of 2(k+1) with a thread per
+//                  node), applies A_1, B_1, and then WALKS along x_2 exactly like sldg_sweep_walk.cu with a
+//                  (k+1) x (k+1) block of x_1-swept values in registers (previous cell kept, first cell kept for
+//                  the periodic wrap), writing output cell (j + s_2 + 1) mod N_1 into a shared output stage;
+//   plane leader:  cp.async.bulk shared -> global of the CR output cells (two copies when they wrap around).
+//
+// One __syncthreads per chunk releases the input stage and publishes the output stage.  Every value is read once
+// and written once.  The shift of x_1 depends on the plane's v_1 node, that of x_2 on its v_2 node.  Out of place
+// only (fin != fout); D_0 must be even (16-byte rule of the bulk copies).
+#include "sldg_async.h"
+#include "sldg_internal.h"
+
+namespace {
+
+using namespace sldg_async;
+
+struct CellParams {
+    const double* fin;
+    double* fout;
+    long long planes;             // prod of D_b, b >= 2
+    int N0, N1, PB, CR, stages;   // cells along x_1, x_2; planes per block; x_2 cells per chunk; input stages
+    long long sdiv0, sdiv1;       // shift index of plane q: (q / sdiv) % smod, per axis
+    long long smod0, smod1;
+    ShiftTable t0, t1;
+};
+
+constexpr int OST = 2;            // output stages
+
+template <int K1> struct CellV {
+    double v[K1];
+    __device__ __forceinline__ void load(const double* p)
+    {
+        if constexpr (K1 % 2 == 0) {
+#pragma unroll
+            for (int j = 0; j < K1; j += 2) {
+                double2 t = *reinterpret_cast<const double2*>(p + j);
+                v[j] = t.x; v[j + 1] = t.y;
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < K1; j++) v[j] = p[j];
+        }
+    }
+    __device__ __forceinline__ void store(double* p) const
+    {
+        if constexpr (K1 % 2 == 0) {
+#pragma unroll
+            for (int j = 0; j < K1; j += 2) *reinterpret_cast<double2*>(p + j) = make_double2(v[j], v[j + 1]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < K1; j++) p[j] = v[j];
+        }
+    }
+};
+
+template <int K1, int MINB>
+__global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellParams P)
+{
+    constexpr int NN = K1 * K1;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int N0 = P.N0, N1 = P.N1, D0 = N0 * K1, CR = P.CR, ST = P.stages;
+    const int PC = CR * K1 * D0;                       // doubles of one plane's chunk
+    const int SS = P.PB * PC;                          // doubles of one stage
+    double* const sin_ = reinterpret_cast<double*>(smem_raw);
+    double* const sout = sin_ + (size_t)ST * SS;
+    const uint32_t sin_s = smem_u32(sin_), sout_s = smem_u32(sout);
+    const uint32_t bars_s = smem_u32(sout + (size_t)OST * SS);
+
+    const int t = threadIdx.x;
+    const int pl = t / N0, i = t - pl * N0;
+    const long long q0 = (long long)blockIdx.x * P.PB;
+    const long long q = q0 + pl;
+    const bool live = q < P.planes && pl < P.PB;
+    const bool leader = live && i == 0;
+    const int nlive = (int)min((long long)P.PB, P.planes - q0);
+    const long long qq = live ? q : P.planes - 1;      // dead threads shadow the last plane (no copies, no stores)
+    const long long D1 = (long long)N1 * K1;
+    const double* const gin = P.fin + qq * D1 * D0;
+    double* const gout = P.fout + qq * D1 * D0;
+    const int NCH = 1 + (N1 - 1 + CR - 1) / CR;        // input chunks: cell 0 alone, then CR cells each
+    const uint32_t cell_bytes = (uint32_t)(K1 * D0) * 8u;
+
+    auto issue_load = [&](int j) {                     // plane leaders only
+        if (leader && j < NCH) {
+            const int st = j % ST;
+            const int c0 = (j == 0) ? 0 : (j - 1) * CR + 1;
+            const int nc = (j == 0) ? 1 : min(CR, N1 - c0);
+            const uint32_t bar = bars_s + (uint32_t)st * 8u;
+            mbar_expect_tx(bar, nc * cell_bytes);
+            bulk_load(sin_s + (uint32_t)(st * SS + pl * PC) * 8u, gin + (long long)c0 * K1 * D0, nc * cell_bytes, bar);
+        }
+    };
+
+    if (t == 0) {
+        for (int st = 0; st < ST; st++) mbar_init(bars_s + (uint32_t)st * 8u, nlive);
+        mbar_init_fence();
+    }
+    __syncthreads();
+    for (int j = 0; j < ST; j++) issue_load(j);
+
+    // ---- x_1: A_1, B_1 and the offsets of the two donor cells inside a row
+    double A1[NN], B1[NN];
+    int oa, ob;
+    bool cp1;
+    {
+        const long long idx = (qq / P.sdiv0) % P.smod0;
+        const int sv = __ldg(P.t0.S + idx);
+        cp1 = (sv & SLDG_COPY_BIT) != 0;
+        const int s = sv & SLDG_S_MASK;
+        int ia = i - s; if (ia < 0) ia += N0;
+        int ib = ia - 1; if (ib < 0) ib += N0;
+        oa = ia * K1; ob = ib * K1;
+        const double* ab = P.t0.AB + idx * P.t0.strideIdx;
+#pragma unroll
+        for (int m = 0; m < NN; m++) {
+            A1[m] = __ldg(ab + m * P.t0.strideM);
+            B1[m] = __ldg(ab + (NN + m) * P.t0.strideM);
+        }
+    }
+    // ---- x_2: A_2, B_2, shift
+    double A2[NN], B2[NN];
+    int s2;
+    bool cp2;
+    {
+        const long long idx = (qq / P.sdiv1) % P.smod1;
+        const int sv = __ldg(P.t1.S + idx);
+        cp2 = (sv & SLDG_COPY_BIT) != 0;
+        s2 = sv & SLDG_S_MASK;
+        const double* ab = P.t1.AB + idx * P.t1.strideIdx;
+#pragma unroll
+        for (int m = 0; m < NN; m++) {
+            A2[m] = __ldg(ab + m * P.t1.strideM);
+            B2[m] = __ldg(ab + (NN + m) * P.t1.strideM);
+        }
+    }
+
+    // x_1-swept (k+1) x (k+1) block [x_2 node j2][x_1 node j1] of this thread's cell from the k+1 rows at `rows`
+    auto swept = [&](const double* rows, double (&N)[NN]) {
+#pragma unroll
+        for (int j2 = 0; j2 < K1; j2++) {
+            const double* row = rows + j2 * D0;
+            CellV<K1> a, b;
+            a.load(row + oa);
+            b.load(row + ob);
+#pragma unroll
+            for (int j1 = 0; j1 < K1; j1++) {
+                double acc = 0.0;
+#pragma unroll
+                for (int m = 0; m < K1; m++) acc += A1[j1 * K1 + m] * a.v[m];
+#pragma unroll
+                for (int m = 0; m < K1; m++) acc += B1[j1 * K1 + m] * b.v[m];
+                N[j2 * K1 + j1] = cp1 ? a.v[j1] : acc;
+            }
+        }
+    };
+
+    double first[NN], prev[NN];
+    // chunk 0: cell 0 alone
+    mbar_wait(bars_s, 0u);
+    swept(sin_ + pl * PC, first);
+#pragma unroll
+    for (int m = 0; m < NN; m++) prev[m] = first[m];
+    __syncthreads();
+    issue_load(ST);
+
+    const int H = (N1 + CR - 1) / CR;                  // output groups of CR cells
+    int io0 = s2 + 1; if (io0 >= N1) io0 -= N1;        // first output cell of the group
+    for (int h = 0; h < H; h++) {
+        const int j = h + 1;                           // input chunk that feeds this group
+        const int st = j % ST;
+        const int nin = min(CR, N1 - 1 - h * CR);      // cells of that chunk (<= 0: none, the wrap cell is `first`)
+        const int nout = min(CR, N1 - h * CR);
+        if (nin > 0) mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
+        const double* ibase = sin_ + st * SS + pl * PC;
+        double* obase = sout + (h & 1) * SS + pl * PC + i * K1;
+        for (int e = 0; e < nout; e++) {
+            double nxt[NN];
+            if (e < nin) swept(ibase + e * K1 * D0, nxt);
+            else {
+#pragma unroll
+                for (int m = 0; m < NN; m++) nxt[m] = first[m];
+            }
+#pragma unroll
+            for (int j2 = 0; j2 < K1; j2++) {
+                CellV<K1> r;
+#pragma unroll
+                for (int j1 = 0; j1 < K1; j1++) {
+                    double acc = 0.0;
+#pragma unroll
+                    for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
+#pragma unroll
+                    for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * prev[l * K1 + j1];
+                    r.v[j1] = cp2 ? nxt[j2 * K1 + j1] : acc;
+                }
+                r.store(obase + (e * K1 + j2) * D0);
+            }
+#pragma unroll
+            for (int m = 0; m < NN; m++) prev[m] = nxt[m];
+        }
+        fence_async_smem();                            // generic-proxy writes of the output stage -> async proxy
+        if (leader) bulk_wait_read<0>();               // the store of group h-1 has left its output stage
+        __syncthreads();
+        if (leader) {
+            const uint32_t src = sout_s + (uint32_t)((h & 1) * SS + pl * PC) * 8u;
+            const int n1 = min(nout, N1 - io0);
+            bulk_store(gout + (long long)io0 * K1 * D0, src, (uint32_t)n1 * cell_bytes);
+            if (nout > n1) bulk_store(gout, src + (uint32_t)n1 * cell_bytes, (uint32_t)(nout - n1) * cell_bytes);
+            bulk_commit();
+        }
+        issue_load(j + ST);
+        io0 += CR; if (io0 >= N1) io0 -= N1;
+    }
+    if (leader) bulk_wait_read<0>();                   // shared memory must outlive the bulk stores reading it
+}
+
+template <int K1, int MINB>
+cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem)
+{
+    auto kern = sweep_fused_cell_kernel<K1, MINB>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const long long grid = (P.planes + P.PB - 1) / P.PB;
+    if (grid > 0x7fffffffLL) return cudaErrorNotSupported;
+    kern<<<(unsigned)grid, threads, smem, c->stream>>>(P);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// g0, g1: geometry of axis 0 and axis 1.  Returns cudaErrorNotSupported when the shape does not fit (the caller
+// falls back to the node-per-thread fused kernel, then to separate sweeps).
+cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
+                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+{
+    if (g1.outer == 0) return cudaSuccess;
+    const long long D0 = (long long)g0.N * g0.K1, D1 = (long long)g1.N * g1.K1;
+    const int K1 = g0.K1;
+    if (fin == fout || g1.inner != D0 || g0.mode != 0 || g1.mode != 0 || g0.sdiv % D1 != 0) return cudaErrorNotSupported;
+    if (K1 > 4 || (D0 & 1) || g0.N > 128) return cudaErrorNotSupported;
+    if ((((uintptr_t)fin) | ((uintptr_t)fout)) & 15) return cudaErrorNotSupported;
+    CellParams P;
+    P.fin = fin; P.fout = fout; P.planes = g1.outer;
+    P.N0 = g0.N; P.N1 = g1.N;
+    long long PB = c->opt_cell_threads / g0.N;
+    if (PB < 1) PB = 1;
+    if (PB > P.planes) PB = P.planes;
+    const long long cellb = (long long)K1 * D0 * 8;            // bytes of one x_2 cell of one plane
+    // Measured on B200 (cfg2-5): 64-thread blocks, 2 input stages of about 9 KB each, i.e. many small resident
+    // blocks, reach the copy rate; larger stages or deeper rings lose occupancy and run slower.
+    long long CR = c->opt_cell_rows > 0 ? c->opt_cell_rows : c->opt_cell_bytes / (PB * cellb);
+    if (CR < 1) CR = 1;
+    if (CR > g1.N) CR = g1.N;
+    int stages = c->opt_cell_stages;
+    const size_t smem_max = 227 * 1024;
+    auto smem_of = [&](long long pb, long long cr, int st) { return (size_t)(st + OST) * pb * cr * cellb + 8 * st + 16; };
+    while (smem_of(PB, CR, stages) > smem_max && CR > 1) CR--;
+    while (smem_of(PB, CR, stages) > smem_max && stages > 2) stages--;
+    while (smem_of(PB, CR, stages) > smem_max && PB > 1) PB--;
+    if (smem_of(PB, CR, stages) > smem_max) return cudaErrorNotSupported;
+    P.PB = (int)PB; P.CR = (int)CR; P.stages = stages;
+    P.sdiv0 = g0.sdiv / D1; P.smod0 = g0.smod;       // axis-0 lines are numbered row + D_1 * plane
+    P.sdiv1 = g1.sdiv; P.smod1 = g1.smod;
+    P.t0 = t0; P.t1 = t1;
+    const int threads = (int)(PB * g0.N);
+    const size_t smem = smem_of(PB, CR, stages);
+    switch (K1) {
+    case 1: return launch<1, 4>(c, P, threads, smem);
+    case 2: return launch<2, 4>(c, P, threads, smem);
+    case 3: return launch<3, 3>(c, P, threads, smem);
+    case 4: return launch<4, 2>(c, P, threads, smem);
+    }
+    return cudaErrorNotSupported;
+}

@@ -255,6 +255,8 @@ FUSE_GEOMS = [
     (3, 3, [4, 3, 5, 3, 4, 2], 1),
     (3, 3, [20, 7, 3, 2, 2, 2], 1),    # D_0 = 40: blocks straddle planes, ragged last block
     (2, 2, [1, 1, 2, 3], 1),
+    (2, 2, [6, 1, 3, 2], 1),           # a single x_2 cell: the wrap cell is the only donor pair
+    (2, 2, [64, 64, 1, 2], 2),         # BASELINE cfg2's x plane
     (2, 2, [100, 3, 2, 2], 2),         # D_0 = 300 > 256 threads: falls back to separate sweeps
 ]
 
@@ -269,8 +271,18 @@ def test_advect_x_plans_agree_bitwise_and_match_oracle(P, geom, tau):
     g, o = make_pair(P, dx, dv, cells, k)
     f0 = W.random_field(o.shape, seed=21 + k)
     outs = []
-    for fuse, inplace, threads in ((1, 1, 256), (1, 0, 256), (0, 1, 256), (0, 0, 256), (1, 1, 64)):
+    # (fuse_x, inplace_walk, fused_threads, fused_impl, cell_rows, cell_threads, cell_stages, x_copy)
+    # x_copy = 1: the plan of the other buffer parity + one copy (for dim_x = 2 the fused pass runs only there)
+    plans = ((1, 1, 256, 0, 0, 128, 3, 0), (1, 0, 256, 0, 0, 128, 3, 0), (0, 1, 256, 0, 0, 128, 3, 0),
+             (0, 0, 256, 0, 0, 128, 3, 0), (0, 0, 256, 0, 0, 128, 3, 1), (1, 1, 256, 0, 0, 128, 3, 1),
+             (1, 1, 256, 2, 0, 128, 3, 0), (1, 1, 64, 2, 0, 128, 3, 1), (1, 1, 256, 2, 0, 128, 3, 1),     # node-per-thread fused kernel
+             (1, 1, 256, 1, 1, 128, 2, 0), (1, 1, 256, 1, 1, 128, 2, 1), (1, 1, 256, 1, 3, 64, 3, 1),     # cell-per-thread fused kernel
+             (1, 1, 256, 1, 5, 96, 4, 1), (1, 1, 256, 1, 64, 32, 6, 1))
+    for fuse, inplace, threads, impl, rows, cthreads, cstages, xcopy in plans:
         g.set_option("fuse_x", fuse); g.set_option("inplace_walk", inplace); g.set_option("fused_threads", threads)
+        g.set_option("x_copy", xcopy)
+        g.set_option("fused_impl", impl); g.set_option("cell_rows", rows); g.set_option("cell_threads", cthreads)
+        g.set_option("cell_stages", cstages)
         fg = f0.to(g.device).contiguous()
         g.advect_x(fg, tau)
         outs.append(fg.cpu().numpy())
@@ -287,8 +299,8 @@ def test_advect_x_integer_shifts_are_exact_in_every_plan(P):
     f0 = W.random_field(o.shape, seed=4)
     f0.view(-1)[::5] = -0.0
     want = o.advect_x(f0.numpy(), 0.5)
-    for fuse in (1, 0):
-        g.set_option("fuse_x", fuse)
+    for fuse, impl, xcopy in ((1, 0, 0), (1, 0, 1), (1, 1, 1), (1, 2, 1), (0, 0, 0)):
+        g.set_option("fuse_x", fuse); g.set_option("fused_impl", impl); g.set_option("x_copy", xcopy)
         fg = f0.to(g.device).contiguous()
         g.advect_x(fg, 0.5)
         assert np.array_equal(fg.cpu().numpy().view(np.int64), want.view(np.int64))
@@ -299,8 +311,8 @@ def test_step_plans_agree_bitwise(P, cfg):
     g, o = pair_of_cfg(P, cfg)
     f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
     outs = []
-    for fuse, inplace in ((1, 1), (1, 0), (0, 1), (0, 0)):
-        g.set_option("fuse_x", fuse); g.set_option("inplace_walk", inplace)
+    for fuse, inplace, impl in ((1, 1, 0), (1, 0, 0), (0, 1, 0), (0, 0, 0), (1, 1, 2)):
+        g.set_option("fuse_x", fuse); g.set_option("inplace_walk", inplace); g.set_option("fused_impl", impl)
         fg = f0.to(g.device).contiguous()
         for _ in range(3):
             g.step(fg, cfg["dt"])
