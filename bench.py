@@ -173,15 +173,15 @@ def run_reference(args, cfg, rank, world):
 
 
 # ----------------------------------------------------------------------------- the CUDA path
-def ncu_traffic(cfg_name):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+def ncu_traffic(cfg_name, kernel):
+    """dram bytes per launch of `kernel` on workload `cfg_name` from the committed ncu capture (profiles/), or None."""
     p = os.path.join(ROOT, "profiles", "traffic.txt")
     try:
         with open(p) as fh:
             for ln in fh:
                 if ln.startswith("{"):
                     d = json.loads(ln)
-                    if d.get("workload") == cfg_name:
+                    if d.get("workload") == cfg_name and d.get("kernel") == kernel:
                         return d
     except Exception:
         pass
@@ -245,7 +245,7 @@ def run_ours(args, cfg, rank, world, local):
     # dominant kernel = the one with the largest share of the step
     kn, (kl, kms) = max(((k, v) for k, v in kinds.items() if k.startswith("sweep")), key=lambda kv: kv[1][1])
     achieved = sweep_bytes(cfg) / (kms / kl * 1e-3) / 1e9
-    tr = ncu_traffic(cfg["name"])
+    tr = ncu_traffic(cfg["name"], kn)
     roofline = {"bound": "hbm", "kernel": kn, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": tr.get("traffic_bytes_per_launch") if tr else None,
                 "algorithmic_bytes_per_launch": sweep_bytes(cfg), "peak_source": peak_src,
@@ -298,11 +298,18 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--workload", type=str, default=None, help="a workload by name, incl. the NEXT-row cases "
+                    "(bot_5d_k3_16, bot_6d_k3_9: the paper's bump-on-tail case, 4th order)")
+    ap.add_argument("--cfl", type=float, default=None, help="choose dt so that the largest x shift is CFL cells (PAPER.md:351)")
     ap.add_argument("--cells", type=str, default=None, help="override cells, e.g. 16,16,16,16 (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     import workloads as W
     cfg = W.CONFIGS[args.config]
+    if args.workload:
+        cfg = {c["name"]: c for c in W.CONFIGS + W.NEXT_CONFIGS}[args.workload]
+    if args.cfl:
+        cfg = W.with_cfl(cfg, args.cfl)
     if args.cells:
         cfg = W.scaled(cfg, [int(c) for c in args.cells.split(",")])
     if args.impl == "reference":

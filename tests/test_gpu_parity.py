@@ -209,6 +209,29 @@ def test_ten_strang_steps(P, cfg):
     assert abs(g.electric_energy(Eg) - o.electric_energy(Eg.cpu().numpy())) <= 1e-12 * o.electric_energy(E_o) + 1e-30
 
 
+def next_cfgs():
+    """the paper's bump-on-tail case (4th order) and CFL > 1 steps
+    (PAPER.md:351-357), on grids the oracle finishes in seconds."""
+    n = W.NEXT_CONFIGS
+    b4 = n[0]
+    return [b4, W.with_cfl(b4, 2.5), W.with_cfl(b4, 5.0),
+            W.scaled(n[1], [4, 3, 4, 3, 2]), W.with_cfl(W.scaled(n[2], [3, 2, 2, 3, 2, 2]), 3.0)]
+
+
+@pytest.mark.parametrize("cfg", next_cfgs(), ids=lambda c: c["name"])
+def test_bump_on_tail_and_cfl_above_one_ten_strang_steps(P, cfg):
+    g, o = pair_of_cfg(P, cfg)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    fg, fo = f0.to(g.device).contiguous(), f0.numpy()
+    m0 = g.mass(fg)
+    for _ in range(10):
+        g.step(fg, cfg["dt"])
+        fo, rho_o, E_o = o.step(fo, cfg["dt"])
+    assert rel_inf(fg.cpu().numpy(), fo) <= TOL_STEPS
+    assert np.abs(g.last_E().cpu().numpy() - E_o).max() <= TOL_STEPS * max(1.0, np.abs(E_o).max())
+    assert abs(g.mass(fg) - m0) <= 1e-12 * abs(m0)
+
+
 def test_step_host_matches_step(P):
     cfg = W.CONFIGS[0]
     g, o = pair_of_cfg(P, cfg)

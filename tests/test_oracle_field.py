@@ -240,3 +240,34 @@ def test_p12_linear_landau_damping_rate():
     omega = math.pi / np.mean(np.diff(tp))
     assert abs(gamma - (-0.1533)) < 0.02 * 0.1533 * 2, gamma
     assert abs(omega - 1.4156) < 0.02 * 1.4156, omega
+
+
+# --------------------------------------------------------------- NEXT rows: bump-on-tail data, CFL > 1 steps
+
+def test_bump_on_tail_density_is_one_plus_eps_sum_cos():
+    """int (0.9 e^{-v^2/2} + 0.2 e^{-2(v-4.5)^2}) dv / sqrt(2 pi) = 0.9 + 0.2 sqrt(pi/2)/sqrt(2 pi) = 1,
+    so rho(0, x) = 1 + 0.03 sum_i cos(0.3 x_i) (velocity truncation at |v| = 9 is far below round-off of the
+    quadrature error).  Pins the workload generator's normalisation and the density weights together."""
+    cfg = W.scaled(W.NEXT_CONFIGS[0], [6, 5, 24, 24])
+    orc = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    c = coords(orc)
+    f0 = W.initial_data(cfg, c).numpy()
+    rho = orc.density(f0)
+    want = 1.0 + 0.03 * (np.cos(0.3 * c[0])[None, :] + np.cos(0.3 * c[1])[:, None])
+    assert np.abs(rho - want).max() < 1e-7
+
+
+@pytest.mark.parametrize("cfl", [1.0, 2.5, 5.0])
+def test_cfl_above_one_steps_conserve_mass_and_stay_bounded(cfl):
+    """the scheme is run at CFL 1..5 (no stability limit).  With a shift of several cells per
+    sweep a Strang step still conserves mass to round-off and does not amplify the data."""
+    cfg = W.with_cfl(W.scaled(W.NEXT_CONFIGS[0], [6, 5, 8, 8]), cfl)
+    orc = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    f = W.initial_data(cfg, coords(orc)).numpy()
+    m0, a0 = orc.mass(f), np.abs(f).max()
+    hx = (cfg["domain"][1] - cfg["domain"][0]) / cfg["cells"][0]
+    assert abs(9.0 * cfg["dt"] / 2 / hx - cfl) < 1e-12
+    for _ in range(4):
+        f, _, _ = orc.step(f, cfg["dt"])
+    assert abs(orc.mass(f) - m0) <= 1e-13 * abs(m0)
+    assert np.abs(f).max() <= 1.5 * a0

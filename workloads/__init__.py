@@ -13,7 +13,8 @@ axis order x_1..x_dx, v_1..v_dv, x_1 fastest.  As a torch tensor the shape is
 (D_{d-1}, ..., D_1, D_0).
 
 The Landau data follow the paper (alpha=0.01, k=0.5,
-[0,4pi]^dx x [-6,6]^dv); the two-stream data are BASELINE.json's (not in the paper).
+[0,4pi]^dx x [-6,6]^dv); the two-stream data are BASELINE.json's (not in the paper);
+the bump-on-tail data are the paper's second validation case.
 No dataset or benchmark suite is involved.
 """
 import math
@@ -41,6 +42,34 @@ CONFIGS = [
          domain=[0, 10 * _PI] * 3 + [-6, 6] * 3, dt=0.05, steps=10, ic="two_stream",
          ic_args=dict(eps=1e-3, k=0.2, v0=2.4)),
 ]
+
+# the paper's own second validation case (bump-on-tail, on
+# [0,20pi/3]^dx x [-9,9]^dv, 4th order = degree 3, time step 0.1) and CFL > 1 time steps.
+# The paper ran 144^5 / 72^6 degrees of freedom on 32 / 64 GPUs; these are sized for one B200.
+_L = 20 * _PI / 3
+NEXT_CONFIGS = [
+    dict(name="bot_4d_k3_small", dim_x=2, dim_v=2, cells=[6, 5, 8, 7], degree=3,
+         domain=[0, _L, 0, _L, -9, 9, -9, 9], dt=0.1, steps=10, ic="bump_on_tail",
+         ic_args=dict(eps=0.03, k=0.3)),
+    dict(name="bot_5d_k3_16", dim_x=2, dim_v=3, cells=[16] * 5, degree=3,
+         domain=[0, _L, 0, _L, -9, 9, -9, 9, -9, 9], dt=0.1, steps=10, ic="bump_on_tail",
+         ic_args=dict(eps=0.03, k=0.3)),
+    dict(name="bot_6d_k3_9", dim_x=3, dim_v=3, cells=[9] * 6, degree=3,
+         domain=[0, _L] * 3 + [-9, 9] * 3, dt=0.1, steps=10, ic="bump_on_tail",
+         ic_args=dict(eps=0.03, k=0.3)),
+]
+
+
+def with_cfl(cfg, cfl):
+    """Same problem with the time step chosen so that the largest x shift max|v| (dt/2) / h_x is `cfl` cells
+    (PAPER.md:351-357 runs CFL 1..5)."""
+    out = dict(cfg)
+    dx = cfg["dim_x"]
+    vmax = max(abs(b) for b in cfg["domain"][2 * dx:])
+    hx = min((cfg["domain"][2 * a + 1] - cfg["domain"][2 * a]) / cfg["cells"][a] for a in range(dx))
+    out["dt"] = 2.0 * cfl * hx / vmax
+    out["name"] = cfg["name"] + f"_cfl{cfl:g}"
+    return out
 
 
 def scaled(cfg, cells):
@@ -103,6 +132,15 @@ def initial_data(cfg, coords, device="cpu", out=None):
         X = X + a["eps"] * _outer_x_first(f)
         g1 = torch.exp(-0.5 * (vs[0] - a["v0"]) ** 2) + torch.exp(-0.5 * (vs[0] + a["v0"]) ** 2)
         V = _outer_x_first([g1] + [torch.exp(-0.5 * t * t) for t in vs[1:]]) / (2 * (2 * _PI) ** (dv / 2))
+    elif cfg["ic"] == "bump_on_tail":
+        # (0.9 exp(-v1^2/2) + 0.2 exp(-2 (v1-4.5)^2)) exp(-sum_{i>=2} v_i^2/2) / (2 pi)^{dv/2}
+        #               * (1 + 0.03 sum_i cos(0.3 x_i))
+        for j in range(dx):
+            f = [torch.ones_like(t) for t in xs]
+            f[j] = torch.cos(a["k"] * xs[j])
+            X = X + a["eps"] * _outer_x_first(f)
+        g1 = 0.9 * torch.exp(-0.5 * vs[0] ** 2) + 0.2 * torch.exp(-2.0 * (vs[0] - 4.5) ** 2)
+        V = _outer_x_first([g1] + [torch.exp(-0.5 * t * t) for t in vs[1:]]) / (2 * _PI) ** (dv / 2)
     else:
         raise ValueError(cfg["ic"])
     Vb = V.reshape(tuple(V.shape) + (1,) * dx)
