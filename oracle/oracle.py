@@ -40,6 +40,13 @@ def lib():
             "orc_step": (None, [vp, dp, dp, dp, dp, C.c_double]),
             "orc_mass": (C.c_double, [vp, dp]),
             "orc_electric_energy": (C.c_double, [vp, dp]),
+            "orc_lagrange_deriv": (C.c_double, [C.c_int, dp, C.c_int, C.c_double]),
+            "orc_sipg_sigma_default": (C.c_double, [C.c_int]),
+            "orc_sipg_MB": (None, [C.c_int, C.c_double, dp, dp]),
+            "orc_sipg_apply": (None, [vp, C.c_double, dp, dp]),
+            "orc_sipg_rhs": (None, [vp, dp, dp]),
+            "orc_grad_phi": (None, [vp, dp, dp]),
+            "orc_poisson_cg": (C.c_int, [vp, C.c_double, dp, dp, dp, C.c_double, C.c_int, dp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(_lib, name)
@@ -77,6 +84,22 @@ def sweep_line(k, u, delta):
     out = np.empty_like(u)
     lib().orc_sweep_line(k, n, float(delta), _p(u), _p(out), 1)
     return out
+
+
+def lagrange_deriv(xi, l, z):
+    xi = np.ascontiguousarray(xi, dtype=np.float64)
+    return lib().orc_lagrange_deriv(len(xi), _p(xi), l, float(z))
+
+
+def sipg_sigma_default(k):
+    return lib().orc_sipg_sigma_default(k)
+
+
+def sipg_MB(k, sigma):
+    """M, B of the SIPG block-tridiagonal matrix (reading I)."""
+    M, B = np.empty((k + 1, k + 1)), np.empty((k + 1, k + 1))
+    lib().orc_sipg_MB(k, float(sigma), _p(M), _p(B))
+    return M, B
 
 
 class Oracle:
@@ -166,3 +189,34 @@ class Oracle:
 
     def electric_energy(self, E):
         return lib().orc_electric_energy(self._h, _p(np.ascontiguousarray(E, dtype=np.float64).reshape(-1)))
+
+    # ---- CGdG Poisson solver
+    def sipg_apply(self, u, sigma=None):
+        sigma = sipg_sigma_default(self.k) if sigma is None else sigma
+        u = np.ascontiguousarray(u, dtype=np.float64).reshape(-1)
+        out = np.empty(self.X)
+        lib().orc_sipg_apply(self._h, float(sigma), _p(u), _p(out))
+        return out.reshape(self.xshape)
+
+    def sipg_rhs(self, rho):
+        r = np.ascontiguousarray(rho, dtype=np.float64).reshape(-1)
+        b = np.empty(self.X)
+        lib().orc_sipg_rhs(self._h, _p(r), _p(b))
+        return b.reshape(self.xshape)
+
+    def grad_phi(self, phi):
+        u = np.ascontiguousarray(phi, dtype=np.float64).reshape(-1)
+        E = np.empty(self.dx * self.X)
+        lib().orc_grad_phi(self._h, _p(u), _p(E))
+        return E.reshape((self.dx,) + self.xshape)
+
+    def poisson_cg(self, rho, phi0=None, tol=1e-3, maxiter=None, sigma=None):
+        """Algorithm 1 from the starting vector phi0 (zeros if None).  Returns (E, phi, iterations, relres)."""
+        sigma = sipg_sigma_default(self.k) if sigma is None else sigma
+        if maxiter is None:
+            maxiter = 4 * int(round(self.X ** (1.0 / self.dx))) + 20         # PAPER.md:567, safety factor 4
+        r = np.ascontiguousarray(rho, dtype=np.float64).reshape(-1)
+        phi = np.zeros(self.X) if phi0 is None else np.array(phi0, dtype=np.float64, order="C").reshape(-1)
+        E, info = np.empty(self.dx * self.X), np.empty(2)
+        it = lib().orc_poisson_cg(self._h, float(sigma), _p(r), _p(phi), _p(E), float(tol), int(maxiter), _p(info))
+        return E.reshape((self.dx,) + self.xshape), phi.reshape(self.xshape), it, float(info[0])

@@ -467,3 +467,180 @@ double orc_electric_energy(const orc_ctx *c, const double *E)
     }
     return (double)(0.5L * acc);
 }
+
+/* ================================================================== NEXT row
+ * CGdG Poisson solver: SIPG discretisation + mean-preserving CG   (Appendix, Algorithm 1)
+ *
+ * Readings (I / T / U / V):
+ *  I  M, B of P:525-527 are garbled; taken from eq. (4) with [v] = v^- - v^+, {v} = (v^- + v^+)/2,
+ *     reference basis on [0,1], weights summing to 1, everything times 1/h:
+ *       M_ab = sum_l w_l phi_a'(xi_l) phi_b'(xi_l)
+ *              + 1/2 phi_b'(0) phi_a(0) + 1/2 phi_b(0) phi_a'(0) + sigma phi_b(0) phi_a(0)
+ *              - 1/2 phi_b'(1) phi_a(1) - 1/2 phi_b(1) phi_a'(1) + sigma phi_b(1) phi_a(1)
+ *       B_ab = -1/2 phi_a'(0) phi_b(1) + 1/2 phi_a(0) phi_b'(1) - sigma phi_a(0) phi_b(1)
+ *     (A_hat u)_i = M u_i + B u_{i-1} + B^T u_{i+1}, periodic;  A_x = A_hat / h_x.
+ *  T  sigma "set to its minimum allowed value", sigma >= k^2: k^2 for k >= 2; for k = 1 the
+ *     value k^2 = 1 leaves a second null vector and first-order convergence, so 2 is used; k = 0 is rejected.
+ *  U  E = -grad phi is the cell-wise derivative of phi^DG at the Gauss-Legendre nodes (paper silent).
+ *  V  mean(.) in Algorithm 1 is the arithmetic mean of the coefficient vector (the null vector of A is the
+ *     constant coefficient vector); the loop is entered only if ||r_0|| >= tol ||b|| and r_0 != 0.
+ * Pins: tests/test_oracle_cgdg.py. */
+
+/* d/dz of the Lagrange basis l_l at z */
+double orc_lagrange_deriv(int n, const double *xi, int l, double z)
+{
+    long double s = 0.0L;
+    for (int m = 0; m < n; m++) {
+        if (m == l) continue;
+        long double p = 1.0L / ((long double)xi[l] - (long double)xi[m]);
+        for (int q = 0; q < n; q++)
+            if (q != l && q != m) p *= ((long double)z - (long double)xi[q]) / ((long double)xi[l] - (long double)xi[q]);
+        s += p;
+    }
+    return (double)s;
+}
+
+double orc_sipg_sigma_default(int k) { return k >= 2 ? (double)(k * k) : 2.0; }
+
+/* M, B of reading I, row-major (k+1)x(k+1) */
+void orc_sipg_MB(int k, double sigma, double *M, double *B)
+{
+    int n = k + 1;
+    double xi[ORC_MAXK + 1], w[ORC_MAXK + 1];
+    orc_gauss_legendre(n, xi, w);
+    for (int a = 0; a < n; a++)
+        for (int b = 0; b < n; b++) {
+            double vol = 0.0;
+            for (int l = 0; l < n; l++)
+                vol += w[l] * orc_lagrange_deriv(n, xi, a, xi[l]) * orc_lagrange_deriv(n, xi, b, xi[l]);
+            double pa0 = orc_lagrange(n, xi, a, 0.0), pa1 = orc_lagrange(n, xi, a, 1.0);
+            double pb0 = orc_lagrange(n, xi, b, 0.0), pb1 = orc_lagrange(n, xi, b, 1.0);
+            double da0 = orc_lagrange_deriv(n, xi, a, 0.0), da1 = orc_lagrange_deriv(n, xi, a, 1.0);
+            double db0 = orc_lagrange_deriv(n, xi, b, 0.0), db1 = orc_lagrange_deriv(n, xi, b, 1.0);
+            M[a * n + b] = vol + 0.5 * db0 * pa0 + 0.5 * pb0 * da0 + sigma * pb0 * pa0
+                               - 0.5 * db1 * pa1 - 0.5 * pb1 * da1 + sigma * pb1 * pa1;
+            B[a * n + b] = -0.5 * da0 * pb1 + 0.5 * pa0 * db1 - sigma * pa0 * pb1;
+        }
+}
+
+/* out = A u on the x grid [X]:  A = sum_d (prod_{e != d} h_e W_e) (x) A_hat_d / h_d */
+void orc_sipg_apply(const orc_ctx *c, double sigma, const double *u, double *out)
+{
+    int n = c->k + 1;
+    double M[(ORC_MAXK + 1) * (ORC_MAXK + 1)], B[(ORC_MAXK + 1) * (ORC_MAXK + 1)];
+    orc_sipg_MB(c->k, sigma, M, B);
+    for (long x = 0; x < c->X; x++) out[x] = 0.0;
+    for (int d = 0; d < c->dx; d++) {
+        long inner = 1;
+        for (int b = 0; b < d; b++) inner *= c->D[b];
+        long N = c->cells[d];
+        for (long x = 0; x < c->X; x++) {
+            /* node indices of x on every axis; weight of the other axes */
+            long rem = x, nd = 0;
+            double wo = 1.0;
+            for (int e = 0; e < c->dx; e++) {
+                long ne = rem % c->D[e];
+                rem /= c->D[e];
+                if (e == d) nd = ne;
+                else wo *= c->h[e] * c->w[ne % n];
+            }
+            long i = nd / n, a = nd % n;
+            long base = x - nd * inner;                       /* node 0 of this line */
+            long im = pmod(i - 1, N), ip = pmod(i + 1, N);
+            double acc = 0.0;
+            for (int b = 0; b < n; b++) acc += M[a * n + b] * u[base + (i * n + b) * inner];
+            for (int b = 0; b < n; b++) acc += B[a * n + b] * u[base + (im * n + b) * inner];
+            for (int b = 0; b < n; b++) acc += B[b * n + a] * u[base + (ip * n + b) * inner];
+            out[x] += wo * (acc / c->h[d]);
+        }
+    }
+}
+
+/* E_d = -(1/h_d) d/dxi phi^DG at the x DG nodes (reading U); E is [dx][X] */
+void orc_grad_phi(const orc_ctx *c, const double *phi, double *E)
+{
+    int n = c->k + 1;
+    double Dm[(ORC_MAXK + 1) * (ORC_MAXK + 1)];               /* Dm[a][b] = phi_b'(xi_a) */
+    for (int a = 0; a < n; a++)
+        for (int b = 0; b < n; b++) Dm[a * n + b] = orc_lagrange_deriv(n, c->xi, b, c->xi[a]);
+    for (int d = 0; d < c->dx; d++) {
+        long inner = 1;
+        for (int b = 0; b < d; b++) inner *= c->D[b];
+        for (long x = 0; x < c->X; x++) {
+            long nd = (x / inner) % c->D[d];
+            long i = nd / n, a = nd % n;
+            long base = x - nd * inner;
+            double acc = 0.0;
+            for (int b = 0; b < n; b++) acc += Dm[a * n + b] * phi[base + (i * n + b) * inner];
+            E[d * c->X + x] = -(acc / c->h[d]);
+        }
+    }
+}
+
+static double vec_mean(const double *v, long n)
+{
+    long double s = 0.0L;
+    for (long i = 0; i < n; i++) s += v[i];
+    return (double)(s / (long double)n);
+}
+static double vec_dot(const double *a, const double *b, long n)
+{
+    long double s = 0.0L;
+    for (long i = 0; i < n; i++) s += (long double)a[i] * (long double)b[i];
+    return (double)s;
+}
+
+/* b = W_x (1 - rho): right-hand side of eq. (4) with the diagonal Gauss-Legendre mass matrix */
+void orc_sipg_rhs(const orc_ctx *c, const double *rho, double *b)
+{
+    int n = c->k + 1;
+    for (long x = 0; x < c->X; x++) {
+        long rem = x;
+        double wx = 1.0;
+        for (int e = 0; e < c->dx; e++) { wx *= c->h[e] * c->w[(rem % c->D[e]) % n]; rem /= c->D[e]; }
+        b[x] = wx * (1.0 - rho[x]);
+    }
+}
+
+/* Algorithm 1, mean-preserving CG, step by step in the paper's order and notation.
+ * phi: in = starting vector u_0 (its mean is removed first), out = solution.  E = -grad phi (reading U).
+ * info[0] = ||r||_2 / ||b||_2 at exit, info[1] = eta.  Returns the number of iterations performed. */
+int orc_poisson_cg(const orc_ctx *c, double sigma, const double *rho, double *phi, double *E, double tol,
+                   int maxiter, double *info)
+{
+    long X = c->X;
+    double *b = malloc(sizeof(double) * X), *r = malloc(sizeof(double) * X);
+    double *p = malloc(sizeof(double) * X), *w = malloc(sizeof(double) * X);
+    double *u = phi;
+    orc_sipg_rhs(c, rho, b);
+    double m = vec_mean(u, X);                                 /* mean(u_0) = 0 */
+    for (long x = 0; x < X; x++) u[x] -= m;
+    orc_sipg_apply(c, sigma, u, w);
+    for (long x = 0; x < X; x++) r[x] = b[x] - w[x];           /* r_0 = b - A u_0 */
+    m = vec_mean(r, X);
+    for (long x = 0; x < X; x++) { r[x] -= m; p[x] = r[x]; }   /* r_0 = r_0 - mean(r_0), p_0 = r_0 */
+    double eta = 0.0;
+    for (long x = 0; x < X; x++) eta += (b[x] + r[x]) * u[x];  /* eta = (b + r_0)^T u_0 */
+    double bb = vec_dot(b, b, X), rr = vec_dot(r, r, X);
+    int it = 0;
+    if (rr > 0.0 && !(sqrt(rr) < tol * sqrt(bb))) {            /* reading V */
+        while (it < maxiter) {
+            orc_sipg_apply(c, sigma, p, w);                    /* [w_i, mean_w] = A p_i */
+            double mw = vec_mean(w, X);
+            double alpha = rr / vec_dot(p, w, X);              /* alpha_i = r_i^T r_i / p_i^T w_i */
+            for (long x = 0; x < X; x++) u[x] += alpha * p[x];
+            for (long x = 0; x < X; x++) r[x] -= alpha * (w[x] - mw);
+            eta += alpha * rr;
+            double rr1 = vec_dot(r, r, X);
+            it++;
+            if (sqrt(rr1) < tol * sqrt(bb)) { rr = rr1; break; }
+            double beta = rr1 / rr;                            /* beta_i = r_{i+1}^T r_{i+1} / r_i^T r_i */
+            for (long x = 0; x < X; x++) p[x] = r[x] + beta * p[x];
+            rr = rr1;
+        }
+    }
+    if (info) { info[0] = bb > 0.0 ? sqrt(rr / bb) : 0.0; info[1] = eta; }
+    orc_grad_phi(c, u, E);
+    free(b); free(r); free(p); free(w);
+    return it;
+}
