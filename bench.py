@@ -202,6 +202,8 @@ def run_ours(args, cfg, rank, world, local):
     coords = [g.node_coords(a) for a in range(g.d)]
     f = g.empty_field()
     W.initial_data(cfg, coords, device=dev, out=f)
+    if args.poisson == "cg":
+        g.set_poisson_solver(1, tol=1e-3)
     dt = cfg["dt"]
     nf = W.field_elems(cfg)
     nsweeps = sweeps_per_step(cfg)
@@ -257,7 +259,7 @@ def run_ours(args, cfg, rank, world, local):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": cfg["name"], "values": nf, "bytes_f": nf * 8, "sweeps_per_step": nsweeps,
-                   "dt": dt, "l2": "inputs larger than L2 (no flush needed)" if nf * 8 > 2 * 126e6 else
+                   "dt": dt, "poisson": args.poisson, "l2": "inputs larger than L2 (no flush needed)" if nf * 8 > 2 * 126e6 else
                    "array fits in L2: numbers are L2-resident, launch-bound",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "pct_of_measured_peak": 100 * value / world / peak, "pct_of_nominal_8TBs": 100 * value / world / NOMINAL_HBM_GBS,
@@ -301,6 +303,8 @@ def main():
     ap.add_argument("--workload", type=str, default=None, help="a workload by name, incl. the NEXT-row cases "
                     "(bot_5d_k3_16, bot_6d_k3_9: the paper's bump-on-tail case, 4th order)")
     ap.add_argument("--cfl", type=float, default=None, help="choose dt so that the largest x shift is CFL cells (PAPER.md:351)")
+    ap.add_argument("--poisson", default="fft", choices=["fft", "cg"], help="field solver inside the step: the FFT "
+                    "route (default) or the CGdG solver with the paper's tolerance 1e-3 and warm start (PAPER.md:496-567)")
     ap.add_argument("--cells", type=str, default=None, help="override cells, e.g. 16,16,16,16 (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -94,6 +94,31 @@ int sldg_poisson(sldg_ctx* ctx, const double* rho, double* E);
  * advect_x(dt/2).  rho and E of the step stay in the workspace (sldg_last_rho / sldg_last_E). */
 int sldg_step(sldg_ctx* ctx, double* f, double dt);
 
+/* ---- CGdG Poisson solver (NEXT row, Appendix) --------------------------------
+ * Alternative to sldg_poisson: symmetric interior penalty (SIPG) dG discretisation of
+ * -Laplace phi = 1 - rho in the advection's own polynomial space (eq. (4); block-tridiagonal
+ * matrix from the small matrices M, B; tensor form P:541-545; readings I, T), solved
+ * matrix-free by the mean-preserving conjugate gradient method of Algorithm 1 starting
+ * from the potential of the previous solve, then E = -grad phi cell-wise at the nodes
+ * (reading U).  Stops when ||r||_2 < tol ||b||_2 (the paper uses tol 1e-3) or after maxiter
+ * iterations (0 = the paper's bound (prod_l N_l (k+1))^(1/dim_x) times a safety factor).
+ * One cooperative launch, no host synchronisation.  degree >= 1 (SLDG_EINVAL for degree 0).
+ * rho [X], E [dim_x][X] device. */
+int sldg_poisson_cg(sldg_ctx* ctx, const double* rho, double* E, double tol, int maxiter);
+/* Which solver sldg_step uses: 0 = sldg_poisson (default), 1 = sldg_poisson_cg with these
+ * parameters; sigma <= 0 selects the default penalty (k^2, 2 for k = 1; reading T). */
+int sldg_set_poisson_solver(sldg_ctx* ctx, int solver, double tol, int maxiter, double sigma);
+/* Zero the stored potential (cold start of the next CG solve). */
+int sldg_cg_reset(sldg_ctx* ctx);
+/* Iterations and relative residual ||r||_2/||b||_2 of the last CG solve (host outputs, may be NULL).
+ * Synchronises. */
+int sldg_cg_info(sldg_ctx* ctx, int* iters_host, double* relres_host);
+/* device pointer [X] to the potential of the last CG solve (mean 0), valid until the workspace changes */
+const double* sldg_last_phi(const sldg_ctx* ctx);
+/* M, B of the SIPG matrix as the library builds them, row-major (k+1)x(k+1), (A_hat u)_i = M u_i +
+ * B u_{i-1} + B^T u_{i+1}; sigma <= 0: default.  Host-only, needs no context or device. */
+int sldg_sipg_matrices(int degree, double sigma, double* hostM, double* hostB);
+
 /* Same path driven from HOST memory: copies f_host (|f| doubles, pinned memory recommended) to
  * the device buffer f_dev, runs nsteps Strang steps, copies the result back into f_host and the
  * last E ([dim_x][X]) into E_host if it is not NULL.  Synchronises. */

@@ -47,6 +47,12 @@ EXPORTS = {
     "sldg_launch_count": (_ll, [_vp]),
     "sldg_timing_axis": (C.c_int, [_vp, _llp, _dp]),
     "sldg_set_option": (C.c_int, [_vp, C.c_char_p, _ll]),
+    "sldg_poisson_cg": (C.c_int, [_vp, _vp, _vp, C.c_double, C.c_int]),
+    "sldg_set_poisson_solver": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, C.c_double]),
+    "sldg_cg_reset": (C.c_int, [_vp]),
+    "sldg_cg_info": (C.c_int, [_vp, _ip, _dp]),
+    "sldg_last_phi": (_vp, [_vp]),
+    "sldg_sipg_matrices": (C.c_int, [C.c_int, C.c_double, _dp, _dp]),
 }
 
 _lib = None
@@ -99,6 +105,13 @@ def AB(degree, alpha, device_arith=False):
     _check(lib().sldg_AB(int(degree), float(alpha), 1 if device_arith else 0,
                          A.ctypes.data_as(_dp), B.ctypes.data_as(_dp)))
     return A, B
+
+
+def sipg_matrices(degree, sigma=0.0):
+    import numpy as np
+    M, B = np.empty((degree + 1, degree + 1)), np.empty((degree + 1, degree + 1))
+    _check(lib().sldg_sipg_matrices(int(degree), float(sigma), M.ctypes.data_as(_dp), B.ctypes.data_as(_dp)))
+    return M, B
 
 
 def gauss_legendre(degree):
@@ -187,6 +200,27 @@ class Sldg:
             E = torch.empty((self.dx,) + self.xshape, dtype=torch.float64, device=self.device)
         _check(lib().sldg_poisson(self._h, _ptr(rho), _ptr(E)), self._h)
         return E
+
+    def poisson_cg(self, rho, E=None, tol=1e-3, maxiter=0):
+        import torch
+        if E is None:
+            E = torch.empty((self.dx,) + self.xshape, dtype=torch.float64, device=self.device)
+        _check(lib().sldg_poisson_cg(self._h, _ptr(rho), _ptr(E), float(tol), int(maxiter)), self._h)
+        return E
+
+    def set_poisson_solver(self, solver, tol=1e-3, maxiter=0, sigma=0.0):
+        _check(lib().sldg_set_poisson_solver(self._h, int(solver), float(tol), int(maxiter), float(sigma)), self._h)
+
+    def cg_reset(self):
+        _check(lib().sldg_cg_reset(self._h), self._h)
+
+    def cg_info(self):
+        it, rel = C.c_int(), C.c_double()
+        _check(lib().sldg_cg_info(self._h, C.byref(it), C.byref(rel)), self._h)
+        return it.value, rel.value
+
+    def last_phi(self):
+        return self._view(lib().sldg_last_phi(self._h), self.xshape)
 
     def step(self, f, dt):
         _check(lib().sldg_step(self._h, _ptr(f), float(dt)), self._h)

@@ -36,7 +36,7 @@ void sldg_ev_end(sldg_ctx* c)
 }
 
 // ------------------------------------------------------------------ layout of the workspace
-struct WsLayout { size_t f2, vS, vAB, Wv, rho, E, part, cplx[6], red, total; long long part_cap; };
+struct WsLayout { size_t f2, vS, vAB, Wv, rho, E, part, cplx[6], red, phi, cg_info, total; long long part_cap; };
 
 static WsLayout ws_layout(const sldg_ctx* c)
 {
@@ -60,6 +60,8 @@ static WsLayout ws_layout(const sldg_ctx* c)
     L.part = take((size_t)L.part_cap * 8);
     for (int i = 0; i < 6; i++) L.cplx[i] = take(X * 8);
     L.red = take(4096 * 8);
+    L.phi = take(X * 8);
+    L.cg_info = take(4 * 8);
     L.total = off;
     return L;
 }
@@ -92,6 +94,8 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
     c->stream = 0; c->last_cuda = 0; c->sm_count = 148;
     c->ws = nullptr; c->ws_bytes = 0; c->ws_ready = false;
     c->timing = false; c->launches = 0;
+    c->phi = nullptr; c->cg_info = nullptr; c->poisson_solver = 0; c->cg_tol = 1e-3; c->cg_sigma = sldg_sipg_sigma_default(degree);
+    c->cg_maxiter = 0;
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
@@ -205,6 +209,9 @@ extern "C" int sldg_set_workspace(sldg_ctx* c, void* dev, size_t bytes)
     c->part = (double*)(b + L.part); c->part_cap = L.part_cap;
     for (int i = 0; i < 6; i++) c->cplx[i] = (double*)(b + L.cplx[i]);
     c->red = (double*)(b + L.red);
+    c->phi = (double*)(b + L.phi); c->cg_info = (double*)(b + L.cg_info);
+    if (cudaMemsetAsync(c->phi, 0, (size_t)c->X * 8 + 0, c->stream) != cudaSuccess ||
+        cudaMemsetAsync(c->cg_info, 0, 32, c->stream) != cudaSuccess) { c->ws_ready = false; return SLDG_ECUDA; }
     sldg_ev_begin(c, KIND_TABLE, -1);
     cudaError_t e = sldg_launch_wv(c);
     sldg_ev_end(c);
@@ -518,6 +525,67 @@ extern "C" int sldg_poisson(sldg_ctx* c, const double* rho, double* E)
     return SLDG_OK;
 }
 
+// ---- CGdG Poisson solver
+static int cg_default_maxiter(const sldg_ctx* c)
+{
+    // convergence within about (prod_l N_l (k+1))^(1/dx) iterations, times a safety factor (4, + 20)
+    return 4 * (int)llround(pow((double)c->X, 1.0 / c->dx)) + 20;
+}
+
+extern "C" int sldg_poisson_cg(sldg_ctx* c, const double* rho, double* E, double tol, int maxiter)
+{
+    if (!c || !rho || !E || !(tol >= 0.0) || maxiter < 0) return SLDG_EINVAL;
+    if (c->k < 1) return SLDG_EINVAL;                       // sigma >= k^2 = 0 gives no penalty: not defined for k = 0
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    if (maxiter == 0) maxiter = c->cg_maxiter > 0 ? c->cg_maxiter : cg_default_maxiter(c);
+    sldg_ev_begin(c, KIND_POISSON, -1);
+    cudaError_t e = sldg_launch_poisson_cg(c, rho, E, tol, maxiter, c->cg_sigma);
+    sldg_ev_end(c);
+    c->launches++;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    return SLDG_OK;
+}
+
+extern "C" int sldg_set_poisson_solver(sldg_ctx* c, int solver, double tol, int maxiter, double sigma)
+{
+    if (!c || solver < 0 || solver > 1 || !(tol >= 0.0) || maxiter < 0) return SLDG_EINVAL;
+    if (solver == 1 && c->k < 1) return SLDG_EINVAL;
+    c->poisson_solver = solver; c->cg_tol = tol; c->cg_maxiter = maxiter;
+    c->cg_sigma = sigma > 0.0 ? sigma : sldg_sipg_sigma_default(c->k);
+    return SLDG_OK;
+}
+
+extern "C" int sldg_cg_reset(sldg_ctx* c)
+{
+    if (!c) return SLDG_EINVAL;
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    CK(cudaMemsetAsync(c->phi, 0, (size_t)c->X * 8, c->stream));
+    return SLDG_OK;
+}
+
+extern "C" int sldg_cg_info(sldg_ctx* c, int* iters_host, double* relres_host)
+{
+    if (!c) return SLDG_EINVAL;
+    if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    double h[2];
+    CK(cudaMemcpyAsync(h, c->cg_info, 16, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (iters_host) *iters_host = (int)h[0];
+    if (relres_host) *relres_host = h[1];
+    return SLDG_OK;
+}
+
+extern "C" const double* sldg_last_phi(const sldg_ctx* c) { return (c && c->ws_ready) ? c->phi : nullptr; }
+
+extern "C" int sldg_sipg_matrices(int degree, double sigma, double* hostM, double* hostB)
+{
+    if (degree < 1 || degree > SLDG_MAX_DEGREE || !hostM || !hostB) return SLDG_EINVAL;
+    double xi[SLDG_MAXK1], w[SLDG_MAXK1], Dm[SLDG_MAXNN];
+    sldg_gl_rule(degree + 1, xi, w);
+    sldg_sipg_tables(degree, xi, w, sigma > 0.0 ? sigma : sldg_sipg_sigma_default(degree), hostM, hostB, Dm);
+    return SLDG_OK;
+}
+
 extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
 {
     int r = check_f(c, f);
@@ -535,7 +603,7 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
     }
     if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, p1 != 0))) return r;
     if ((r = sldg_density(c, cur, c->rho))) return r;
-    if ((r = sldg_poisson(c, c->rho, c->E))) return r;
+    if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
     if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;
     if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f))) return r;       // ... ends in f
     if (cur != f) return copy_back(c, f, cur);                                  // unreachable by construction

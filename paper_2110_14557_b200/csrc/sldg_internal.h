@@ -103,6 +103,10 @@ struct sldg_ctx {
     double* part; long long part_cap;   // rho partial sums
     double* cplx[6];                // complex scratch, X doubles each
     double* red;                    // reduction partials [4096]
+    double* phi;                    // [X] potential of the CGdG solver (warm start of the next solve)
+    double* cg_info;                // [4] iterations, relative residual of the last CGdG solve
+    int poisson_solver;             // 0 = FFT route (reading P1), 1 = CGdG
+    double cg_tol, cg_sigma; int cg_maxiter;
     bool ws_ready;
 
     // instrumentation
@@ -155,6 +159,9 @@ cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double
 cudaError_t sldg_launch_wv(sldg_ctx* c);
 cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho);
 cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E);
+cudaError_t sldg_launch_poisson_cg(sldg_ctx* c, const double* rho, double* E, double tol, int maxiter, double sigma);
+double sldg_sipg_sigma_default(int k);
+void sldg_sipg_tables(int k, const double* xi, const double* w, double sigma, double* M, double* B, double* Dm);
 cudaError_t sldg_launch_energy(sldg_ctx* c, const double* E, double* out1);
 cudaError_t sldg_launch_mass(sldg_ctx* c, const double* f, double* out1);
 

@@ -94,3 +94,16 @@ def test_argument_validation():
     assert L.sldg_AB(1, float("nan"), 0, a, a) == -1
     assert L.sldg_AB(1, 0.5, 0, None, a) == -1
     assert L.sldg_gauss_legendre(-1, a, a) == -1
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4])
+def test_sipg_matrices_host(k):
+    """M, B of the CGdG solver (reading I) as the library builds them on the host: against the
+    independently written oracle, and the properties eq. (4) fixes -- M symmetric, rows of M + B + B^T sum to 0
+    (constants are in the null space)."""
+    M, B = P.sipg_matrices(k)
+    Mo, Bo = O.sipg_MB(k, O.sipg_sigma_default(k))
+    assert np.abs(M - Mo).max() < 1e-12 * np.abs(Mo).max() and np.abs(B - Bo).max() < 1e-12 * np.abs(Mo).max()
+    assert np.abs(M - M.T).max() < 1e-13 * np.abs(M).max()
+    assert np.abs((M + B + B.T).sum(axis=1)).max() < 1e-12 * np.abs(M).max()
+    assert P.lib().sldg_sipg_matrices(0, 1.0, M.ctypes.data_as(P.binding._dp), B.ctypes.data_as(P.binding._dp)) == -1
