@@ -49,9 +49,12 @@ template <> struct Vec<2> {
 #ifndef SLDG_WALK_U3
 #define SLDG_WALK_U3 4
 #endif
+#ifndef SLDG_WALK_U4
+#define SLDG_WALK_U4 4
+#endif
 // cells loaded ahead of the one being computed (loads in flight per thread = U * K1 * VEC values)
 template <int K1> struct Unroll {
-    static constexpr int U = (K1 == 1) ? SLDG_WALK_U1 : (K1 == 2) ? SLDG_WALK_U2 : (K1 == 3) ? SLDG_WALK_U3 : 2;
+    static constexpr int U = (K1 == 1) ? SLDG_WALK_U1 : (K1 == 2) ? SLDG_WALK_U2 : (K1 == 3) ? SLDG_WALK_U3 : (K1 == 4) ? SLDG_WALK_U4 : 2;
 };
 
 // MODE 0: one shift per thread (x-sweep, shift indexed by a digit of the outer index)
