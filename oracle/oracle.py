@@ -20,6 +20,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(_build.build())
         dp, ip, vp, lg = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p, C.c_long
+        fp = C.POINTER(C.c_float)
         sig = {
             "orc_gauss_legendre": (None, [C.c_int, dp, dp]),
             "orc_lagrange": (C.c_double, [C.c_int, dp, C.c_int, C.c_double]),
@@ -40,6 +41,12 @@ def lib():
             "orc_step": (None, [vp, dp, dp, dp, dp, C.c_double]),
             "orc_mass": (C.c_double, [vp, dp]),
             "orc_electric_energy": (C.c_double, [vp, dp]),
+            "orc_sweep_axis_f32": (None, [vp, fp, fp, C.c_int, dp, C.c_int, C.c_int]),
+            "orc_advect_x_f32": (None, [vp, fp, fp, C.c_double]),
+            "orc_advect_v_f32": (None, [vp, fp, fp, dp, C.c_double]),
+            "orc_density_f32": (None, [vp, fp, dp]),
+            "orc_step_f32": (None, [vp, fp, fp, dp, dp, C.c_double]),
+            "orc_mass_f32": (C.c_double, [vp, fp]),
             "orc_lagrange_deriv": (C.c_double, [C.c_int, dp, C.c_int, C.c_double]),
             "orc_sipg_sigma_default": (C.c_double, [C.c_int]),
             "orc_sipg_MB": (None, [C.c_int, C.c_double, dp, dp]),
@@ -57,6 +64,11 @@ def lib():
 def _p(a):
     assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _pf(a):
+    assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(C.POINTER(C.c_float))
 
 
 def gauss_legendre(n):
@@ -220,3 +232,46 @@ class Oracle:
         E, info = np.empty(self.dx * self.X), np.empty(2)
         it = lib().orc_poisson_cg(self._h, float(sigma), _p(r), _p(phi), _p(E), float(tol), int(maxiter), _p(info))
         return E.reshape((self.dx,) + self.xshape), phi.reshape(self.xshape), it, float(info[0])
+
+    # ---- single precision mode (reading W): float32 storage and sweep arithmetic, fp64 field solve
+    def sweep_axis_f32(self, f, axis, delta, mode=None, saxis=None):
+        if mode is None:
+            mode = 0 if axis < self.dx else 1
+        if saxis is None:
+            saxis = self.dx + axis if mode == 0 else -1
+        delta = np.ascontiguousarray(delta, dtype=np.float64)
+        assert delta.size == (self.D[saxis] if mode == 0 else self.X)
+        fin = np.ascontiguousarray(f, dtype=np.float32).reshape(-1)
+        out = np.empty_like(fin)
+        lib().orc_sweep_axis_f32(self._h, _pf(fin), _pf(out), axis, _p(delta), mode, saxis)
+        return out.reshape(self.shape)
+
+    def advect_x_f32(self, f, tau):
+        g = np.array(f, dtype=np.float32, order="C").reshape(-1)
+        tmp = np.empty_like(g)
+        lib().orc_advect_x_f32(self._h, _pf(g), _pf(tmp), float(tau))
+        return g.reshape(self.shape)
+
+    def advect_v_f32(self, f, E, tau):
+        g = np.array(f, dtype=np.float32, order="C").reshape(-1)
+        tmp = np.empty_like(g)
+        E = np.ascontiguousarray(E, dtype=np.float64).reshape(-1)
+        assert E.size == self.dx * self.X
+        lib().orc_advect_v_f32(self._h, _pf(g), _pf(tmp), _p(E), float(tau))
+        return g.reshape(self.shape)
+
+    def density_f32(self, f):
+        fin = np.ascontiguousarray(f, dtype=np.float32).reshape(-1)
+        rho = np.empty(self.X)
+        lib().orc_density_f32(self._h, _pf(fin), _p(rho))
+        return rho.reshape(self.xshape)
+
+    def step_f32(self, f, dt):
+        g = np.array(f, dtype=np.float32, order="C").reshape(-1)
+        tmp = np.empty_like(g)
+        rho, E = np.empty(self.X), np.empty(self.dx * self.X)
+        lib().orc_step_f32(self._h, _pf(g), _pf(tmp), _p(rho), _p(E), float(dt))
+        return g.reshape(self.shape), rho.reshape(self.xshape), E.reshape((self.dx,) + self.xshape)
+
+    def mass_f32(self, f):
+        return lib().orc_mass_f32(self._h, _pf(np.ascontiguousarray(f, dtype=np.float32).reshape(-1)))

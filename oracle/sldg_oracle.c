@@ -644,3 +644,135 @@ int orc_poisson_cg(const orc_ctx *c, double sigma, const double *rho, double *ph
     free(b); free(r); free(p); free(w);
     return it;
 }
+
+/* ================================================================== NEXT row
+ * Single precision mode ("running simulations ... in single precision is a viable option. This reduces
+ * memory consumption by a factor of two"; Tables 3-4 report fp32 throughout).
+ *
+ * Reading W: f is STORED in fp32 and the sweep arithmetic of eq. (3) runs in fp32
+ * (coefficients A, B rounded to fp32, every product and sum rounded to fp32); everything that is O(X) stays
+ * fp64: the shift delta, s = floor(delta), alpha and A(alpha), B(alpha) before rounding, rho (fp64 sum of the
+ * fp32 values), the field solve and E.  So integer decisions are taken in fp64 exactly as in the fp64 path.
+ * Same functions as above with float storage; no other change of order. */
+
+static void sweep_line_AB_f32(int k, int N, long s, double alpha, const float *A, const float *B,
+                              const float *uin, float *uout, long stride)
+{
+    int n = k + 1;
+    for (long i = 0; i < N; i++) {
+        long ia = pmod(i - s, N);
+        long ib = pmod(i - s - 1, N);
+        for (int j = 0; j < n; j++) {
+            if (alpha == 0.0) {
+                uout[(i * n + j) * stride] = uin[(ia * n + j) * stride];
+            } else {
+                float acc = 0.0f;
+                for (int l = 0; l < n; l++) acc += A[j * n + l] * uin[(ia * n + l) * stride];
+                for (int l = 0; l < n; l++) acc += B[j * n + l] * uin[(ib * n + l) * stride];
+                uout[(i * n + j) * stride] = acc;
+            }
+        }
+    }
+}
+
+void orc_sweep_axis_f32(const orc_ctx *c, const float *fin, float *fout, int axis,
+                        const double *delta, int mode, int saxis)
+{
+    long inner = 1, outer = 1, Da = c->D[axis];
+    for (int a = 0; a < axis; a++) inner *= c->D[a];
+    for (int a = axis + 1; a < c->d; a++) outer *= c->D[a];
+    long sdiv = 1;
+    if (mode == 0) for (int a = axis + 1; a < saxis; a++) sdiv *= c->D[a];
+    long lines = inner * outer;
+    long nidx = (mode == 0) ? c->D[saxis] : c->X;
+    int nn = (c->k + 1) * (c->k + 1);
+    long *S = (long *)malloc(sizeof(long) * nidx);
+    double *AL = (double *)malloc(sizeof(double) * nidx);
+    float *AB = (float *)malloc(sizeof(float) * nidx * 2 * nn);
+    double A64[(ORC_MAXK + 1) * (ORC_MAXK + 1)], B64[(ORC_MAXK + 1) * (ORC_MAXK + 1)];
+    for (long i = 0; i < nidx; i++) {
+        split_delta(delta[i], c->cells[axis], &S[i], &AL[i]);              /* fp64 decision */
+        if (AL[i] != 0.0) {
+            orc_AB(c->k, AL[i], A64, B64);
+            for (int m = 0; m < nn; m++) { AB[i * 2 * nn + m] = (float)A64[m]; AB[i * 2 * nn + nn + m] = (float)B64[m]; }
+        }
+    }
+#pragma omp parallel for schedule(static) num_threads(c->threads)
+    for (long t = 0; t < lines; t++) {
+        long p = t % inner, q = t / inner;
+        long idx = (mode == 0) ? (q / sdiv) % c->D[saxis] : p % c->X;
+        long base = q * Da * inner + p;
+        sweep_line_AB_f32(c->k, c->cells[axis], S[idx], AL[idx], AB + idx * 2 * nn, AB + idx * 2 * nn + nn,
+                          fin + base, fout + base, inner);
+    }
+    free(S); free(AL); free(AB);
+}
+
+void orc_advect_x_f32(const orc_ctx *c, float *f, float *tmp, double tau)
+{
+    for (int d = 0; d < c->dx; d++) {
+        int b = c->dx + d;
+        double *delta = (double *)malloc(sizeof(double) * c->D[b]);
+        for (long n = 0; n < c->D[b]; n++) delta[n] = (node_coord(c, b, n) * tau) / c->h[d];
+        orc_sweep_axis_f32(c, f, tmp, d, delta, 0, b);
+        memcpy(f, tmp, sizeof(float) * c->nf);
+        free(delta);
+    }
+}
+
+void orc_advect_v_f32(const orc_ctx *c, float *f, float *tmp, const double *E, double tau)
+{
+    for (int d = 0; d < c->dx; d++) {
+        int a = c->dx + d;
+        double *delta = (double *)malloc(sizeof(double) * c->X);
+        for (long n = 0; n < c->X; n++) delta[n] = ((-E[d * c->X + n]) * tau) / c->h[a];
+        orc_sweep_axis_f32(c, f, tmp, a, delta, 1, -1);
+        memcpy(f, tmp, sizeof(float) * c->nf);
+        free(delta);
+    }
+}
+
+/* rho in fp64 from the fp32 values (reading W) */
+void orc_density_f32(const orc_ctx *c, const float *f, double *rho)
+{
+    long X = c->X, V = c->V;
+    double *W = (double *)malloc(sizeof(double) * V);
+    for (long v = 0; v < V; v++) {
+        long r = v; double wv = 1.0;
+        for (int a = c->dx; a < c->d; a++) {
+            long n = r % c->D[a]; r /= c->D[a];
+            wv *= c->h[a] * c->w[n % (c->k + 1)];
+        }
+        W[v] = wv;
+    }
+#pragma omp parallel for schedule(static) num_threads(c->threads)
+    for (long x = 0; x < X; x++) {
+        long double acc = 0.0L;
+        for (long v = 0; v < V; v++) acc += (long double)W[v] * (long double)f[v * X + x];
+        rho[x] = (double)acc;
+    }
+    free(W);
+}
+
+void orc_step_f32(const orc_ctx *c, float *f, float *tmp, double *rho, double *E, double dt)
+{
+    orc_advect_x_f32(c, f, tmp, dt / 2.0);
+    orc_density_f32(c, f, rho);
+    orc_poisson(c, rho, E);
+    orc_advect_v_f32(c, f, tmp, E, dt);
+    orc_advect_x_f32(c, f, tmp, dt / 2.0);
+}
+
+double orc_mass_f32(const orc_ctx *c, const float *f)
+{
+    long double acc = 0.0L;
+    for (long t = 0; t < c->nf; t++) {
+        long r = t; double wn = 1.0;
+        for (int a = 0; a < c->d; a++) {
+            long n = r % c->D[a]; r /= c->D[a];
+            wn *= c->h[a] * c->w[n % (c->k + 1)];
+        }
+        acc += (long double)wn * (long double)f[t];
+    }
+    return (double)acc;
+}
