@@ -60,6 +60,21 @@ int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degr
                 const double* domain);
 int sldg_destroy(sldg_ctx* ctx);
 
+/* ---- single precision mode (NEXT row; Tables 3-4) ---------------------------------
+ * "Running simulations with the semi-Lagrangian discontinuous Galerkin scheme in single precision is
+ * a viable option. This reduces memory consumption by a factor of two".  Reading W: in an
+ * SLDG_F32 context f is STORED as float and the sweep arithmetic of eq. (3) runs in fp32 (A, B
+ * evaluated in fp64, rounded to fp32); the shift delta, s = floor(delta), alpha, rho (fp64 sum of the
+ * fp32 values), the field solve and E stay fp64, so integer decisions are those of the fp64 path.
+ * sldg_create == sldg_create_prec(..., SLDG_F64).  In an SLDG_F32 context every `f` / `f_host` /
+ * `f_dev` argument of the calls below points to |f| FLOAT values (pass the float pointer cast to
+ * double*); rho, E and delta tables stay double.  The workspace holds a float second buffer. */
+#define SLDG_F64 0
+#define SLDG_F32 1
+int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree,
+                     const double* domain, int precision);
+int sldg_precision(const sldg_ctx* ctx);                          /* SLDG_F64 / SLDG_F32 */
+
 /* stream = a cudaStream_t passed as void*; NULL selects the legacy default stream. */
 int sldg_set_stream(sldg_ctx* ctx, void* stream);
 

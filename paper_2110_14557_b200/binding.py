@@ -19,6 +19,8 @@ _llp = C.POINTER(C.c_longlong)
 # name -> (restype, argtypes); every symbol include/sldg.h declares
 EXPORTS = {
     "sldg_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, _ip, C.c_int, _dp]),
+    "sldg_create_prec": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, _ip, C.c_int, _dp, C.c_int]),
+    "sldg_precision": (C.c_int, [_vp]),
     "sldg_destroy": (C.c_int, [_vp]),
     "sldg_set_stream": (C.c_int, [_vp, _vp]),
     "sldg_workspace_bytes": (C.c_size_t, [_vp]),
@@ -125,8 +127,11 @@ def gauss_legendre(degree):
 class Sldg:
     """One solver context: sldg_create(dim_x, dim_v, cells, degree, domain) plus a torch-owned workspace."""
 
-    def __init__(self, dim_x, dim_v, cells, degree, domain, device="cuda:0", stream=None):
+    def __init__(self, dim_x, dim_v, cells, degree, domain, device="cuda:0", stream=None, precision="f64"):
+        """precision "f32": single precision mode (sldg_create_prec, SLDG_F32): f tensors are float32."""
         import torch
+        self.precision = precision
+        self.dtype = {"f64": torch.float64, "f32": torch.float32}[precision]
         self._h = None
         L = lib()
         if not torch.cuda.is_available():
@@ -138,8 +143,8 @@ class Sldg:
         dom = [float(v) for v in domain]
         assert len(self.cells) == self.d and len(dom) == 2 * self.d
         h = _vp()
-        _check(L.sldg_create(C.byref(h), dim_x, dim_v, (C.c_int * self.d)(*self.cells), degree,
-                             (C.c_double * (2 * self.d))(*dom)))
+        _check(L.sldg_create_prec(C.byref(h), dim_x, dim_v, (C.c_int * self.d)(*self.cells), degree,
+                                  (C.c_double * (2 * self.d))(*dom), 1 if precision == "f32" else 0))
         self._h = h
         self.D = [L.sldg_nodes(h, a) for a in range(self.d)]
         self.nf = L.sldg_field_elems(h)
@@ -167,6 +172,12 @@ class Sldg:
             pass
 
     # ---- helpers
+    def _fp(self, t):
+        """pointer of a contiguous f tensor of the context's precision"""
+        import torch
+        assert isinstance(t, torch.Tensor) and t.dtype == self.dtype and t.is_contiguous(), (t.dtype, self.dtype)
+        return C.c_void_p(t.data_ptr())
+
     def node_coords(self, axis):
         import numpy as np
         out = np.empty(self.D[axis])
@@ -175,23 +186,23 @@ class Sldg:
 
     def empty_field(self):
         import torch
-        return torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        return torch.empty(self.shape, dtype=self.dtype, device=self.device)
 
     def AB(self, alpha, device_arith=False):
         return AB(self.k, alpha, device_arith)
 
     # ---- hot path (names as in include/sldg.h)
     def advect_x(self, f, dt):
-        _check(lib().sldg_advect_x(self._h, _ptr(f), float(dt)), self._h)
+        _check(lib().sldg_advect_x(self._h, self._fp(f), float(dt)), self._h)
 
     def advect_v(self, f, E, dt):
-        _check(lib().sldg_advect_v(self._h, _ptr(f), _ptr(E), float(dt)), self._h)
+        _check(lib().sldg_advect_v(self._h, self._fp(f), _ptr(E), float(dt)), self._h)
 
     def density(self, f, rho=None):
         import torch
         if rho is None:
             rho = torch.empty(self.xshape, dtype=torch.float64, device=self.device)
-        _check(lib().sldg_density(self._h, _ptr(f), _ptr(rho)), self._h)
+        _check(lib().sldg_density(self._h, self._fp(f), _ptr(rho)), self._h)
         return rho
 
     def poisson(self, rho, E=None):
@@ -223,10 +234,10 @@ class Sldg:
         return self._view(lib().sldg_last_phi(self._h), self.xshape)
 
     def step(self, f, dt):
-        _check(lib().sldg_step(self._h, _ptr(f), float(dt)), self._h)
+        _check(lib().sldg_step(self._h, self._fp(f), float(dt)), self._h)
 
     def step_host(self, f_host, f_dev, dt, nsteps=1, E_host=None):
-        _check(lib().sldg_step_host(self._h, _ptr(f_host), _ptr(f_dev),
+        _check(lib().sldg_step_host(self._h, self._fp(f_host), self._fp(f_dev),
                                     _ptr(E_host) if E_host is not None else None, float(dt), int(nsteps)), self._h)
 
     def advect_axis(self, f, axis, delta):
@@ -234,7 +245,7 @@ class Sldg:
         d = np.ascontiguousarray(np.asarray(delta, dtype=np.float64))
         want = self.D[self.dx + axis] if axis < self.dx else self.X
         assert d.size == want, (d.size, want)
-        _check(lib().sldg_advect_axis(self._h, _ptr(f), int(axis), d.ctypes.data_as(_dp)), self._h)
+        _check(lib().sldg_advect_axis(self._h, self._fp(f), int(axis), d.ctypes.data_as(_dp)), self._h)
 
     def last_rho(self):
         return self._view(lib().sldg_last_rho(self._h), self.xshape)
@@ -259,7 +270,7 @@ class Sldg:
 
     def mass(self, f):
         out = C.c_double()
-        _check(lib().sldg_mass(self._h, _ptr(f), C.byref(out)), self._h)
+        _check(lib().sldg_mass(self._h, self._fp(f), C.byref(out)), self._h)
         return out.value
 
     # ---- instrumentation

@@ -11,7 +11,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsldg_b200.so")
 SOURCES = ["sldg_api.cu", "sldg_sweep_walk.cu", "sldg_sweep_tma.cu", "sldg_sweep_line.cu", "sldg_sweep_fused.cu", "sldg_sweep_fused_cell.cu", "sldg_field.cu", "sldg_cgdg.cu", "sldg_tables.cpp"]
-HEADERS = [os.path.join(CSRC, "sldg_internal.h"), os.path.join(CSRC, "sldg_async.h"), os.path.join(HERE, "..", "include", "sldg.h")]
+DUAL = ["sldg_sweep_walk.cu", "sldg_sweep_line.cu", "sldg_sweep_fused_cell.cu"]
+HEADERS = [os.path.join(CSRC, "sldg_real.h"), os.path.join(CSRC, "sldg_internal.h"), os.path.join(CSRC, "sldg_async.h"), os.path.join(HERE, "..", "include", "sldg.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC,-ffp-contract=off", "-cudart", "static"]
@@ -34,6 +35,11 @@ def build(force=False, verbose=False):
         if force or _stale(obj, [src] + HEADERS):
             subprocess.check_call([NVCC] + FLAGS + extra + ["-c", src, "-o", obj])
         objs.append(obj)
+        if s in DUAL:          # second compilation: real = float (single precision mode, sldg_real.h)
+            obj32 = os.path.join(CSRC, os.path.splitext(s)[0] + "_f32.o")
+            if force or _stale(obj32, [src] + HEADERS):
+                subprocess.check_call([NVCC] + FLAGS + extra + ["-DSLDG_REAL_FLOAT", "-c", src, "-o", obj32])
+            objs.append(obj32)
     if force or _stale(LIB, objs):
         subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-o", LIB] + objs)
     return LIB

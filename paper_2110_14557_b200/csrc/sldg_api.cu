@@ -44,7 +44,7 @@ static WsLayout ws_layout(const sldg_ctx* c)
     size_t off = 0;
     const size_t X = (size_t)c->X, NN2 = 2 * (size_t)c->K1 * c->K1;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-    L.f2 = take((size_t)c->nf * 8);
+    L.f2 = take((size_t)c->nf * c->esize);
     L.vS = take(X * 4);
     L.vAB = take(X * NN2 * 8);
     L.Wv = take((size_t)c->V * 8);
@@ -69,7 +69,32 @@ static WsLayout ws_layout(const sldg_ctx* c)
 // ------------------------------------------------------------------ lifetime
 extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree, const double* domain)
 {
+    return sldg_create_prec(out, dim_x, dim_v, cells, degree, domain, SLDG_F64);
+}
+
+extern "C" int sldg_precision(const sldg_ctx* c) { return c ? c->prec : SLDG_EINVAL; }
+
+// precision dispatch of the kernels that exist as _f64 and _f32 (sldg_real.h)
+cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g, const ShiftTable& t)
+{
+    return c->prec == SLDG_F32 ? sldg_launch_sweep_walk_f32(c, fin, fout, g, t) : sldg_launch_sweep_walk_f64(c, fin, fout, g, t);
+}
+cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g, const ShiftTable& t)
+{
+    return c->prec == SLDG_F32 ? sldg_launch_sweep_line_f32(c, fin, fout, g, t) : sldg_launch_sweep_line_f64(c, fin, fout, g, t);
+}
+cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
+                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+{
+    return c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell_f32(c, fin, fout, g0, g1, t0, t1)
+                               : sldg_launch_sweep_fused_cell_f64(c, fin, fout, g0, g1, t0, t1);
+}
+
+extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree, const double* domain,
+                                int precision)
+{
     if (!out || !cells || !domain) return SLDG_EINVAL;
+    if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
     if (dim_x < 1 || dim_x > 3 || dim_v < dim_x || dim_v > 3) return SLDG_EINVAL;
     if (degree < 0 || degree > SLDG_MAX_DEGREE) return SLDG_EINVAL;
     const int d = dim_x + dim_v;
@@ -80,6 +105,7 @@ extern "C" int sldg_create(sldg_ctx** out, int dim_x, int dim_v, const int* cell
     sldg_ctx* c = new (std::nothrow) sldg_ctx();
     if (!c) return SLDG_ENOMEM;
     c->dx = dim_x; c->dv = dim_v; c->d = d; c->k = degree; c->K1 = degree + 1;
+    c->prec = precision; c->esize = precision == SLDG_F32 ? 4 : 8;
     c->nf = 1; c->X = 1; c->V = 1;
     for (int a = 0; a < d; a++) {
         c->cells[a] = cells[a];
@@ -265,9 +291,14 @@ static int upload_table(sldg_ctx* c, const double* delta, long long n, int N, in
     // the pinned staging buffers may still be in flight from a previous upload on this stream
     CK(cudaStreamSynchronize(c->stream));
     for (long long i = 0; i < n; i++) host_entry(c, delta[i], N, c->hS + i, c->hAB + (size_t)i * NN2);
+    if (c->prec == SLDG_F32) {          // A, B were evaluated in long double; the sweep takes them rounded to fp32
+        std::vector<float> h4((size_t)n * NN2);
+        for (size_t i = 0; i < h4.size(); i++) h4[i] = (float)c->hAB[i];
+        memcpy(c->hAB, h4.data(), h4.size() * 4);
+    }
     sldg_ev_begin(c, KIND_COPY, -1);
     CK(cudaMemcpyAsync(dS, c->hS, (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(dAB, c->hAB, (size_t)n * NN2 * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(dAB, c->hAB, (size_t)n * NN2 * c->esize, cudaMemcpyHostToDevice, c->stream));
     sldg_ev_end(c);
     return SLDG_OK;
 }
@@ -287,7 +318,7 @@ static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scrat
         sldg_ev_begin(c, KIND_SWEEP0, axis);
         e = cudaErrorNotSupported;
         if (c->opt_axis0_impl == 0 || c->opt_axis0_impl == 1) e = sldg_launch_sweep_line(c, fin, fout, g, t);
-        if (e == cudaErrorNotSupported && c->opt_axis0_impl != 3) {
+        if (e == cudaErrorNotSupported && c->opt_axis0_impl != 3 && c->prec == SLDG_F64) {
             e = sldg_launch_sweep_tma(c, fin, fout, g, t);
             if (e == cudaErrorInvalidConfiguration) e = cudaErrorNotSupported;
         }
@@ -317,7 +348,7 @@ static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scrat
 static int copy_back(sldg_ctx* c, double* dst, const double* src)
 {
     sldg_ev_begin(c, KIND_COPY, -1);
-    cudaError_t e = cudaMemcpyAsync(dst, src, (size_t)c->nf * 8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaError_t e = cudaMemcpyAsync(dst, src, (size_t)c->nf * c->esize, cudaMemcpyDeviceToDevice, c->stream);
     sldg_ev_end(c);
     if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
     return SLDG_OK;
@@ -389,7 +420,11 @@ struct XPlan { bool ok, fused, x1_oop; bool inplace[3]; int passes, flips; };
 
 static bool fused_possible(const sldg_ctx* c)
 {
-    return c->opt_fuse_x && c->dx >= 2 && c->D[0] <= c->opt_fused_threads;
+    if (!c->opt_fuse_x || c->dx < 2) return false;
+    if (c->prec == SLDG_F32)            // only the cell-per-thread kernel exists in fp32: its shape rules
+        return c->opt_fused_impl != 2 && c->K1 <= 4 && c->cells[0] <= 128 && ((c->K1 * c->D[0] * 4) & 15) == 0 &&
+               (size_t)4 * c->K1 * c->D[0] * 4 + 64 <= 227 * 1024;
+    return c->D[0] <= c->opt_fused_threads;
 }
 
 static XPlan x_plan(const sldg_ctx* c, bool flip)
@@ -435,7 +470,7 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
         sldg_ev_begin(c, KIND_FUSED, 0);
         cudaError_t e = cudaErrorNotSupported;
         if (c->opt_fused_impl != 2) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
-        if (e == cudaErrorNotSupported) e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        if (e == cudaErrorNotSupported && c->prec == SLDG_F64) e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
         sldg_ev_end(c);
         c->launches++;
         if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
@@ -615,10 +650,10 @@ extern "C" int sldg_step_host(sldg_ctx* c, double* f_host, double* f_dev, double
     int r = check_f(c, f_dev);
     if (r) return r;
     if (!f_host || nsteps < 0) return SLDG_EINVAL;
-    CK(cudaMemcpyAsync(f_dev, f_host, (size_t)c->nf * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(f_dev, f_host, (size_t)c->nf * c->esize, cudaMemcpyHostToDevice, c->stream));
     for (int s = 0; s < nsteps; s++)
         if ((r = sldg_step(c, f_dev, dt))) return r;
-    CK(cudaMemcpyAsync(f_host, f_dev, (size_t)c->nf * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(f_host, f_dev, (size_t)c->nf * c->esize, cudaMemcpyDeviceToHost, c->stream));
     if (E_host) CK(cudaMemcpyAsync(E_host, c->E, (size_t)c->X * 8 * c->dx, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return SLDG_OK;
@@ -648,7 +683,12 @@ extern "C" int sldg_advect_axis(sldg_ctx* c, double* f, int axis, const double* 
         }
         CK(cudaStreamSynchronize(c->stream));
         CK(cudaMemcpy(c->vS, S.data(), (size_t)X * 4, cudaMemcpyHostToDevice));
-        CK(cudaMemcpy(c->vAB, AB.data(), (size_t)(X * NN2) * 8, cudaMemcpyHostToDevice));
+        if (c->prec == SLDG_F32) {
+            std::vector<float> AB4(AB.size());
+            for (size_t i = 0; i < AB.size(); i++) AB4[i] = (float)AB[i];
+            CK(cudaMemcpy(c->vAB, AB4.data(), AB4.size() * 4, cudaMemcpyHostToDevice));
+        } else
+            CK(cudaMemcpy(c->vAB, AB.data(), (size_t)(X * NN2) * 8, cudaMemcpyHostToDevice));
         t.S = c->vS; t.AB = c->vAB; t.strideIdx = 1; t.strideM = X;
     }
     int axes[1] = {axis};

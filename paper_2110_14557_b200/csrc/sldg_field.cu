@@ -18,9 +18,9 @@ namespace {
 // ------------------------------------------------------------------ v-sweep shift table (row a5)
 // delta = ((-E) * tau) / h_v in exactly this operation order (reading O3); s = floor(delta), alpha = delta - s.
 // A(alpha), B(alpha) by Horner on the polynomial coefficients.  Output SoA: AB[m][X].
-template <int K1>
+template <int K1, class TAB>
 __global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double hv, int N, long long X,
-                              int* __restrict__ S, double* __restrict__ AB)
+                              int* __restrict__ S, TAB* __restrict__ AB)
 {
     long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (x >= X) return;
@@ -38,8 +38,8 @@ __global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double 
     for (int m = 0; m < NN; m++) {
         double a = sldg_horner<K1>(c_poly, 0, m, xc), b = sldg_horner<K1>(c_poly, 1, m, xc);
         if (cp) { a = (m % (K1 + 1) == 0) ? 1.0 : 0.0; b = 0.0; }
-        AB[(long long)m * X + x] = a;
-        AB[(long long)(NN + m) * X + x] = b;
+        AB[(long long)m * X + x] = (TAB)a;
+        AB[(long long)(NN + m) * X + x] = (TAB)b;
     }
 }
 
@@ -61,8 +61,12 @@ __global__ void wv_kernel(WvParams P, double* __restrict__ Wv)
 // ------------------------------------------------------------------ rho (row a3)
 // f seen as [V][X] (X contiguous).  Block = 128 threads x 2 values along x; grid.y splits V into chunks.
 // Each chunk writes a partial sum; a second kernel adds the partials in a fixed order (deterministic).
-template <int VEC>
-__global__ void __launch_bounds__(128) rho_partial_kernel(const double* __restrict__ f, const double* __restrict__ Wv,
+template <class T> struct Pair;
+template <> struct Pair<double> { typedef double2 type; };
+template <> struct Pair<float> { typedef float2 type; };
+
+template <int VEC, class T>
+__global__ void __launch_bounds__(128) rho_partial_kernel(const T* __restrict__ f, const double* __restrict__ Wv,
                                                           long long X, long long V, long long vchunk,
                                                           double* __restrict__ part)
 {
@@ -74,24 +78,24 @@ __global__ void __launch_bounds__(128) rho_partial_kernel(const double* __restri
     constexpr int U = SLDG_RHO_U;
     long long v = v0;
     for (; v + U <= v1; v += U) {
-        double t[U][VEC];
+        T t[U][VEC];
 #pragma unroll
         for (int u = 0; u < U; u++) {
-            const double* p = f + (v + u) * X + x;
-            if (VEC == 2) { double2 d = __ldcs(reinterpret_cast<const double2*>(p)); t[u][0] = d.x; t[u][VEC - 1] = d.y; }
+            const T* p = f + (v + u) * X + x;
+            if (VEC == 2) { typename Pair<T>::type d = __ldcs(reinterpret_cast<const typename Pair<T>::type*>(p)); t[u][0] = d.x; t[u][VEC - 1] = d.y; }
             else t[u][0] = __ldcs(p);
         }
 #pragma unroll
         for (int u = 0; u < U; u++) {
             double wv = __ldg(Wv + v + u);
 #pragma unroll
-            for (int e = 0; e < VEC; e++) acc[e] = fma(wv, t[u][e], acc[e]);
+            for (int e = 0; e < VEC; e++) acc[e] = fma(wv, (double)t[u][e], acc[e]);
         }
     }
     for (; v < v1; v++) {
         double wv = __ldg(Wv + v);
 #pragma unroll
-        for (int e = 0; e < VEC; e++) acc[e] = fma(wv, __ldcs(f + v * X + x + e), acc[e]);
+        for (int e = 0; e < VEC; e++) acc[e] = fma(wv, (double)__ldcs(f + v * X + x + e), acc[e]);
     }
 #pragma unroll
     for (int e = 0; e < VEC; e++) part[(long long)blockIdx.y * X + x + e] = acc[e];
@@ -171,7 +175,8 @@ __device__ __forceinline__ double block_sum(double v)
 }
 
 // partial[b] = sum over a grid-stride slice of  W_n * g(n);  NCOMP = 0: g = f[n];  NCOMP > 0: g = sum_d E_d[n]^2
-__global__ void __launch_bounds__(256) weighted_sum_kernel(WgtParams P, const double* __restrict__ a, int ncomp,
+template <class T>
+__global__ void __launch_bounds__(256) weighted_sum_kernel(WgtParams P, const T* __restrict__ a, int ncomp,
                                                            double* __restrict__ partial)
 {
     double acc = 0.0;
@@ -181,8 +186,8 @@ __global__ void __launch_bounds__(256) weighted_sum_kernel(WgtParams P, const do
         double wn = 1.0;
         for (int d = 0; d < P.nd; d++) { long long n = r % P.D[d]; r /= P.D[d]; wn *= P.w[d][n]; }
         double g;
-        if (ncomp == 0) g = a[t];
-        else { g = 0.0; for (int d = 0; d < ncomp; d++) { double e = a[(long long)d * P.total + t]; g = fma(e, e, g); } }
+        if (ncomp == 0) g = (double)a[t];
+        else { g = 0.0; for (int d = 0; d < ncomp; d++) { double e = (double)a[(long long)d * P.total + t]; g = fma(e, e, g); } }
         acc = fma(wn, g, acc);
     }
     acc = block_sum(acc);
@@ -199,17 +204,25 @@ __global__ void __launch_bounds__(256) final_sum_kernel(const double* __restrict
 
 }  // namespace
 
-cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB)
+template <class TAB>
+static void vtable_dispatch(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, TAB* AB)
 {
     int block = 128;
     unsigned grid = (unsigned)((c->X + block - 1) / block);
     switch (c->K1) {
-    case 1: vtable_kernel<1><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 2: vtable_kernel<2><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 3: vtable_kernel<3><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 4: vtable_kernel<4><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 5: vtable_kernel<5><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 1: vtable_kernel<1, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 2: vtable_kernel<2, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 3: vtable_kernel<3, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 4: vtable_kernel<4, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 5: vtable_kernel<5, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
     }
+}
+
+// A, B are evaluated in fp64 and stored in the sweep's type (float in single precision mode, reading W)
+cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB)
+{
+    if (c->prec == SLDG_F32) vtable_dispatch<float>(c, Ed, tau, hv, N, S, reinterpret_cast<float*>(AB));
+    else vtable_dispatch<double>(c, Ed, tau, hv, N, S, AB);
     return cudaGetLastError();
 }
 
@@ -226,7 +239,8 @@ cudaError_t sldg_launch_wv(sldg_ctx* c)
 cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho)
 {
     const long long X = c->X, V = c->V;
-    int vec = ((X & 1) == 0 && (((uintptr_t)f) & 15) == 0) ? 2 : 1;
+    const bool f32 = c->prec == SLDG_F32;
+    int vec = ((X & 1) == 0 && (((uintptr_t)f) & (f32 ? 7 : 15)) == 0) ? 2 : 1;
     if (c->opt_rho_vec == 1) vec = 1;
     long long xtiles = (X + 128LL * vec - 1) / (128LL * vec);
     // ONE wave of equal blocks: at most opt_rho_blocks (8) blocks per SM, rounded DOWN so that no second, partial
@@ -240,8 +254,11 @@ cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho)
     long long vchunk = (V + nchunk - 1) / nchunk;
     nchunk = (V + vchunk - 1) / vchunk;
     dim3 grid((unsigned)xtiles, (unsigned)nchunk);
-    if (vec == 2) rho_partial_kernel<2><<<grid, 128, 0, c->stream>>>(f, c->Wv, X, V, vchunk, c->part);
-    else rho_partial_kernel<1><<<grid, 128, 0, c->stream>>>(f, c->Wv, X, V, vchunk, c->part);
+    const float* f4 = reinterpret_cast<const float*>(f);
+    if (f32 && vec == 2) rho_partial_kernel<2, float><<<grid, 128, 0, c->stream>>>(f4, c->Wv, X, V, vchunk, c->part);
+    else if (f32) rho_partial_kernel<1, float><<<grid, 128, 0, c->stream>>>(f4, c->Wv, X, V, vchunk, c->part);
+    else if (vec == 2) rho_partial_kernel<2, double><<<grid, 128, 0, c->stream>>>(f, c->Wv, X, V, vchunk, c->part);
+    else rho_partial_kernel<1, double><<<grid, 128, 0, c->stream>>>(f, c->Wv, X, V, vchunk, c->part);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     rho_final_kernel<<<(unsigned)((X + 255) / 256), 256, 0, c->stream>>>(c->part, X, (int)nchunk, rho);
@@ -289,7 +306,8 @@ cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E)
     return cudaGetLastError();
 }
 
-static cudaError_t weighted_sum(sldg_ctx* c, const double* a, int nd, int axis0, int ncomp, long long total,
+template <class T>
+static cudaError_t weighted_sum(sldg_ctx* c, const T* a, int nd, int axis0, int ncomp, long long total,
                                 double scale, double* out1)
 {
     WgtParams P;
@@ -297,7 +315,7 @@ static cudaError_t weighted_sum(sldg_ctx* c, const double* a, int nd, int axis0,
     for (int d = 0; d < nd; d++) { P.D[d] = c->D[axis0 + d]; P.w[d] = c->dWx[axis0 + d]; }
     long long nb = (total + 255) / 256;
     if (nb > 2048) nb = 2048;
-    weighted_sum_kernel<<<(unsigned)nb, 256, 0, c->stream>>>(P, a, ncomp, c->red);
+    weighted_sum_kernel<T><<<(unsigned)nb, 256, 0, c->stream>>>(P, a, ncomp, c->red);
     final_sum_kernel<<<1, 256, 0, c->stream>>>(c->red, (int)nb, scale, out1);
     c->launches += 2;
     return cudaGetLastError();
@@ -310,5 +328,6 @@ cudaError_t sldg_launch_energy(sldg_ctx* c, const double* E, double* out1)
 
 cudaError_t sldg_launch_mass(sldg_ctx* c, const double* f, double* out1)
 {
+    if (c->prec == SLDG_F32) return weighted_sum(c, reinterpret_cast<const float*>(f), c->d, 0, 0, c->nf, 1.0, out1);
     return weighted_sum(c, f, c->d, 0, 0, c->nf, 1.0, out1);
 }

@@ -48,7 +48,7 @@ SLDG_HD double sldg_horner(const Coef& c, int which, int m, double xc)
 
 struct ShiftTable {          // device-resident shift table of one sweep
     const int* S;            // [n]  (s mod N) | copy bit
-    const double* AB;        // A then B, element m of index i at AB[i*strideIdx + m*strideM]
+    const void* AB;          // A then B (double, or float in single precision mode), element m of index i at AB[i*strideIdx + m*strideM]
     long long strideIdx, strideM;
 };
 
@@ -66,6 +66,8 @@ struct EventRec { cudaEvent_t a, b; int kind, axis; };
 
 struct sldg_ctx {
     int dx, dv, d, k, K1;
+    int prec;                       // SLDG_F64 / SLDG_F32: storage and sweep arithmetic type of f (reading W)
+    size_t esize;                   // bytes per value of f
     int cells[SLDG_MAX_DIM];
     long long D[SLDG_MAX_DIM];
     double lo[SLDG_MAX_DIM], hi[SLDG_MAX_DIM], h[SLDG_MAX_DIM];
@@ -144,6 +146,17 @@ void sldg_eval_AB_host(const ABPolyLD* p, int k, double alpha, double* A, double
 void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* invT);
 
 // ---- kernel launchers (each returns cudaError_t of the launch)
+// walk / line / fused-cell kernels exist in both precisions (sldg_real.h): _f64 and _f32 launchers; fin/fout are
+// arrays of that type.  The un-suffixed names (sldg_api.cu) dispatch on ctx->prec.
+#define SLDG_DECL_SWEEPS(sfx)                                                                                       \
+    cudaError_t sldg_launch_sweep_walk##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g,           \
+                                            const ShiftTable& t);                                                   \
+    cudaError_t sldg_launch_sweep_line##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g,           \
+                                            const ShiftTable& t);                                                   \
+    cudaError_t sldg_launch_sweep_fused_cell##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,    \
+                                                  const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
+SLDG_DECL_SWEEPS(_f64)
+SLDG_DECL_SWEEPS(_f32)
 cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
                                    const ShiftTable& t);
 cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,

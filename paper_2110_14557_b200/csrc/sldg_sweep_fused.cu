@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(256) sweep_fused_kernel(const FusedParams P)
         int ia = cell - s; if (ia < 0) ia += N0;
         int ib = ia - 1; if (ib < 0) ib += N0;
         da = pl * D0 + ia * K1; db = pl * D0 + ib * K1;
-        const double* ab = P.t0.AB + idx * P.t0.strideIdx;
+        const double* ab = static_cast<const double*>(P.t0.AB) + idx * P.t0.strideIdx;
 #pragma unroll
         for (int m = 0; m < K1; m++) {
             a1[m] = __ldg(ab + (jj * K1 + m) * P.t0.strideM);
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(256) sweep_fused_kernel(const FusedParams P)
         const int sv = __ldg(P.t1.S + idx);
         cp2 = (sv & SLDG_COPY_BIT) != 0;
         s2 = sv & SLDG_S_MASK;
-        const double* ab = P.t1.AB + idx * P.t1.strideIdx;
+        const double* ab = static_cast<const double*>(P.t1.AB) + idx * P.t1.strideIdx;
 #pragma unroll
         for (int m = 0; m < NN; m++) {
             A[m] = __ldg(ab + m * P.t1.strideM);

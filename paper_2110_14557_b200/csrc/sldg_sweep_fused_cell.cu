@@ -20,17 +20,18 @@
 //
 // One __syncthreads per chunk releases the input stage and publishes the output stage.  Every value is read once
 // and written once.  The shift of x_1 depends on the plane's v_1 node, that of x_2 on its v_2 node.  Out of place
-// only (fin != fout); D_0 must be even (16-byte rule of the bulk copies).
+// only (fin != fout); the k+1 rows of a cell must be a multiple of 16 bytes (rule of the bulk copies).
 #include "sldg_async.h"
 #include "sldg_internal.h"
+#include "sldg_real.h"
 
 namespace {
 
 using namespace sldg_async;
 
 struct CellParams {
-    const double* fin;
-    double* fout;
+    const real* fin;
+    real* fout;
     long long planes;             // prod of D_b, b >= 2
     int N0, N1, PB, CR, stages;   // cells along x_1, x_2; planes per block; x_2 cells per chunk; input stages
     long long sdiv0, sdiv1;       // shift index of plane q: (q / sdiv) % smod, per axis
@@ -41,13 +42,13 @@ struct CellParams {
 constexpr int OST = 2;            // output stages
 
 template <int K1> struct CellV {
-    double v[K1];
-    __device__ __forceinline__ void load(const double* p)
+    real v[K1];
+    __device__ __forceinline__ void load(const real* p)
     {
         if constexpr (K1 % 2 == 0) {
 #pragma unroll
             for (int j = 0; j < K1; j += 2) {
-                double2 t = *reinterpret_cast<const double2*>(p + j);
+                real2 t = *reinterpret_cast<const real2*>(p + j);
                 v[j] = t.x; v[j + 1] = t.y;
             }
         } else {
@@ -55,11 +56,11 @@ template <int K1> struct CellV {
             for (int j = 0; j < K1; j++) v[j] = p[j];
         }
     }
-    __device__ __forceinline__ void store(double* p) const
+    __device__ __forceinline__ void store(real* p) const
     {
         if constexpr (K1 % 2 == 0) {
 #pragma unroll
-            for (int j = 0; j < K1; j += 2) *reinterpret_cast<double2*>(p + j) = make_double2(v[j], v[j + 1]);
+            for (int j = 0; j < K1; j += 2) *reinterpret_cast<real2*>(p + j) = make_real2(v[j], v[j + 1]);
         } else {
 #pragma unroll
             for (int j = 0; j < K1; j++) p[j] = v[j];
@@ -75,10 +76,10 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     const int N0 = P.N0, N1 = P.N1, D0 = N0 * K1, CR = P.CR, ST = P.stages;
     const int PC = CR * K1 * D0;                       // doubles of one plane's chunk
     const int SS = P.PB * PC;                          // doubles of one stage
-    double* const sin_ = reinterpret_cast<double*>(smem_raw);
-    double* const sout = sin_ + (size_t)ST * SS;
+    real* const sin_ = reinterpret_cast<real*>(smem_raw);
+    real* const sout = sin_ + (size_t)ST * SS;
     const uint32_t sin_s = smem_u32(sin_), sout_s = smem_u32(sout);
-    const uint32_t bars_s = smem_u32(sout + (size_t)OST * SS);
+    const uint32_t bars_s = (smem_u32(sout + (size_t)OST * SS) + 7u) & ~7u;
 
     const int t = threadIdx.x;
     const int pl = t / N0, i = t - pl * N0;
@@ -89,10 +90,10 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     const int nlive = (int)min((long long)P.PB, P.planes - q0);
     const long long qq = live ? q : P.planes - 1;      // dead threads shadow the last plane (no copies, no stores)
     const long long D1 = (long long)N1 * K1;
-    const double* const gin = P.fin + qq * D1 * D0;
-    double* const gout = P.fout + qq * D1 * D0;
+    const real* const gin = P.fin + qq * D1 * D0;
+    real* const gout = P.fout + qq * D1 * D0;
     const int NCH = 1 + (N1 - 1 + CR - 1) / CR;        // input chunks: cell 0 alone, then CR cells each
-    const uint32_t cell_bytes = (uint32_t)(K1 * D0) * 8u;
+    const uint32_t cell_bytes = (uint32_t)(K1 * D0) * (uint32_t)sizeof(real);
 
     auto issue_load = [&](int j) {                     // plane leaders only
         if (leader && j < NCH) {
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
             const int nc = (j == 0) ? 1 : min(CR, N1 - c0);
             const uint32_t bar = bars_s + (uint32_t)st * 8u;
             mbar_expect_tx(bar, nc * cell_bytes);
-            bulk_load(sin_s + (uint32_t)(st * SS + pl * PC) * 8u, gin + (long long)c0 * K1 * D0, nc * cell_bytes, bar);
+            bulk_load(sin_s + (uint32_t)(st * SS + pl * PC) * (uint32_t)sizeof(real), gin + (long long)c0 * K1 * D0, nc * cell_bytes, bar);
         }
     };
 
@@ -113,7 +114,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     for (int j = 0; j < ST; j++) issue_load(j);
 
     // ---- x_1: A_1, B_1 and the offsets of the two donor cells inside a row
-    double A1[NN], B1[NN];
+    real A1[NN], B1[NN];
     int oa, ob;
     bool cp1;
     {
@@ -124,7 +125,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         int ia = i - s; if (ia < 0) ia += N0;
         int ib = ia - 1; if (ib < 0) ib += N0;
         oa = ia * K1; ob = ib * K1;
-        const double* ab = P.t0.AB + idx * P.t0.strideIdx;
+        const real* ab = static_cast<const real*>(P.t0.AB) + idx * P.t0.strideIdx;
 #pragma unroll
         for (int m = 0; m < NN; m++) {
             A1[m] = __ldg(ab + m * P.t0.strideM);
@@ -132,7 +133,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         }
     }
     // ---- x_2: A_2, B_2, shift
-    double A2[NN], B2[NN];
+    real A2[NN], B2[NN];
     int s2;
     bool cp2;
     {
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         const int sv = __ldg(P.t1.S + idx);
         cp2 = (sv & SLDG_COPY_BIT) != 0;
         s2 = sv & SLDG_S_MASK;
-        const double* ab = P.t1.AB + idx * P.t1.strideIdx;
+        const real* ab = static_cast<const real*>(P.t1.AB) + idx * P.t1.strideIdx;
 #pragma unroll
         for (int m = 0; m < NN; m++) {
             A2[m] = __ldg(ab + m * P.t1.strideM);
@@ -149,16 +150,16 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     }
 
     // x_1-swept (k+1) x (k+1) block [x_2 node j2][x_1 node j1] of this thread's cell from the k+1 rows at `rows`
-    auto swept = [&](const double* rows, double (&N)[NN]) {
+    auto swept = [&](const real* rows, real (&N)[NN]) {
 #pragma unroll
         for (int j2 = 0; j2 < K1; j2++) {
-            const double* row = rows + j2 * D0;
+            const real* row = rows + j2 * D0;
             CellV<K1> a, b;
             a.load(row + oa);
             b.load(row + ob);
 #pragma unroll
             for (int j1 = 0; j1 < K1; j1++) {
-                double acc = 0.0;
+                real acc = 0;
 #pragma unroll
                 for (int m = 0; m < K1; m++) acc += A1[j1 * K1 + m] * a.v[m];
 #pragma unroll
@@ -168,7 +169,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         }
     };
 
-    double first[NN], prev[NN];
+    real first[NN], prev[NN];
     // chunk 0: cell 0 alone
     mbar_wait(bars_s, 0u);
     swept(sin_ + pl * PC, first);
@@ -185,10 +186,10 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         const int nin = min(CR, N1 - 1 - h * CR);      // cells of that chunk (<= 0: none, the wrap cell is `first`)
         const int nout = min(CR, N1 - h * CR);
         if (nin > 0) mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
-        const double* ibase = sin_ + st * SS + pl * PC;
-        double* obase = sout + (h & 1) * SS + pl * PC + i * K1;
+        const real* ibase = sin_ + st * SS + pl * PC;
+        real* obase = sout + (h & 1) * SS + pl * PC + i * K1;
         for (int e = 0; e < nout; e++) {
-            double nxt[NN];
+            real nxt[NN];
             if (e < nin) swept(ibase + e * K1 * D0, nxt);
             else {
 #pragma unroll
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
                 CellV<K1> r;
 #pragma unroll
                 for (int j1 = 0; j1 < K1; j1++) {
-                    double acc = 0.0;
+                    real acc = 0;
 #pragma unroll
                     for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
 #pragma unroll
@@ -215,7 +216,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         if (leader) bulk_wait_read<0>();               // the store of group h-1 has left its output stage
         __syncthreads();
         if (leader) {
-            const uint32_t src = sout_s + (uint32_t)((h & 1) * SS + pl * PC) * 8u;
+            const uint32_t src = sout_s + (uint32_t)((h & 1) * SS + pl * PC) * (uint32_t)sizeof(real);
             const int n1 = min(nout, N1 - io0);
             bulk_store(gout + (long long)io0 * K1 * D0, src, (uint32_t)n1 * cell_bytes);
             if (nout > n1) bulk_store(gout, src + (uint32_t)n1 * cell_bytes, (uint32_t)(nout - n1) * cell_bytes);
@@ -243,22 +244,22 @@ cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem)
 
 // g0, g1: geometry of axis 0 and axis 1.  Returns cudaErrorNotSupported when the shape does not fit (the caller
 // falls back to the node-per-thread fused kernel, then to separate sweeps).
-cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
-                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,
+                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
 {
     if (g1.outer == 0) return cudaSuccess;
     const long long D0 = (long long)g0.N * g0.K1, D1 = (long long)g1.N * g1.K1;
     const int K1 = g0.K1;
     if (fin == fout || g1.inner != D0 || g0.mode != 0 || g1.mode != 0 || g0.sdiv % D1 != 0) return cudaErrorNotSupported;
-    if (K1 > 4 || (D0 & 1) || g0.N > 128) return cudaErrorNotSupported;
+    if (K1 > 4 || (((long long)K1 * D0 * sizeof(real)) & 15) || g0.N > 128) return cudaErrorNotSupported;
     if ((((uintptr_t)fin) | ((uintptr_t)fout)) & 15) return cudaErrorNotSupported;
     CellParams P;
-    P.fin = fin; P.fout = fout; P.planes = g1.outer;
+    P.fin = static_cast<const real*>(fin); P.fout = static_cast<real*>(fout); P.planes = g1.outer;
     P.N0 = g0.N; P.N1 = g1.N;
     long long PB = c->opt_cell_threads / g0.N;
     if (PB < 1) PB = 1;
     if (PB > P.planes) PB = P.planes;
-    const long long cellb = (long long)K1 * D0 * 8;            // bytes of one x_2 cell of one plane
+    const long long cellb = (long long)K1 * D0 * sizeof(real);            // bytes of one x_2 cell of one plane
     // Measured on B200 (cfg2-5): 64-thread blocks, 2 input stages of about 9 KB each, i.e. many small resident
     // blocks, reach the copy rate; larger stages or deeper rings lose occupancy and run slower.
     long long CR = c->opt_cell_rows > 0 ? c->opt_cell_rows : c->opt_cell_bytes / (PB * cellb);

@@ -21,6 +21,7 @@
 // inside the same kernel.  The shift index of line q is (q / sdiv) % smod; it is computed once per batch and
 // tracked incrementally inside it; A, B are re-read from the (L1-resident) table only when the index changes.
 #include "sldg_internal.h"
+#include "sldg_real.h"
 
 namespace {
 
@@ -29,8 +30,8 @@ constexpr int OSTAGES = 2;        // output buffers per warp
 constexpr int MAXBATCH = 8;       // chunks per claim: STAGES <= batch <= MAXBATCH (issue side at most one batch ahead)
 
 struct LineParams {
-    const double* fin;
-    double* fout;
+    const real* fin;
+    real* fout;
     unsigned long long* counter;  // [0] next batch, [1] warps done
     long long nlines, nchunks;
     int N, L;                     // cells per line, lines per chunk
@@ -76,13 +77,13 @@ __device__ __forceinline__ void bulk_store(void* gdst, uint32_t smem_src, uint32
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 
 template <int K1> struct Cell {
-    double v[K1];
-    __device__ __forceinline__ void load(const double* p)
+    real v[K1];
+    __device__ __forceinline__ void load(const real* p)
     {
         if constexpr (K1 % 2 == 0) {
 #pragma unroll
             for (int j = 0; j < K1; j += 2) {
-                double2 t = *reinterpret_cast<const double2*>(p + j);
+                real2 t = *reinterpret_cast<const real2*>(p + j);
                 v[j] = t.x; v[j + 1] = t.y;
             }
         } else {
@@ -90,11 +91,11 @@ template <int K1> struct Cell {
             for (int j = 0; j < K1; j++) v[j] = p[j];
         }
     }
-    __device__ __forceinline__ void store(double* p) const
+    __device__ __forceinline__ void store(real* p) const
     {
         if constexpr (K1 % 2 == 0) {
 #pragma unroll
-            for (int j = 0; j < K1; j += 2) *reinterpret_cast<double2*>(p + j) = make_double2(v[j], v[j + 1]);
+            for (int j = 0; j < K1; j += 2) *reinterpret_cast<real2*>(p + j) = make_real2(v[j], v[j + 1]);
         } else {
 #pragma unroll
             for (int j = 0; j < K1; j++) p[j] = v[j];
@@ -115,9 +116,9 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
     const long long chunk_vals = (long long)P.L * D0;
 
     // per-warp shared memory: STAGES input buffers, OSTAGES output buffers; barriers behind all buffers
-    double* wbase = reinterpret_cast<double*>(smem_raw) + (size_t)wib * (STAGES + OSTAGES) * cap;
+    real* wbase = reinterpret_cast<real*>(smem_raw) + (size_t)wib * (STAGES + OSTAGES) * cap;
     const uint32_t wbase_s = smem_u32(wbase);
-    const uint32_t bars_s = smem_u32(reinterpret_cast<double*>(smem_raw) + (size_t)WARPS * (STAGES + OSTAGES) * cap) +
+    const uint32_t bars_s = smem_u32(reinterpret_cast<real*>(smem_raw) + (size_t)WARPS * (STAGES + OSTAGES) * cap) +
                             (uint32_t)wib * STAGES * 8u;
 
     // claim(): lane 0 fires the atomic; the value is read (shuffled) one batch later
@@ -129,9 +130,9 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
         if (lane == 0 && c < nchunks) {
             const bool last = (c == nchunks - 1);
             if (last ? P.last_tma : P.full_tma) {
-                const uint32_t bytes = (uint32_t)((last ? P.last_nl : P.L) * D0) * 8u;
+                const uint32_t bytes = (uint32_t)((last ? P.last_nl : P.L) * D0) * (uint32_t)sizeof(real);
                 mbar_expect_tx(bars_s + st * 8u, bytes);
-                bulk_load(wbase_s + (uint32_t)(st * cap) * 8u, P.fin + c * chunk_vals, bytes, bars_s + st * 8u);
+                bulk_load(wbase_s + (uint32_t)(st * cap) * (uint32_t)sizeof(real), P.fin + c * chunk_vals, bytes, bars_s + st * 8u);
             }
         }
     };
@@ -157,7 +158,7 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
     int lane_l = 0, lane_i = lane;                        // (line, cell) of the lane's first cell in a chunk
     while (lane_i >= N) { lane_i -= N; lane_l++; }
 
-    double A[NN], B[NN];
+    real A[NN], B[NN];
     int cur = -1, s = 0;
     bool cp = false;
     uint32_t phases = 0;          // bit st = parity the next wait on barrier st expects
@@ -173,8 +174,8 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
         const int nl = last ? P.last_nl : P.L;
         const int nval = nl * D0;
         const bool tma = (last ? P.last_tma : P.full_tma) != 0;
-        double* sin_ = wbase + st * cap;
-        double* sout = wbase + (STAGES + ost) * cap;
+        real* sin_ = wbase + st * cap;
+        real* sout = wbase + (STAGES + ost) * cap;
 
         if (newbatch) {           // the only integer divisions of the kernel: once per batch
             const long long q0 = c * P.L;
@@ -189,7 +190,7 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
             mbar_wait(bars_s + st * 8u, (phases >> st) & 1u);
             phases ^= 1u << st;
         } else {
-            const double* gin = P.fin + c * chunk_vals;
+            const real* gin = P.fin + c * chunk_vals;
             for (int t = lane; t < nval; t += 32) sin_[t] = gin[t];
         }
         // the bulk store that read sout two turns ago must have finished reading shared memory
@@ -202,16 +203,16 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
             int left = r0c - lane_l;                       // lines before the shift index changes
             int idxl = idx0;
             while (left <= 0) { left += sdivc; idxl = (idxl + 1 == P.smod) ? 0 : idxl + 1; }
-            const double* pl = sin_ + lane_l * D0;         // start of the lane's current line
-            double* po = sout + lane * K1;
-            const double* pend = sout + nl * D0;
+            const real* pl = sin_ + lane_l * D0;         // start of the lane's current line
+            real* po = sout + lane * K1;
+            const real* pend = sout + nl * D0;
             for (; po < pend; po += 32 * K1) {
                 if (idxl != cur) {
                     cur = idxl;
                     const int sv = __ldg(P.t.S + idxl);
                     cp = (sv & SLDG_COPY_BIT) != 0;
                     s = sv & SLDG_S_MASK;
-                    const double* ab = P.t.AB + (long long)idxl * P.t.strideIdx;
+                    const real* ab = static_cast<const real*>(P.t.AB) + (long long)idxl * P.t.strideIdx;
 #pragma unroll
                     for (int m = 0; m < NN; m++) {
                         A[m] = __ldg(ab + m * P.t.strideM);
@@ -226,7 +227,7 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
                     b.load(pl + ib * K1);
 #pragma unroll
                     for (int j = 0; j < K1; j++) {
-                        double acc = 0.0;
+                        real acc = 0;
 #pragma unroll
                         for (int m = 0; m < K1; m++) acc += A[j * K1 + m] * a.v[m];
 #pragma unroll
@@ -251,11 +252,11 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
         if (tma) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> async proxy
             __syncwarp();
-            if (lane == 0) bulk_store(P.fout + c * chunk_vals, wbase_s + (uint32_t)((STAGES + ost) * cap) * 8u,
-                                      (uint32_t)nval * 8u);
+            if (lane == 0) bulk_store(P.fout + c * chunk_vals, wbase_s + (uint32_t)((STAGES + ost) * cap) * (uint32_t)sizeof(real),
+                                      (uint32_t)nval * (uint32_t)sizeof(real));
         } else {
             __syncwarp();
-            double* gout = P.fout + c * chunk_vals;
+            real* gout = P.fout + c * chunk_vals;
             for (int t = lane; t < nval; t += 32) gout[t] = sout[t];
             __syncwarp();
         }
@@ -326,16 +327,17 @@ cudaError_t dispatch(sldg_ctx* c, LineParams& P, int stages, size_t smem)
 }  // namespace
 
 // Shared memory of one CTA for `stages` input buffers of `cap` doubles per warp.
-static size_t line_smem(int stages, long long cap) { return (size_t)WARPS * (stages + OSTAGES) * cap * 8 + WARPS * 4 * 8 + 16; }
+static size_t line_smem(int stages, long long cap) { return (size_t)WARPS * (stages + OSTAGES) * cap * sizeof(real) + WARPS * 4 * 8 + 16; }
 
 // Returns cudaErrorNotSupported when a line is too long for the per-warp pipelines (caller falls back).
-cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
-                                   const ShiftTable& t)
+cudaError_t SLDG_SFX(sldg_launch_sweep_line)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g,
+                                             const ShiftTable& t)
 {
     if (g.outer == 0) return cudaSuccess;
     if (g.smod > 0x7fffffffLL || !c->dCounter) return cudaErrorNotSupported;
     const long long D0 = (long long)g.N * g.K1;
-    const long long line_bytes = D0 * 8;
+    const long long line_bytes = D0 * (long long)sizeof(real);
+    const long long Q = 16 / (long long)sizeof(real);            // values per 16 bytes
     const size_t smem_max = 227 * 1024;
     int stages = c->opt_tile_stages;
     if (stages < 1) stages = 1;
@@ -344,17 +346,17 @@ cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout,
     // (keeps chunk starts 16-byte aligned), and no more than fits STAGES + OSTAGES times per warp
     long long L = c->opt_tile_bytes / line_bytes;
     if (L < 1) L = 1;
-    auto cap_of = [&](long long l) { return (l * D0 + 1) & ~1LL; };
+    auto cap_of = [&](long long l) { return (l * D0 + Q - 1) / Q * Q; };
     while (L > 1 && line_smem(stages, cap_of(L)) > smem_max) L--;
     while (stages > 1 && line_smem(stages, cap_of(L)) > smem_max) stages--;
     if (line_smem(stages, cap_of(L)) > smem_max) return cudaErrorNotSupported;
     // small problems: shorter chunks so that there are a few chunks per warp
     const long long want_chunks = 4LL * c->sm_count * WARPS * stages;
     if (g.outer / L < want_chunks) { L = g.outer / want_chunks; if (L < 1) L = 1; }
-    if ((D0 & 1) && L > 1) L &= ~1LL;
+    if ((D0 % Q) && L >= Q) L = L / Q * Q;                        // chunk starts stay 16-byte aligned
     if (L > g.outer) L = g.outer;
     LineParams P;
-    P.fin = fin; P.fout = fout; P.counter = c->dCounter;
+    P.fin = static_cast<const real*>(fin); P.fout = static_cast<real*>(fout); P.counter = c->dCounter;
     P.nlines = g.outer; P.N = g.N; P.L = (int)L; P.batch = MAXBATCH; P.cap = (int)cap_of(L);
     P.nchunks = (g.outer + L - 1) / L;
     P.last_nl = (int)(g.outer - (P.nchunks - 1) * L);

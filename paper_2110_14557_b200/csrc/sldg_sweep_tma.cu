@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(256) sweep_tma_kernel(const TmaParams P)
             int sv = __ldg(P.t.S + idx);
             cp = (sv & SLDG_COPY_BIT) != 0;
             s = sv & SLDG_S_MASK;
-            const double* ab = P.t.AB + idx * P.t.strideIdx;
+            const double* ab = static_cast<const double*>(P.t.AB) + idx * P.t.strideIdx;
 #pragma unroll
             for (int m = 0; m < NN; m++) {
                 A[m] = __ldg(ab + m * P.t.strideM);

@@ -9,12 +9,13 @@
 // (j + s + 1) mod N = A u_{j+1} + B u_j.  The first cell is kept to close the periodic wrap, so every value
 // is read exactly once and written exactly once (16 B per value, the algorithmic minimum).
 #include "sldg_internal.h"
+#include "sldg_real.h"
 
 namespace {
 
 struct WalkParams {
-    const double* fin;
-    double* fout;
+    const real* fin;
+    real* fout;
     long long innerV, inner, nwork;
     int N;
     long long sdiv, smod;
@@ -23,20 +24,20 @@ struct WalkParams {
 
 template <int VEC> struct Vec;
 template <> struct Vec<1> {
-    double v[1];
-    __device__ __forceinline__ void load(const double* p) { v[0] = __ldcs(p); }
-    __device__ __forceinline__ void store(double* p) const { __stcs(p, v[0]); }
+    real v[1];
+    __device__ __forceinline__ void load(const real* p) { v[0] = __ldcs(p); }
+    __device__ __forceinline__ void store(real* p) const { __stcs(p, v[0]); }
 };
 template <> struct Vec<2> {
-    double v[2];
-    __device__ __forceinline__ void load(const double* p)
+    real v[2];
+    __device__ __forceinline__ void load(const real* p)
     {
-        double2 t = __ldcs(reinterpret_cast<const double2*>(p));
+        real2 t = __ldcs(reinterpret_cast<const real2*>(p));
         v[0] = t.x; v[1] = t.y;
     }
-    __device__ __forceinline__ void store(double* p) const
+    __device__ __forceinline__ void store(real* p) const
     {
-        __stcs(reinterpret_cast<double2*>(p), make_double2(v[0], v[1]));
+        __stcs(reinterpret_cast<real2*>(p), make_real2(v[0], v[1]));
     }
 };
 
@@ -76,7 +77,7 @@ __global__ void __launch_bounds__(256) sweep_walk_kernel(const WalkParams P)
         q = g / P.innerV; p = (g - q * P.innerV) * VEC;
     }
 
-    double A[NS][NN], B[NS][NN];
+    real A[NS][NN], B[NS][NN];
     int s[NS];
     bool cp[NS];
 #pragma unroll
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(256) sweep_walk_kernel(const WalkParams P)
         int sv = __ldg(P.t.S + idx);
         cp[e] = (sv & SLDG_COPY_BIT) != 0;
         s[e] = sv & SLDG_S_MASK;
-        const double* ab = P.t.AB + idx * P.t.strideIdx;
+        const real* ab = static_cast<const real*>(P.t.AB) + idx * P.t.strideIdx;
 #pragma unroll
         for (int m = 0; m < NN; m++) {
             A[e][m] = __ldg(ab + m * P.t.strideM);
@@ -96,8 +97,8 @@ __global__ void __launch_bounds__(256) sweep_walk_kernel(const WalkParams P)
     const int N = P.N;
     const long long rs = P.inner;                       // row stride (elements)
     const long long base = q * (long long)N * K1 * rs + p;
-    const double* in = P.fin + base;
-    double* out = P.fout + base;
+    const real* in = P.fin + base;
+    real* out = P.fout + base;
 
     Vec<VEC> first[K1], prev[K1], nxt[U][K1];
 #pragma unroll
@@ -129,7 +130,7 @@ __global__ void __launch_bounds__(256) sweep_walk_kernel(const WalkParams P)
                     const int es = (NS == 1) ? 0 : e;
 #pragma unroll
                     for (int j = 0; j < K1; j++) {
-                        double acc = 0.0;
+                        real acc = 0;
 #pragma unroll
                         for (int l = 0; l < K1; l++) acc += A[es][j * K1 + l] * nxt[u][l].v[e];
 #pragma unroll
@@ -177,18 +178,18 @@ cudaError_t dispatch(sldg_ctx* c, const WalkParams& P, int vec, int mode)
 
 }  // namespace
 
-cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,
-                                   const ShiftTable& t)
+cudaError_t SLDG_SFX(sldg_launch_sweep_walk)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g,
+                                             const ShiftTable& t)
 {
     WalkParams P;
-    P.fin = fin; P.fout = fout;
+    P.fin = static_cast<const real*>(fin); P.fout = static_cast<real*>(fout);
     P.inner = g.inner; P.N = g.N;
     P.sdiv = g.sdiv; P.smod = g.smod; P.t = t;
     // Measured on B200: one value per thread (64-bit loads, more threads, more loads in
     // flight) beats 128-bit loads except for x-sweeps of degree >= 2, where the thread count is ample either way.
     int vec = (g.mode == 0 && g.K1 >= 3) ? 2 : 1;
     if (c->opt_walk_vec) vec = c->opt_walk_vec;
-    if ((g.inner & 1) || (((uintptr_t)fin | (uintptr_t)fout) & 15)) vec = 1;
+    if ((g.inner & 1) || (((uintptr_t)fin | (uintptr_t)fout) & (2 * sizeof(real) - 1))) vec = 1;
     P.innerV = g.inner / vec;
     P.nwork = P.innerV * g.outer;
     if (P.nwork == 0) return cudaSuccess;
