@@ -43,9 +43,12 @@ def sweeps_per_step(cfg):
     return 3 * cfg["dim_x"]
 
 
+ESIZE = 8                         # bytes per value of f; --dtype f32 (single precision mode) sets 4
+
+
 def sweep_bytes(cfg):
     import workloads as W
-    return 2 * W.field_elems(cfg) * 8
+    return 2 * W.field_elems(cfg) * ESIZE
 
 
 # ----------------------------------------------------------------------------- clocks
@@ -139,11 +142,14 @@ def time_oracle(cfg, steps, warmup, budget_s=25.0):
     cores = O.lib().orc_max_threads()
     o = O.Oracle(s["dim_x"], s["dim_v"], s["cells"], s["degree"], s["domain"], threads=cores)
     f = W.initial_data(s, [o.node_coords(a) for a in range(o.d)]).numpy()
+    ostep = o.step
+    if ESIZE == 4:                        # single precision mode: the oracle's fp32 functions
+        f, ostep = f.astype("float32"), o.step_f32
     for _ in range(max(0, warmup)):
-        f, _, _ = o.step(f, s["dt"])
+        f, _, _ = ostep(f, s["dt"])
     done, t0 = 0, time.perf_counter()
     while done < steps:
-        f, _, _ = o.step(f, s["dt"])
+        f, _, _ = ostep(f, s["dt"])
         done += 1
         if time.perf_counter() - t0 > budget_s:
             break
@@ -163,7 +169,7 @@ def run_reference(args, cfg, rank, world):
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": r["steps"], "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": cfg["name"], "note": "CPU oracle on a bounded sample; " + r["sample"]},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -198,10 +204,17 @@ def run_ours(args, cfg, rank, world, local):
                          "to time the CPU oracle)")
     dev = torch.device("cuda", local)
     torch.cuda.set_device(dev)
-    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], device=dev)
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], device=dev, precision=args.dtype)
     coords = [g.node_coords(a) for a in range(g.d)]
     f = g.empty_field()
-    W.initial_data(cfg, coords, device=dev, out=f)
+    if args.dtype == "f32":               # the generator works in fp64: fill slab by slab along the slowest axis
+        D = f.shape[0]
+        step = max(1, D // 8)
+        for a in range(0, D, step):
+            b = min(D, a + step)
+            f[a:b].copy_(W.initial_data(cfg, coords[:-1] + [coords[-1][a:b]], device=dev))
+    else:
+        W.initial_data(cfg, coords, device=dev, out=f)
     if args.poisson == "cg":
         g.set_poisson_solver(1, tol=1e-3)
     dt = cfg["dt"]
@@ -256,10 +269,10 @@ def run_ours(args, cfg, rank, world, local):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
         "data": "synthetic",
-        "config": {"workload": cfg["name"], "values": nf, "bytes_f": nf * 8, "sweeps_per_step": nsweeps,
-                   "dt": dt, "poisson": args.poisson, "l2": "inputs larger than L2 (no flush needed)" if nf * 8 > 2 * 126e6 else
+        "config": {"workload": cfg["name"], "values": nf, "bytes_f": nf * ESIZE, "sweeps_per_step": nsweeps,
+                   "dt": dt, "poisson": args.poisson, "l2": "inputs larger than L2 (no flush needed)" if nf * ESIZE > 2 * 126e6 else
                    "array fits in L2: numbers are L2-resident, launch-bound",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "pct_of_measured_peak": 100 * value / world / peak, "pct_of_nominal_8TBs": 100 * value / world / NOMINAL_HBM_GBS,
@@ -269,7 +282,7 @@ def run_ours(args, cfg, rank, world, local):
     # end to end through the C-ABI with HOST buffers (sldg_step_host): H2D of f, one Strang step, D2H of f, per step
     if rank == 0 or world > 1:
         try:
-            fh = torch.empty(g.shape, dtype=torch.float64, pin_memory=True)
+            fh = torch.empty(g.shape, dtype=f.dtype, pin_memory=True)
             fh.copy_(f)
             nrep = max(1, min(args.steps, 3))
             g.step_host(fh, f, dt, nsteps=1)                    # warm-up
@@ -280,8 +293,8 @@ def run_ours(args, cfg, rank, world, local):
             torch.cuda.synchronize(dev)
             e2e_ms_local = 1e3 * (time.perf_counter() - t0)
             e2e_ms, e2e_bytes = aggregate(e2e_ms_local, bytes_step * nrep, device=dev)
-            line["e2e"] = {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": nf * 8,
-                           "d2h_bytes_per_step": nf * 8, "ms_per_step": e2e_ms / nrep, "steps": nrep,
+            line["e2e"] = {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": nf * ESIZE,
+                           "d2h_bytes_per_step": nf * ESIZE, "ms_per_step": e2e_ms / nrep, "steps": nrep,
                            "api": "sldg_step_host (pinned host f -> device, 1 Strang step, device -> host)"}
             del fh
         except Exception as ex:                                  # e.g. not enough pinned host memory
@@ -305,10 +318,14 @@ def main():
     ap.add_argument("--cfl", type=float, default=None, help="choose dt so that the largest x shift is CFL cells (PAPER.md:351)")
     ap.add_argument("--poisson", default="fft", choices=["fft", "cg"], help="field solver inside the step: the FFT "
                     "route (default) or the CGdG solver with the paper's tolerance 1e-3 and warm start (PAPER.md:496-567)")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="f32: single precision mode (PAPER.md:191); "
+                    "the metric then counts 2*|f|*4 B per sweep")
     ap.add_argument("--cells", type=str, default=None, help="override cells, e.g. 16,16,16,16 (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     import workloads as W
+    global ESIZE
+    ESIZE = 4 if args.dtype == "f32" else 8
     cfg = W.CONFIGS[args.config]
     if args.workload:
         cfg = {c["name"]: c for c in W.CONFIGS + W.NEXT_CONFIGS}[args.workload]

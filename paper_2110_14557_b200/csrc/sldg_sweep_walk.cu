@@ -187,7 +187,13 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_walk)(sldg_ctx* c, const void* fin, void*
     P.sdiv = g.sdiv; P.smod = g.smod; P.t = t;
     // Measured on B200: one value per thread (64-bit loads, more threads, more loads in
     // flight) beats 128-bit loads except for x-sweeps of degree >= 2, where the thread count is ample either way.
+#ifdef SLDG_REAL_FLOAT
+    // fp32 (measured on cfg2 / cfg4): 64-bit loads win on every slow axis except the FIRST velocity axis
+    // (inner == X, one shift entry per value), where one value per thread is 1.5x faster.
+    int vec = (g.mode == 1 && g.inner == g.smod) ? 1 : 2;
+#else
     int vec = (g.mode == 0 && g.K1 >= 3) ? 2 : 1;
+#endif
     if (c->opt_walk_vec) vec = c->opt_walk_vec;
     if ((g.inner & 1) || (((uintptr_t)fin | (uintptr_t)fout) & (2 * sizeof(real) - 1))) vec = 1;
     P.innerV = g.inner / vec;
