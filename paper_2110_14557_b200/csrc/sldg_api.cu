@@ -120,6 +120,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     c->stream = 0; c->last_cuda = 0; c->sm_count = 148;
     c->ws = nullptr; c->ws_bytes = 0; c->ws_ready = false;
     c->timing = false; c->launches = 0;
+    c->graph_exec = nullptr; c->graph_f = nullptr; c->graph_dt = 0.0; c->graph_launches = 0; c->opt_graph = 1;
     c->phi = nullptr; c->cg_info = nullptr; c->poisson_solver = 0; c->cg_tol = 1e-3; c->cg_sigma = sldg_sipg_sigma_default(degree);
     c->cg_maxiter = 0;
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
@@ -191,6 +192,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
 extern "C" int sldg_destroy(sldg_ctx* c)
 {
     if (!c) return SLDG_EINVAL;
+    sldg_graph_drop(c);
     for (int a = 0; a < SLDG_MAX_DIM; a++) {
         if (c->dS[a]) cudaFree(c->dS[a]);
         if (c->dAB[a]) cudaFree(c->dAB[a]);
@@ -216,6 +218,7 @@ extern "C" int sldg_destroy(sldg_ctx* c)
 extern "C" int sldg_set_stream(sldg_ctx* c, void* stream)
 {
     if (!c) return SLDG_EINVAL;
+    sldg_graph_drop(c);
     c->stream = (cudaStream_t)stream;
     return SLDG_OK;
 }
@@ -228,6 +231,7 @@ extern "C" int sldg_set_workspace(sldg_ctx* c, void* dev, size_t bytes)
     if (((uintptr_t)dev) & 255) return SLDG_EINVAL;
     WsLayout L = ws_layout(c);
     if (bytes < L.total) return SLDG_ENOWORKSPACE;
+    sldg_graph_drop(c);
     char* b = (char*)dev;
     c->ws = b; c->ws_bytes = bytes;
     c->f2 = (double*)(b + L.f2); c->vS = (int*)(b + L.vS); c->vAB = (double*)(b + L.vAB);
@@ -399,6 +403,7 @@ static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
                 volatile double vt = v * dt;
                 delta[(size_t)n] = vt / c->h[a];
             }
+            sldg_graph_drop(c);                 // a captured step reads these device tables
             int r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
             if (r) return r;
             bool safe = true;
@@ -585,6 +590,7 @@ extern "C" int sldg_set_poisson_solver(sldg_ctx* c, int solver, double tol, int 
 {
     if (!c || solver < 0 || solver > 1 || !(tol >= 0.0) || maxiter < 0) return SLDG_EINVAL;
     if (solver == 1 && c->k < 1) return SLDG_EINVAL;
+    sldg_graph_drop(c);
     c->poisson_solver = solver; c->cg_tol = tol; c->cg_maxiter = maxiter;
     c->cg_sigma = sigma > 0.0 ? sigma : sldg_sipg_sigma_default(c->k);
     return SLDG_OK;
@@ -621,10 +627,9 @@ extern "C" int sldg_sipg_matrices(int degree, double sigma, double* hostM, doubl
     return SLDG_OK;
 }
 
-extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
+static int step_enqueue(sldg_ctx* c, double* f, double dt)
 {
-    int r = check_f(c, f);
-    if (r) return r;
+    int r;
     double *cur = f, *oth = c->f2;
     // The dx v-sweeps flip the buffer pair dx times; the two x half steps choose their flip parities (p1, p2) so
     // that the step ends in f with no device copy, at the fewest passes over f.
@@ -642,6 +647,53 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
     if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;
     if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f))) return r;       // ... ends in f
     if (cur != f) return copy_back(c, f, cur);                                  // unreachable by construction
+    return SLDG_OK;
+}
+
+void sldg_graph_drop(sldg_ctx* c)
+{
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+}
+
+// Small problems (BASELINE config 1: 2 MB) are launch-latency bound: the ~16 launches of a Strang step are
+// captured once into a CUDA graph and replayed.  The graph is keyed on (f, dt) and
+// dropped whenever an option, the stream, the workspace or the solver changes.  Not used with timing on (events
+// cannot be recorded inside a capture) or with the CG solver (cooperative launch).
+extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    const bool small = (size_t)c->nf * c->esize <= ((size_t)256 << 20);
+    const bool use_graph = !c->timing && c->poisson_solver == 0 && (c->opt_graph == 2 || (c->opt_graph == 1 && small));
+    if (!use_graph) return step_enqueue(c, f, dt);
+    if (c->graph_exec && c->graph_f == f && c->graph_dt == dt) {
+        CK(cudaGraphLaunch(c->graph_exec, c->stream));
+        c->launches += c->graph_launches;
+        return SLDG_OK;
+    }
+    sldg_graph_drop(c);
+    ShiftTable tabs[3];
+    if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;       // host tables + upload (synchronises): before the capture
+    const long long l0 = c->launches;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return step_enqueue(c, f, dt);
+    }
+    r = step_enqueue(c, f, dt);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    if (r || e != cudaSuccess || !g) {
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        c->launches = l0;
+        if (r) return r;
+        return step_enqueue(c, f, dt);                          // capture not possible: plain launches
+    }
+    e = cudaGraphInstantiate(&c->graph_exec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { c->graph_exec = nullptr; cudaGetLastError(); c->launches = l0; return step_enqueue(c, f, dt); }
+    c->graph_f = f; c->graph_dt = dt; c->graph_launches = c->launches - l0;
+    CK(cudaGraphLaunch(c->graph_exec, c->stream));
     return SLDG_OK;
 }
 
@@ -823,6 +875,8 @@ extern "C" long long sldg_launch_count(const sldg_ctx* c) { return c ? c->launch
 extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
 {
     if (!c || !name) return SLDG_EINVAL;
+    sldg_graph_drop(c);
+    if (!strcmp(name, "graph")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_graph = (int)value; return SLDG_OK; }
     if (!strcmp(name, "tile_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_tile_bytes = (int)value; return SLDG_OK; }
     if (!strcmp(name, "axis0_impl")) { if (value < 0 || value > 3) return SLDG_EINVAL; c->opt_axis0_impl = (int)value; return SLDG_OK; }
     if (!strcmp(name, "tile_stages")) { if (value < 1 || value > 4) return SLDG_EINVAL; c->opt_tile_stages = (int)value; return SLDG_OK; }

@@ -119,6 +119,10 @@ struct sldg_ctx {
     long long t_launch[SLDG_NKINDS]; double t_ms[SLDG_NKINDS];
     long long a_launch[SLDG_MAX_DIM]; double a_ms[SLDG_MAX_DIM];
 
+    // CUDA graph of one Strang step (small problems)
+    cudaGraphExec_t graph_exec; const double* graph_f; double graph_dt; long long graph_launches;
+    int opt_graph;                  // 0 = never, 1 = problems up to 256 MB (default), 2 = always
+
     // tuning
     int opt_tile_bytes;             // axis-0 kernels: bytes per chunk (per warp) / per tile (block-wide kernel)
     int opt_tile_stages;            // axis-0 line kernel: input ring depth per warp (1..4)
@@ -178,6 +182,7 @@ void sldg_sipg_tables(int k, const double* xi, const double* w, double sigma, do
 cudaError_t sldg_launch_energy(sldg_ctx* c, const double* E, double* out1);
 cudaError_t sldg_launch_mass(sldg_ctx* c, const double* f, double* out1);
 
+void sldg_graph_drop(sldg_ctx* c);          // forget the captured Strang-step graph (any state change)
 // instrumentation helpers (sldg_api.cu)
 void sldg_ev_begin(sldg_ctx* c, int kind, int axis);
 void sldg_ev_end(sldg_ctx* c);

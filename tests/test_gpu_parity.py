@@ -342,3 +342,33 @@ def test_step_plans_agree_bitwise(P, cfg):
         outs.append(fg.cpu().numpy())
     for x in outs[1:]:
         assert np.array_equal(outs[0], x)
+
+
+# --------------------------------------------------------------- CUDA graph replay of the Strang step
+
+@pytest.mark.parametrize("cfg", [small_cfgs()[0], small_cfgs()[3]], ids=lambda c: c["name"])
+def test_graph_replay_of_the_step_is_bitwise_the_plain_step(P, cfg):
+    """Small problems replay a captured CUDA graph (launch-latency bound): same kernels,
+    same order, same bits; the graph is rebuilt when dt changes or when another call rewrites the x-sweep tables."""
+    g, o = pair_of_cfg(P, cfg)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    dt = cfg["dt"]
+    seq = [dt, dt, dt, 0.5 * dt, 0.5 * dt, dt]
+    outs = []
+    for graph in (0, 2, 1):
+        g.set_option("graph", graph)
+        fg = f0.to(g.device).contiguous()
+        n0 = g.launch_count()
+        for i, h in enumerate(seq):
+            g.step(fg, h)
+            if i == 1:
+                g.advect_x(fg, 0.3 * dt)            # rewrites the cached x tables: the graph must not survive
+        outs.append((fg.cpu().numpy(), g.launch_count() - n0))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][0], outs[2][0])
+    assert outs[0][1] == outs[1][1] == outs[2][1]                 # replays count the launches they contain
+    fo = f0.numpy()
+    for i, h in enumerate(seq):
+        fo, _, _ = o.step(fo, h)
+        if i == 1:
+            fo = o.advect_x(fo, 0.3 * dt)
+    assert rel_inf(outs[0][0], fo) <= TOL_STEPS
