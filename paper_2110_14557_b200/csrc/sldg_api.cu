@@ -126,7 +126,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
-    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
+    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 2; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
@@ -421,7 +421,7 @@ static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
 
 // Plan of one x advection: x_1 and x_2 in one fused pass or separately, which sweeps run in place, such that the
 // number of buffer flips has the requested parity.  Fewest passes over f wins; ties go to fewer in-place walks.
-struct XPlan { bool ok, fused, x1_oop; bool inplace[3]; int passes, flips; };
+struct XPlan { bool ok, fused, fused3, x1_oop; bool inplace[3]; int passes, flips; };
 
 static bool fused_possible(const sldg_ctx* c)
 {
@@ -432,10 +432,29 @@ static bool fused_possible(const sldg_ctx* c)
     return c->D[0] <= c->opt_fused_threads;
 }
 
+// the shape rules of sldg_launch_sweep_fused3 (sldg_sweep_fused3.cu), so that a plan never meets NotSupported
+static bool fused3_possible(const sldg_ctx* c)
+{
+    if (!c->opt_fuse3 || !c->opt_fuse_x || c->dx != 3 || c->K1 > 2 || c->cells[0] > 256) return false;
+    const long long cellb = (long long)c->K1 * c->D[0] * (long long)c->esize;
+    if (cellb & 15) return false;
+    long long S = c->opt_f3_threads / c->cells[0];
+    if (S < 1) S = 1;
+    if (S > c->cells[1]) S = c->cells[1];
+    const long long nstrips = (c->cells[1] + S - 1) / S;
+    S = (c->cells[1] + nstrips - 1) / nstrips;
+    return (size_t)c->K1 * (2 * (S + 1) + 2 * S) * cellb + 64 <= 227 * 1024;
+}
+
 static XPlan x_plan(const sldg_ctx* c, bool flip)
 {
-    XPlan best; best.ok = false; best.passes = 1 << 30; best.flips = 0;
+    XPlan best; best.ok = false; best.fused3 = false; best.passes = 1 << 30; best.flips = 0;
     const int dx = c->dx;
+    if (flip && fused3_possible(c)) {       // all three sweeps in one out-of-place pass: one flip
+        best.ok = true; best.fused3 = true; best.fused = false; best.x1_oop = true; best.passes = 1; best.flips = 1;
+        for (int i = 0; i < 3; i++) best.inplace[i] = false;
+        return best;
+    }
     for (int fused = fused_possible(c) ? 1 : 0; fused >= 0; fused--) {
         const int first_slow = fused ? 2 : 1;
         const int nslow = dx > first_slow ? dx - first_slow : 0;
@@ -471,6 +490,17 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     XPlan p = x_plan(c, flip);
     if (!p.ok) return SLDG_EINVAL;          // cannot happen: the unfused plan reaches either parity
     int a = 0;
+    if (p.fused3) {
+        SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
+        sldg_ev_begin(c, KIND_FUSED, 0);
+        cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3_f32(c, *cur, *oth, g3, tabs)
+                                            : sldg_launch_sweep_fused3_f64(c, *cur, *oth, g3, tabs);
+        sldg_ev_end(c);
+        c->launches++;
+        if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+        double* t = *cur; *cur = *oth; *oth = t;
+        return SLDG_OK;
+    }
     if (p.fused) {
         sldg_ev_begin(c, KIND_FUSED, 0);
         cudaError_t e = cudaErrorNotSupported;
@@ -884,6 +914,9 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "fuse_x")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse_x = (int)value; return SLDG_OK; }
     if (!strcmp(name, "inplace_walk")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_inplace_walk = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fused_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_fused_threads = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fuse3")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse3 = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "f3_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_f3_threads = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "f3_stages")) { if (value < 2 || value > 4) return SLDG_EINVAL; c->opt_f3_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "x_copy")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_copy = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fused_impl")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fused_impl = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_threads")) { if (value < 1 || value > 128) return SLDG_EINVAL; c->opt_cell_threads = (int)value; return SLDG_OK; }

@@ -133,6 +133,9 @@ struct sldg_ctx {
     int opt_fused_threads;          // fused kernel: threads per block (<= 256) = planes per block * D_0
     int opt_inplace_walk;           // 1: slow-axis x sweeps may run in place when their table allows
     int opt_fused_impl;             // 0 = auto (cell kernel, else node kernel), 1 = cell-per-thread TMA kernel, 2 = node-per-thread kernel
+    int opt_fuse3;                  // 1: x_1, x_2 and x_3 sweeps in one pass (dim_x = 3, degree <= 1)
+    int opt_f3_threads;             // fused3 kernel: threads per block (<= 256) = N_0 * strip cells
+    int opt_f3_stages;              // fused3 kernel: input stages (2..4)
     int opt_x_copy;                 // 1: sldg_advect_x runs the plan that ends in the workspace, then copies back (tests)
     int opt_cell_threads;           // fused cell kernel: threads per block (<= 128) = planes per block * N_0
     int opt_cell_rows;              // fused cell kernel: x_2 cells per chunk (0 = from opt_cell_bytes)
@@ -159,6 +162,8 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
                                             const ShiftTable& t);                                                   \
     cudaError_t sldg_launch_sweep_fused_cell##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,    \
                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
+cudaError_t sldg_launch_sweep_fused3_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t);
+cudaError_t sldg_launch_sweep_fused3_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t);
 SLDG_DECL_SWEEPS(_f64)
 SLDG_DECL_SWEEPS(_f32)
 cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,

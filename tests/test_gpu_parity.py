@@ -372,3 +372,64 @@ def test_graph_replay_of_the_step_is_bitwise_the_plain_step(P, cfg):
         if i == 1:
             fo = o.advect_x(fo, 0.3 * dt)
     assert rel_inf(outs[0][0], fo) <= TOL_STEPS
+
+
+# --------------------------------------------------------------- fused x1+x2+x3 pass (dim_x = 3, degree <= 1)
+
+F3_GEOMS = [
+    (3, 3, [4, 3, 5, 3, 4, 2], 1),
+    (3, 3, [20, 7, 3, 2, 2, 2], 1),    # D_0 = 40 as in BASELINE cfg4; 7 x_2 cells: ragged strips
+    (3, 3, [6, 5, 1, 2, 3, 2], 1),     # a single x_3 cell: the wrap cell is the only donor pair
+    (3, 3, [4, 1, 3, 2, 2, 3], 1),     # a single x_2 cell: halo = the cell itself
+    (3, 3, [8, 6, 4, 2, 3, 2], 0),     # degree 0 (D_0 = 8: bulk-copy rule holds)
+    (3, 3, [5, 4, 3, 2, 2, 2], 0),     # degree 0, D_0 = 5: rows not a multiple of 16 B -> planner falls back
+]
+
+
+@pytest.mark.parametrize("geom", F3_GEOMS, ids=lambda g: f"{'x'.join(map(str, g[2]))}-k{g[3]}")
+@pytest.mark.parametrize("tau", [0.013, 0.4, 7.7])
+def test_fused3_pass_agrees_bitwise_with_separate_sweeps_and_matches_oracle(P, geom, tau):
+    dx, dv, cells, k = geom
+    g, o = make_pair(P, dx, dv, cells, k)
+    f0 = W.random_field(o.shape, seed=31 + k)
+    outs = []
+    # (fuse3, fuse_x, x_copy, f3_threads, f3_stages)
+    for fuse3, fuse, xcopy, thr, st in ((0, 0, 0, 128, 2), (0, 1, 0, 128, 2), (1, 1, 1, 128, 2), (1, 1, 1, 256, 3),
+                                        (1, 1, 1, 24, 4), (1, 1, 1, 1, 2)):
+        g.set_option("fuse3", fuse3); g.set_option("fuse_x", fuse); g.set_option("x_copy", xcopy)
+        g.set_option("f3_threads", thr); g.set_option("f3_stages", st)
+        fg = f0.to(g.device).contiguous()
+        g.advect_x(fg, tau)
+        outs.append(fg.cpu().numpy())
+    for x in outs[1:]:
+        assert np.array_equal(outs[0], x)
+    assert rel_inf(outs[0], o.advect_x(f0.numpy(), tau)) <= TOL_SWEEP * dx
+
+
+def test_fused3_integer_shifts_are_exact(P):
+    dom = [0, 1.0, 0, 1.5, 0, 0.5, -4.0, 4.0, -4.0, 4.0, -4.0, 4.0]
+    g, o = make_pair(P, 3, 3, [4, 6, 2, 8, 8, 8], 0, dom)          # h_x = 0.25; v nodes -3.5..3.5; tau 0.5 -> delta = 2 v
+    f0 = W.random_field(o.shape, seed=4)
+    f0.view(-1)[::5] = -0.0
+    want = o.advect_x(f0.numpy(), 0.5)
+    for fuse3 in (1, 0):
+        g.set_option("fuse3", fuse3); g.set_option("x_copy", 1)
+        fg = f0.to(g.device).contiguous()
+        g.advect_x(fg, 0.5)
+        assert np.array_equal(fg.cpu().numpy().view(np.int64), want.view(np.int64))
+
+
+@pytest.mark.parametrize("cfg", small_cfgs()[3:], ids=lambda c: c["name"])
+def test_step_with_and_without_fused3_agree_bitwise(P, cfg):
+    g, o = pair_of_cfg(P, cfg)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    outs = []
+    for fuse3 in (1, 0):
+        g.set_option("fuse3", fuse3)
+        fg = f0.to(g.device).contiguous()
+        n0 = g.launch_count()
+        for _ in range(3):
+            g.step(fg, cfg["dt"])
+        outs.append((fg.cpu().numpy(), g.launch_count() - n0))
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert outs[0][1] < outs[1][1]                                  # the fused plan really ran (fewer launches)
