@@ -134,6 +134,11 @@ const double* sldg_last_phi(const sldg_ctx* ctx);
  * B u_{i-1} + B^T u_{i+1}; sigma <= 0: default.  Host-only, needs no context or device. */
 int sldg_sipg_matrices(int degree, double sigma, double* hostM, double* hostB);
 
+/* nsteps Strang steps; the result is in f and equals nsteps calls of sldg_step bit for bit.  Consecutive
+ * steps may keep their intermediate result in the workspace buffer, which lets every x half step of a
+ * dim_x = 3 problem run as ONE fused pass (a single sldg_step needs one two-pass x half step to end in f). */
+int sldg_steps(sldg_ctx* ctx, double* f, double dt, int nsteps);
+
 /* Same path driven from HOST memory: copies f_host (|f| doubles, pinned memory recommended) to
  * the device buffer f_dev, runs nsteps Strang steps, copies the result back into f_host and the
  * last E ([dim_x][X]) into E_host if it is not NULL.  Synchronises. */
@@ -172,8 +177,8 @@ int sldg_advect_axis(sldg_ctx* ctx, double* f, int axis, const double* delta_hos
 /* ---- instrumentation --------------------------------------------------------------------
  * With timing on, every kernel launch is bracketed by CUDA events on the context's stream.
  * Kinds: 0 = sweep along axis 0 (TMA/SMEM kernel), 1 = sweep along a slow axis, 2 = rho,
- * 3 = Poisson/E, 4 = shift tables, 5 = copies, 6 = fused x_1+x_2 pass (two sweeps in one launch; the
- * per-axis figures of sldg_timing_axis book half of its time on each of the two axes).  sldg_timing_read synchronises, adds the elapsed
+ * 3 = Poisson/E, 4 = shift tables, 5 = copies, 6 = fused x pass (x_1+x_2, or x_1+x_2+x_3 for dim_x = 3, in one launch;
+ * the per-axis figures of sldg_timing_axis book an equal share of its time on each fused axis).  sldg_timing_read synchronises, adds the elapsed
  * times of all events recorded since the last read, and returns per kind the number of launches
  * and the total milliseconds (arrays of SLDG_NKINDS entries, host). */
 #define SLDG_NKINDS 7

@@ -11,7 +11,7 @@ _LIBNAME = "libsldg_b200.so"
 
 NKINDS = 7
 MAX_DIM = 6
-KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x1x2"]
+KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x"]
 
 _vp, _dp, _ip, _ll = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_longlong
 _llp = C.POINTER(C.c_longlong)
@@ -30,6 +30,7 @@ EXPORTS = {
     "sldg_density": (C.c_int, [_vp, _vp, _vp]),
     "sldg_poisson": (C.c_int, [_vp, _vp, _vp]),
     "sldg_step": (C.c_int, [_vp, _vp, C.c_double]),
+    "sldg_steps": (C.c_int, [_vp, _vp, C.c_double, C.c_int]),
     "sldg_step_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int]),
     "sldg_field_elems": (_ll, [_vp]),
     "sldg_rho_elems": (_ll, [_vp]),
@@ -235,6 +236,9 @@ class Sldg:
 
     def step(self, f, dt):
         _check(lib().sldg_step(self._h, self._fp(f), float(dt)), self._h)
+
+    def steps(self, f, dt, nsteps):
+        _check(lib().sldg_steps(self._h, self._fp(f), float(dt), int(nsteps)), self._h)
 
     def step_host(self, f_host, f_dev, dt, nsteps=1, E_host=None):
         _check(lib().sldg_step_host(self._h, self._fp(f_host), self._fp(f_dev),

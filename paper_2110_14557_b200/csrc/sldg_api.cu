@@ -492,7 +492,7 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     int a = 0;
     if (p.fused3) {
         SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
-        sldg_ev_begin(c, KIND_FUSED, 0);
+        sldg_ev_begin(c, KIND_FUSED, 3);                       // axis field of a fused event = number of fused axes
         cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3_f32(c, *cur, *oth, g3, tabs)
                                             : sldg_launch_sweep_fused3_f64(c, *cur, *oth, g3, tabs);
         sldg_ev_end(c);
@@ -657,25 +657,44 @@ extern "C" int sldg_sipg_matrices(int degree, double sigma, double* hostM, doubl
     return SLDG_OK;
 }
 
-static int step_enqueue(sldg_ctx* c, double* f, double dt)
+// passes over f of one Strang step whose total number of buffer flips has parity `flip_total`; *p1 = flip parity of
+// the first x half step that achieves it
+static int step_cost(const sldg_ctx* c, bool flip_total, int* p1)
+{
+    int best = 1 << 30;
+    for (int q1 = 0; q1 < 2; q1++) {
+        const int q2 = (q1 + c->dx + (flip_total ? 1 : 0)) & 1;
+        XPlan a = x_plan(c, q1 != 0), b = x_plan(c, q2 != 0);
+        if (a.ok && b.ok && a.passes + b.passes < best) { best = a.passes + b.passes; if (p1) *p1 = q1; }
+    }
+    return best;
+}
+
+// One Strang step on the pair (*cur, *oth).  The dx v-sweeps flip the pair dx times; the two x half steps choose
+// their flip parities so that the step ends in the buffer it started in (flip_total = false: no device copy for
+// the caller's f) or in the other one (flip_total = true: sldg_steps alternates), at the fewest passes over f.
+static int step_core(sldg_ctx* c, double** cur, double** oth, double dt, bool flip_total)
 {
     int r;
-    double *cur = f, *oth = c->f2;
-    // The dx v-sweeps flip the buffer pair dx times; the two x half steps choose their flip parities (p1, p2) so
-    // that the step ends in f with no device copy, at the fewest passes over f.
+    double* const start = *cur;
     ShiftTable tabs[3];
     if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;
-    int best = 1 << 30, p1 = 0;
-    for (int q1 = 0; q1 < 2; q1++) {
-        const int q2 = (q1 + c->dx) & 1;
-        XPlan a = x_plan(c, q1 != 0), b = x_plan(c, q2 != 0);
-        if (a.ok && b.ok && a.passes + b.passes < best) { best = a.passes + b.passes; p1 = q1; }
-    }
-    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, p1 != 0))) return r;
-    if ((r = sldg_density(c, cur, c->rho))) return r;
+    int p1 = 0;
+    step_cost(c, flip_total, &p1);
+    if ((r = advect_x_impl(c, cur, oth, dt / 2.0, p1 != 0))) return r;
+    if ((r = sldg_density(c, *cur, c->rho))) return r;
     if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
-    if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;
-    if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f))) return r;       // ... ends in f
+    if ((r = advect_v_impl(c, cur, oth, c->E, dt))) return r;
+    const bool want_other = flip_total;                       // where the step has to end, relative to `start`
+    const bool now_other = (*cur != start);
+    return advect_x_impl(c, cur, oth, dt / 2.0, now_other != want_other);
+}
+
+static int step_enqueue(sldg_ctx* c, double* f, double dt)
+{
+    double *cur = f, *oth = c->f2;
+    int r = step_core(c, &cur, &oth, dt, false);
+    if (r) return r;
     if (cur != f) return copy_back(c, f, cur);                                  // unreachable by construction
     return SLDG_OK;
 }
@@ -727,14 +746,40 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
     return SLDG_OK;
 }
 
+// nsteps Strang steps.  Consecutive steps may leave their result in alternate buffers when that saves passes (for
+// dim_x = 3 both x half steps of a step can then be the one-pass fused x_1+x_2+x_3 sweep); the last step restores
+// the parity, so the result is in f.  Same arithmetic as nsteps calls of sldg_step, bit for bit.
+extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
+{
+    int r = check_f(c, f);
+    if (r) return r;
+    if (nsteps < 0) return SLDG_EINVAL;
+    const bool small = (size_t)c->nf * c->esize <= ((size_t)256 << 20);
+    if (!c->timing && c->poisson_solver == 0 && (c->opt_graph == 2 || (c->opt_graph == 1 && small))) {
+        for (int s = 0; s < nsteps; s++)
+            if ((r = sldg_step(c, f, dt))) return r;            // small problems: graph replay per step
+        return SLDG_OK;
+    }
+    ShiftTable tabs[3];
+    if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;      // fills tab_safe, which the plans depend on
+    double *cur = f, *oth = c->f2;
+    for (int s = 0; s < nsteps; s++) {
+        bool flip;
+        if (s == nsteps - 1) flip = (cur != f);                 // the last step ends in f
+        else flip = step_cost(c, true, nullptr) < step_cost(c, false, nullptr);
+        if ((r = step_core(c, &cur, &oth, dt, flip))) return r;
+    }
+    if (cur != f) return copy_back(c, f, cur);                  // unreachable by construction
+    return SLDG_OK;
+}
+
 extern "C" int sldg_step_host(sldg_ctx* c, double* f_host, double* f_dev, double* E_host, double dt, int nsteps)
 {
     int r = check_f(c, f_dev);
     if (r) return r;
     if (!f_host || nsteps < 0) return SLDG_EINVAL;
     CK(cudaMemcpyAsync(f_dev, f_host, (size_t)c->nf * c->esize, cudaMemcpyHostToDevice, c->stream));
-    for (int s = 0; s < nsteps; s++)
-        if ((r = sldg_step(c, f_dev, dt))) return r;
+    if ((r = sldg_steps(c, f_dev, dt, nsteps))) return r;
     CK(cudaMemcpyAsync(f_host, f_dev, (size_t)c->nf * c->esize, cudaMemcpyDeviceToHost, c->stream));
     if (E_host) CK(cudaMemcpyAsync(E_host, c->E, (size_t)c->X * 8 * c->dx, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -886,7 +931,7 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
         if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
             c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
-            if (r.kind == KIND_FUSED) { for (int a = 0; a < 2; a++) { c->a_launch[a]++; c->a_ms[a] += 0.5 * t; } }
+            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2; for (int a = 0; a < nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
         }
         c->ev_free.push_back(r);
     }

@@ -433,3 +433,24 @@ def test_step_with_and_without_fused3_agree_bitwise(P, cfg):
         outs.append((fg.cpu().numpy(), g.launch_count() - n0))
     assert np.array_equal(outs[0][0], outs[1][0])
     assert outs[0][1] < outs[1][1]                                  # the fused plan really ran (fewer launches)
+
+
+@pytest.mark.parametrize("cfg", [small_cfgs()[1], small_cfgs()[3], small_cfgs()[4]], ids=lambda c: c["name"])
+@pytest.mark.parametrize("n", [1, 2, 3, 4])
+def test_steps_equals_repeated_step_bitwise(P, cfg, n):
+    """sldg_steps may alternate buffers between steps (one-pass x half steps for dim_x = 3): same bits, result in f."""
+    g, o = pair_of_cfg(P, cfg)
+    g.set_option("graph", 0)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    fa, fb = f0.to(g.device).contiguous(), f0.to(g.device).contiguous()
+    n0 = g.launch_count()
+    for _ in range(n):
+        g.step(fa, cfg["dt"])
+    n1 = g.launch_count()
+    g.steps(fb, cfg["dt"], n)
+    n2 = g.launch_count()
+    assert torch.equal(fa, fb)
+    if cfg["dim_x"] == 3 and n >= 2:
+        assert n2 - n1 < n1 - n0                                    # fewer passes
+    else:
+        assert n2 - n1 == n1 - n0
