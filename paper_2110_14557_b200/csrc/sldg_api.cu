@@ -126,8 +126,8 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
-    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 2; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
-    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->dWx[a] = nullptr; }
+    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
+    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
     c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
@@ -406,12 +406,13 @@ static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
             sldg_graph_drop(c);                 // a captured step reads these device tables
             int r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
             if (r) return r;
-            bool safe = true;
+            bool safe = true, anycp = false;
             for (long long n = 0; n < c->D[b]; n++) {
+                if (c->hS[n] & SLDG_COPY_BIT) anycp = true;
                 const int sv = c->hS[n] & SLDG_S_MASK;
                 if (sv != 0 && sv != c->cells[a] - 1) safe = false;
             }
-            c->tab_safe[a] = safe;
+            c->tab_safe[a] = safe; c->tab_anycp[a] = anycp;
             c->tab_valid[a] = true; c->tab_tau[a] = dt;
         }
         tabs[a].S = c->dS[a]; tabs[a].AB = c->dAB[a]; tabs[a].strideIdx = NN2; tabs[a].strideM = 1;
@@ -493,8 +494,9 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     if (p.fused3) {
         SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
         sldg_ev_begin(c, KIND_FUSED, 3);                       // axis field of a fused event = number of fused axes
-        cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3_f32(c, *cur, *oth, g3, tabs)
-                                            : sldg_launch_sweep_fused3_f64(c, *cur, *oth, g3, tabs);
+        const int anycp = (c->tab_anycp[0] || c->tab_anycp[1] || c->tab_anycp[2]) ? 1 : 0;
+        cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3_f32(c, *cur, *oth, g3, tabs, anycp)
+                                            : sldg_launch_sweep_fused3_f64(c, *cur, *oth, g3, tabs, anycp);
         sldg_ev_end(c);
         c->launches++;
         if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }

@@ -85,6 +85,7 @@ struct sldg_ctx {
     double* dAB[SLDG_MAX_DIM];      //                                       [D_{dx+a}][2 K1^2]
     double tab_tau[SLDG_MAX_DIM];   // dt the cached table of x axis a was built for
     bool tab_valid[SLDG_MAX_DIM];
+    bool tab_anycp[SLDG_MAX_DIM];   // some entry of the cached table has alpha == 0 (copy bit)
     bool tab_safe[SLDG_MAX_DIM];    // every shift of the cached table is 0 or -1: a walk may run in place
     int* dS_hook; double* dAB_hook; long long hook_cap;   // test-hook tables (x axes)
     double* dFwdT[3];               // forward transfer+DFT matrices, transposed [n][m], re then im
@@ -162,8 +163,8 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
                                             const ShiftTable& t);                                                   \
     cudaError_t sldg_launch_sweep_fused_cell##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,    \
                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
-cudaError_t sldg_launch_sweep_fused3_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t);
-cudaError_t sldg_launch_sweep_fused3_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t);
+cudaError_t sldg_launch_sweep_fused3_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
+cudaError_t sldg_launch_sweep_fused3_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 SLDG_DECL_SWEEPS(_f64)
 SLDG_DECL_SWEEPS(_f32)
 cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,

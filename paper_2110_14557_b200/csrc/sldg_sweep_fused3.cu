@@ -67,8 +67,11 @@ __device__ __forceinline__ void load_table(const ShiftTable& t, long long idx, r
     }
 }
 
-template <int K1>
-__global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
+// CP = false: no entry of the three tables has alpha == 0 (the host knows), the copy selects are compiled out.
+// The block has one extra warp whose first thread (the PRODUCER) issues every bulk copy, so that no compute warp
+// carries the address arithmetic of the copies or is late at the per-step barrier.
+template <int K1, bool CP>
+__global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
 {
     constexpr int NN = K1 * K1, N3 = K1 * K1 * K1;
     constexpr uint32_t ES = (uint32_t)sizeof(real);
@@ -84,12 +87,14 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
     const uint32_t bars_s = (smem_u32(sout + (size_t)F3_OST * OS) + 7u) & ~7u;
 
     const int t = threadIdx.x;
+    const int NT = S * N0;                                 // compute threads; the producer is thread roundup32(NT)
+    const bool lead = (t == (int)blockDim.x - 32);
     const int e1 = t / N0, i0 = t - e1 * N0;
     const long long q = blockIdx.x / P.nstrips;
     const int strip = (int)(blockIdx.x - q * P.nstrips);
     const int c0 = strip * S;
     const int nS = min(S, N1 - c0);
-    const bool active = e1 < nS;
+    const bool active = t < NT && e1 < nS;
     const long long D1 = (long long)N1 * K1, D2 = (long long)N2 * K1;
     const real* const gin = P.fin + q * D2 * D1 * D0;
     real* const gout = P.fout + q * D2 * D1 * D0;
@@ -108,7 +113,7 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
     const uint32_t cellb = (uint32_t)CELL * ES;
 
     auto issue_load = [&](int j) {                         // x_3 cell j -> stage j % ST
-        if (t == 0 && j < N2) {
+        if (lead && j < N2) {
             const int st = j % ST;
             const uint32_t bar = bars_s + (uint32_t)st * 8u;
             mbar_expect_tx(bar, (uint32_t)(K1 * (nS + 1)) * cellb);
@@ -122,7 +127,7 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
         }
     };
 
-    if (t == 0) {
+    if (lead) {
         for (int st = 0; st < ST; st++) mbar_init(bars_s + (uint32_t)st * 8u, 1);
         mbar_init_fence();
     }
@@ -151,7 +156,7 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
                         for (int m = 0; m < K1; m++) acc += A1[j1 * K1 + m] * a.v[m];
 #pragma unroll
                         for (int m = 0; m < K1; m++) acc += B1[j1 * K1 + m] * b.v[m];
-                        sw[dn][j2 * K1 + j1] = cp1 ? a.v[j1] : acc;
+                        sw[dn][j2 * K1 + j1] = (CP && cp1) ? a.v[j1] : acc;
                     }
                 }
             }
@@ -164,14 +169,16 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
                     for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * sw[0][l * K1 + j1];
 #pragma unroll
                     for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * sw[1][l * K1 + j1];
-                    N[(j3 * K1 + j2) * K1 + j1] = cp2 ? sw[0][j2 * K1 + j1] : acc;
+                    N[(j3 * K1 + j2) * K1 + j1] = (CP && cp2) ? sw[0][j2 * K1 + j1] : acc;
                 }
         }
     };
 
     real first[N3], prev[N3];
-    mbar_wait(bars_s, 0u);                                 // x_3 cell 0
-    if (active) swept12(sin_, first);
+    if (active) {
+        mbar_wait(bars_s, 0u);                             // x_3 cell 0
+        swept12(sin_, first);
+    }
 #pragma unroll
     for (int m = 0; m < N3; m++) prev[m] = first[m];
     __syncthreads();
@@ -183,8 +190,10 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
         const int st = j % ST;
         real nxt[N3];
         if (j < N2) {
-            mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
-            if (active) swept12(sin_ + st * SS, nxt);
+            if (active) {
+                mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
+                swept12(sin_ + st * SS, nxt);
+            }
         } else {
 #pragma unroll
             for (int m = 0; m < N3; m++) nxt[m] = first[m];
@@ -203,7 +212,7 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
                         for (int l = 0; l < K1; l++) acc += A3[j3 * K1 + l] * nxt[(l * K1 + j2) * K1 + j1];
 #pragma unroll
                         for (int l = 0; l < K1; l++) acc += B3[j3 * K1 + l] * prev[(l * K1 + j2) * K1 + j1];
-                        r.v[j1] = cp3 ? nxt[(j3 * K1 + j2) * K1 + j1] : acc;
+                        r.v[j1] = (CP && cp3) ? nxt[(j3 * K1 + j2) * K1 + j1] : acc;
                     }
                     r.store(obase + j3 * OP + j2 * D0);
                 }
@@ -211,9 +220,9 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
 #pragma unroll
         for (int m = 0; m < N3; m++) prev[m] = nxt[m];
         fence_async_smem();
-        if (t == 0) bulk_wait_read<0>();                   // the stores of step h-1 have left their output stage
+        if (lead) bulk_wait_read<0>();                     // the stores of step h-1 have left their output stage
         __syncthreads();
-        if (t == 0) {
+        if (lead) {
 #pragma unroll
             for (int j3 = 0; j3 < K1; j3++)
                 bulk_store(gout + (((long long)(io3 * K1 + j3)) * D1 + (long long)c0 * K1) * D0,
@@ -223,18 +232,18 @@ __global__ void __launch_bounds__(256) sweep_fused3_kernel(const F3Params P)
         issue_load(j + ST);
         io3++; if (io3 >= N2) io3 = 0;
     }
-    if (t == 0) bulk_wait_read<0>();
+    if (lead) bulk_wait_read<0>();
 }
 
-template <int K1>
+template <int K1, bool CP>
 cudaError_t launch(sldg_ctx* c, const F3Params& P, int threads, size_t smem)
 {
-    auto kern = sweep_fused3_kernel<K1>;
+    auto kern = sweep_fused3_kernel<K1, CP>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long grid = P.cubes * P.nstrips;
     if (grid > 0x7fffffffLL) return cudaErrorNotSupported;
-    kern<<<(unsigned)grid, threads, smem, c->stream>>>(P);
+    kern<<<(unsigned)grid, ((threads + 31) & ~31) + 32, smem, c->stream>>>(P);
     return cudaGetLastError();
 }
 
@@ -243,7 +252,7 @@ cudaError_t launch(sldg_ctx* c, const F3Params& P, int threads, size_t smem)
 // g0, g1, g2: geometry of axes 0, 1, 2.  cudaErrorNotSupported when the shape does not fit (the caller plans the
 // fused x_1+x_2 pass plus a separate x_3 sweep instead).
 cudaError_t SLDG_SFX(sldg_launch_sweep_fused3)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g,
-                                               const ShiftTable* t)
+                                               const ShiftTable* t, int any_copy)
 {
     if (g[2].outer == 0) return cudaSuccess;
     const int K1 = g[0].K1;
@@ -272,5 +281,6 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fused3)(sldg_ctx* c, const void* fin, voi
     for (int a = 0; a < 3; a++) { P.smod[a] = g[a].smod; P.t[a] = t[a]; }
     const int threads = (int)(S * g[0].N);
     const size_t smem = smem_of(S, stages);
-    return K1 == 1 ? launch<1>(c, P, threads, smem) : launch<2>(c, P, threads, smem);
+    if (any_copy) return K1 == 1 ? launch<1, true>(c, P, threads, smem) : launch<2, true>(c, P, threads, smem);
+    return K1 == 1 ? launch<1, false>(c, P, threads, smem) : launch<2, false>(c, P, threads, smem);
 }

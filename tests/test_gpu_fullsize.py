@@ -73,8 +73,12 @@ def full(request, P):
     torch.cuda.empty_cache()
 
 
-def test_advect_x_on_full_x_space_of_sampled_velocity_cells(full):
+@pytest.mark.parametrize("xcopy", [0, 1], ids=["even-parity plan", "odd-parity plan (the one-pass fused sweeps)"])
+def test_advect_x_on_full_x_space_of_sampled_velocity_cells(full, xcopy):
+    """x_copy = 1 runs the plan sldg_step / sldg_steps use for their flipping x half steps: the fused x1+x2 pass
+    (dim_x = 2) or the fused x1+x2+x3 pass (dim_x = 3), in the launch configuration bench.py times."""
     cfg, g, f = full
+    g.set_option("x_copy", xcopy)
     dx, dv = cfg["dim_x"], cfg["dim_v"]
     vaxes = list(range(dx, dx + dv))
     cells = cell_samples(cfg["cells"][dx:], 5, seed=1)
@@ -91,6 +95,7 @@ def test_advect_x_on_full_x_space_of_sampled_velocity_cells(full):
         want = o.advect_x(b, tau)
         got = f[slab_index(g, vaxes, c)].cpu().numpy()
         assert rel_inf(got, want) <= TOL * dx, (c, rel_inf(got, want))
+    g.set_option("x_copy", 0)
 
 
 def test_density_poisson_advect_v_on_full_v_space_of_sampled_x_cells(full):
