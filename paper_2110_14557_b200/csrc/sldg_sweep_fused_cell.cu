@@ -169,12 +169,19 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         }
     };
 
-    real first[NN], prev[NN];
+    // the x_1-swept first cell closes the periodic wrap at the end of the walk: in registers for k <= 2, parked in
+    // shared memory (one column per thread, conflict free) for k = 3 where the four matrices fill the register file
+    constexpr bool FS = K1 >= 4;
+    real* const first_s = reinterpret_cast<real*>(smem_raw + (((size_t)(ST + OST) * SS * sizeof(real) + 8 * ST + 31) & ~(size_t)15));
+    real first[FS ? 1 : NN], prev[NN];
     // chunk 0: cell 0 alone
     mbar_wait(bars_s, 0u);
-    swept(sin_ + pl * PC, first);
+    swept(sin_ + pl * PC, prev);
 #pragma unroll
-    for (int m = 0; m < NN; m++) prev[m] = first[m];
+    for (int m = 0; m < NN; m++) {
+        if constexpr (FS) first_s[m * blockDim.x + t] = prev[m];
+        else first[m] = prev[m];
+    }
     __syncthreads();
     issue_load(ST);
 
@@ -193,7 +200,10 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
             if (e < nin) swept(ibase + e * K1 * D0, nxt);
             else {
 #pragma unroll
-                for (int m = 0; m < NN; m++) nxt[m] = first[m];
+                for (int m = 0; m < NN; m++) {
+                    if constexpr (FS) nxt[m] = first_s[m * blockDim.x + t];
+                    else nxt[m] = first[m];
+                }
             }
 #pragma unroll
             for (int j2 = 0; j2 < K1; j2++) {
@@ -267,7 +277,9 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin,
     if (CR > g1.N) CR = g1.N;
     int stages = c->opt_cell_stages;
     const size_t smem_max = 227 * 1024;
-    auto smem_of = [&](long long pb, long long cr, int st) { return (size_t)(st + OST) * pb * cr * cellb + 8 * st + 16; };
+    auto smem_of = [&](long long pb, long long cr, int st) {
+        return (size_t)(st + OST) * pb * cr * cellb + 8 * st + 48 + (K1 >= 4 ? (size_t)pb * g0.N * K1 * K1 * sizeof(real) : 0);
+    };
     while (smem_of(PB, CR, stages) > smem_max && CR > 1) CR--;
     while (smem_of(PB, CR, stages) > smem_max && stages > 2) stages--;
     while (smem_of(PB, CR, stages) > smem_max && PB > 1) PB--;
