@@ -454,3 +454,29 @@ def test_steps_equals_repeated_step_bitwise(P, cfg, n):
         assert n2 - n1 < n1 - n0                                    # fewer passes
     else:
         assert n2 - n1 == n1 - n0
+
+
+# --------------------------------------------------------------- determinism under load (race detector of last resort)
+
+@pytest.mark.parametrize("geom,prec", [((2, 2, [48, 40, 12, 10], 2), "f64"), ((3, 3, [12, 10, 12, 6, 5, 4], 1), "f64"),
+                                       ((2, 2, [32, 32, 16, 12], 3), "f64"), ((3, 3, [12, 10, 12, 6, 5, 4], 1), "f32"),
+                                       ((2, 3, [32, 24, 8, 8, 6], 1), "f32")],
+                         ids=lambda v: v if isinstance(v, str) else "x".join(map(str, v[2])) + f"-k{v[3]}")
+def test_repeated_steps_are_bitwise_identical(P, geom, prec):
+    """Grids large enough to fill every SM several times: 6 runs of 3 Strang steps (fused passes, TMA rings, bulk
+    stores, in-place walks) from the same data give the same bits; a missing barrier or fence would not."""
+    dx, dv, cells, k = geom
+    dom = []
+    for a in range(dx + dv):
+        dom += [0.0, 4 * math.pi] if a < dx else [-6.0, 6.0]
+    g = P.Sldg(dx, dv, cells, k, dom, precision=prec)
+    g.set_option("graph", 0)
+    f0 = W.random_field(g.shape, seed=77, device=g.device).to(g.dtype)
+    ref = None
+    for rep in range(6):
+        f = f0.clone()
+        g.steps(f, 0.1, 3)
+        if ref is None:
+            ref = f
+        else:
+            assert torch.equal(ref, f), rep
