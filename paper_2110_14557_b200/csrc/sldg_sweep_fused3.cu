@@ -90,8 +90,8 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     const int NT = S * N0;                                 // compute threads; the producer is thread roundup32(NT)
     const bool lead = (t == (int)blockDim.x - 32);
     const int e1 = t / N0, i0 = t - e1 * N0;
-    const long long q = blockIdx.x / P.nstrips;
-    const int strip = (int)(blockIdx.x - q * P.nstrips);
+    const long long q = (long long)(blockIdx.x / (unsigned)P.nstrips);
+    const int strip = (int)(blockIdx.x - (unsigned)q * (unsigned)P.nstrips);
     const int c0 = strip * S;
     const int nS = min(S, N1 - c0);
     const bool active = t < NT && e1 < nS;
@@ -102,9 +102,17 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     real A1[NN], B1[NN], A2[NN], B2[NN], A3[NN], B3[NN];
     int s1, s2, s3;
     bool cp1, cp2, cp3;
-    load_table<K1>(P.t[0], (q / P.sdiv[0]) % P.smod[0], A1, B1, s1, cp1);
-    load_table<K1>(P.t[1], (q / P.sdiv[1]) % P.smod[1], A2, B2, s2, cp2);
-    load_table<K1>(P.t[2], (q / P.sdiv[2]) % P.smod[2], A3, B3, s3, cp3);
+    long long ix[3];
+    if (P.cubes < (1LL << 31)) {                           // 32-bit divisions when they fit (the usual case)
+#pragma unroll
+        for (int a = 0; a < 3; a++) ix[a] = ((unsigned)q / (unsigned)P.sdiv[a]) % (unsigned)P.smod[a];
+    } else {
+#pragma unroll
+        for (int a = 0; a < 3; a++) ix[a] = (q / P.sdiv[a]) % P.smod[a];
+    }
+    load_table<K1>(P.t[0], ix[0], A1, B1, s1, cp1);
+    load_table<K1>(P.t[1], ix[1], A2, B2, s2, cp2);
+    load_table<K1>(P.t[2], ix[2], A3, B3, s3, cp3);
     int ia = i0 - s1; if (ia < 0) ia += N0;
     int ib = ia - 1; if (ib < 0) ib += N0;
     const int oa = ia * K1, ob = ib * K1;
