@@ -1,0 +1,75 @@
+"""Whole-path checks of the CUDA solver against what the paper fixes (no oracle in the loop): the validation run of
+PAPER.md:149-181 -- linear Landau damping, alpha = 0.01, k = 0.5 on [0,4pi]^dx x [-6,6]^dv -- at a resolution the CPU
+oracle could not run in a test (2x2v, 32^2 x 64^2 cells, k = 2: 3.4e8 values), in fp64, in single precision
+(the curves overlap) and with the CGdG field solver (no significant difference).
+The decay rate gamma = -0.1533 and frequency omega = 1.4156 are BASELINE.json's / kinetic theory's; the oracle is
+pinned to the same numbers in tests/test_oracle_field.py::test_p12 on a 1x1v grid.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def damping_fit(t, ee, dt):
+    pk = [i for i in range(1, len(ee) - 1) if ee[i] > ee[i - 1] and ee[i] > ee[i + 1]]
+    tp, lp = [], []
+    for i in pk:
+        y0, y1, y2 = np.log(ee[i - 1:i + 2])
+        off = 0.5 * (y0 - y2) / (y0 - 2 * y1 + y2)
+        tp.append(t[i] + off * dt)
+        lp.append(y1 - 0.25 * (y0 - y2) * off)
+    tp, lp = np.array(tp), np.array(lp)
+    return np.polyfit(tp, lp, 1)[0] / 2, math.pi / np.mean(np.diff(tp)), len(pk)
+
+
+def run(P, precision, solver, nsteps=150, dt=0.1):
+    cfg = dict(name="landau2x2v", dim_x=2, dim_v=2, cells=[32, 32, 64, 64], degree=2,
+               domain=[0, 4 * math.pi, 0, 4 * math.pi, -6, 6, -6, 6], dt=dt, ic="landau",
+               ic_args=dict(eps=0.01, k=0.5, axes=[0]))
+    g = P.Sldg(2, 2, cfg["cells"], 2, cfg["domain"], precision=precision)
+    if solver == "cg":
+        g.set_poisson_solver(1, tol=1e-3)                      # the paper's tolerance
+    f = g.empty_field()
+    f.copy_(W.initial_data(cfg, [g.node_coords(a) for a in range(4)], device=g.device))
+    m0 = g.mass(f)
+    t, ee = [], []
+    for n in range(nsteps):
+        g.step(f, dt)
+        t.append((n + 0.5) * dt)                               # rho, E of a step are those of its middle
+        ee.append(g.electric_energy(g.last_E()))
+    return np.array(t), np.array(ee), abs(g.mass(f) - m0) / abs(m0)
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2110_14557_b200 as pkg
+    if not torch.cuda.is_available():
+        pytest.fail("gpu test without a CUDA device")
+    return pkg
+
+
+def test_linear_landau_damping_rate_fp64_fp32_and_cgdg(P):
+    t, e64, drift = run(P, "f64", "fft")
+    gamma, omega, npk = damping_fit(t, e64, 0.1)
+    assert npk >= 5
+    assert abs(gamma + 0.1533) < 0.04 * 0.1533, gamma
+    assert abs(omega - 1.4156) < 0.02 * 1.4156, omega
+    assert drift < 1e-12
+    # t = 0.05: E_1 = -(eps/k) sin(k x_1) up to O(dt): energy 1/4 (eps/k)^2 L^2 in 2-d (closed form p11)
+    assert abs(e64[0] / (0.25 * 0.02 ** 2 * (4 * math.pi) ** 2) - 1) < 0.02
+    # single precision: the curves overlap while the field is above the fp32 noise floor
+    _, e32, drift32 = run(P, "f32", "fft")
+    early = t < 8.0
+    assert np.abs(np.log(e32[early] / e64[early])).max() < 0.05
+    g32, w32, _ = damping_fit(t[early], e32[early], 0.1)
+    assert abs(g32 + 0.1533) < 0.08 * 0.1533 and drift32 < 1e-5
+    # CGdG field solver at the paper's tolerance: no significant difference
+    _, ecg, _ = run(P, "f64", "cg")
+    gcg, wcg, _ = damping_fit(t, ecg, 0.1)
+    assert abs(gcg + 0.1533) < 0.06 * 0.1533 and abs(wcg - 1.4156) < 0.03 * 1.4156, (gcg, wcg)
