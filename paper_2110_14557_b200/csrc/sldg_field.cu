@@ -113,29 +113,63 @@ __global__ void rho_final_kernel(const double* __restrict__ part, long long X, i
 // ------------------------------------------------------------------ Poisson / E (row a4)
 // out[q][m][p] = sum_n M[m][n] in[q][n][p], complex; M stored transposed MT[n][m] (re block, then im block).
 // HAS_IM = 0: the input is real.
+// A small complex GEMM per axis (D <= a few hundred): blocks of 16 x 16 outputs (m, column c = q * inner + p), the
+// n loop staged through shared memory in chunks of 32 so that M and the input are read from L2 once per tile and not
+// once per output.  Per output the sum runs over n in ascending order with the same fused multiply-adds as a plain
+// loop, so results do not depend on the tiling.
 template <int HAS_IM>
-__global__ void apply_axis_kernel(const double* __restrict__ inr, const double* __restrict__ ini,
-                                  const double* __restrict__ MT, long long D, long long inner, long long total,
-                                  double* __restrict__ outr, double* __restrict__ outi)
+__global__ void __launch_bounds__(256) apply_axis_kernel(const double* __restrict__ inr, const double* __restrict__ ini,
+                                                         const double* __restrict__ MT, long long D, long long inner,
+                                                         long long total, double* __restrict__ outr,
+                                                         double* __restrict__ outi)
 {
-    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= total) return;
-    long long p = t % inner, m = (t / inner) % D, q = t / (inner * D);
-    const double* Mr = MT + m; const double* Mi = MT + D * D + m;
-    const double* xr = inr + q * D * inner + p;
-    const double* xi = HAS_IM ? ini + q * D * inner + p : nullptr;
+    constexpr int TM = 16, TC = 16, KC = 32;
+    __shared__ double sMr[KC][TM + 1], sMi[KC][TM + 1], sXr[KC][TC + 1], sXi[KC][TC + 1];
+    const long long ncols = total / D;
+    const int tc = threadIdx.x % TC, tm = threadIdx.x / TC;            // column fastest: coalesced when inner >= 16
+    const long long c = (long long)blockIdx.x * TC + tc;
+    const long long m = (long long)blockIdx.y * TM + tm;
+    const bool colok = c < ncols, ok = colok && m < D;
+    const long long q = colok ? c / inner : 0, pp = colok ? c - q * inner : 0;
+    const long long xbase = q * D * inner + pp;
     double ar = 0.0, ai = 0.0;
-    for (long long n = 0; n < D; n++) {
-        double mr = __ldg(Mr + n * D), mi = __ldg(Mi + n * D);
-        double vr = xr[n * inner];
-        ar = fma(mr, vr, ar); ai = fma(mi, vr, ai);
-        if (HAS_IM) {
-            double vi = xi[n * inner];
-            ar = fma(-mi, vi, ar); ai = fma(mr, vi, ai);
+    for (long long n0 = 0; n0 < D; n0 += KC) {
+        // stage M[m-tile][n0..n0+KC) (stored transposed: MT[n][m]) and in[n0..n0+KC)[column tile]
+        for (int e = threadIdx.x; e < KC * TM; e += 256) {
+            const int kn = e / TM, km = e - kn * TM;
+            const long long n = n0 + kn, mm = (long long)blockIdx.y * TM + km;
+            const bool v = n < D && mm < D;
+            sMr[kn][km] = v ? __ldg(MT + n * D + mm) : 0.0;
+            sMi[kn][km] = v ? __ldg(MT + D * D + n * D + mm) : 0.0;
         }
+        for (int e = threadIdx.x; e < KC * TC; e += 256) {
+            const int kn = e / TC, kc = e - kn * TC;
+            const long long n = n0 + kn, cc = (long long)blockIdx.x * TC + kc;
+            double vr = 0.0, vi = 0.0;
+            if (n < D && cc < ncols) {
+                const long long qq = cc / inner, p2 = cc - qq * inner;
+                vr = inr[qq * D * inner + n * inner + p2];
+                if (HAS_IM) vi = ini[qq * D * inner + n * inner + p2];
+            }
+            sXr[kn][kc] = vr; sXi[kn][kc] = vi;
+        }
+        __syncthreads();
+        const int kmax = (int)min((long long)KC, D - n0);
+        for (int k = 0; k < kmax; k++) {
+            const double mr = sMr[k][tm], mi = sMi[k][tm], vr = sXr[k][tc];
+            ar = fma(mr, vr, ar); ai = fma(mi, vr, ai);
+            if (HAS_IM) {
+                const double vi = sXi[k][tc];
+                ar = fma(-mi, vi, ar); ai = fma(mr, vi, ai);
+            }
+        }
+        __syncthreads();
     }
-    outr[t] = ar;
-    if (outi) outi[t] = ai;
+    if (ok) {
+        const long long o = xbase + m * inner;
+        outr[o] = ar;
+        if (outi) outi[o] = ai;
+    }
 }
 
 // E^_d = i kappa_d rho^ / |kappa|^2 (kappa != 0), 0 at kappa = 0; kappa_d := 0 at the Nyquist index of an even axis.
@@ -279,8 +313,9 @@ cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E)
         bool last = (a == c->dx - 1);
         double* dr = last ? rr : ((a & 1) ? br : ar);
         double* di = last ? ri : ((a & 1) ? bi : ai);
-        if (si) apply_axis_kernel<1><<<grid, block, 0, c->stream>>>(sr, si, c->dFwdT[a], c->D[a], inner, X, dr, di);
-        else apply_axis_kernel<0><<<grid, block, 0, c->stream>>>(sr, si, c->dFwdT[a], c->D[a], inner, X, dr, di);
+        const dim3 ag((unsigned)((X / c->D[a] + 15) / 16), (unsigned)((c->D[a] + 15) / 16));
+        if (si) apply_axis_kernel<1><<<ag, 256, 0, c->stream>>>(sr, si, c->dFwdT[a], c->D[a], inner, X, dr, di);
+        else apply_axis_kernel<0><<<ag, 256, 0, c->stream>>>(sr, si, c->dFwdT[a], c->D[a], inner, X, dr, di);
         c->launches++;
         sr = dr; si = di; inner *= c->D[a];
     }
@@ -294,7 +329,8 @@ cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E)
         inner = 1;
         for (int a = 0; a < c->dx; a++) {
             bool last = (a == c->dx - 1);
-            apply_axis_kernel<1><<<grid, block, 0, c->stream>>>(pr, pi, c->dInvT[a], c->D[a], inner, X,
+            const dim3 ag((unsigned)((X / c->D[a] + 15) / 16), (unsigned)((c->D[a] + 15) / 16));
+            apply_axis_kernel<1><<<ag, 256, 0, c->stream>>>(pr, pi, c->dInvT[a], c->D[a], inner, X,
                                                                 last ? E + (long long)d * X : qr, last ? nullptr : qi);
             c->launches++;
             double* t;
