@@ -41,7 +41,7 @@ def build(force=False, verbose=False):
                 subprocess.check_call([NVCC] + FLAGS + extra + ["-DSLDG_REAL_FLOAT", "-c", src, "-o", obj32])
             objs.append(obj32)
     if force or _stale(LIB, objs):
-        subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-o", LIB] + objs)
+        subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
     return LIB
 
 
