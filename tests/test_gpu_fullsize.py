@@ -176,3 +176,14 @@ def test_single_sweeps_on_sampled_lines(full, kind):
             assert np.array_equal(lines_out, want), axis
         else:
             assert rel_inf(lines_out, want) <= TOL, (axis, rel_inf(lines_out, want))
+
+
+def test_constants_are_preserved_by_two_steps_at_full_size(full):
+    """rows of A + B sum to 1 (invariant p4), so a constant f stays constant to round-off through
+    every sweep of sldg_steps at full size (fused passes, in-place walks, v sweeps with E = 0 up to round-off).
+    Runs last: it overwrites the module's f."""
+    cfg, g, f = full
+    f.fill_(0.375)
+    g.steps(f, cfg["dt"], 2)
+    lo, hi = float(f.min()), float(f.max())
+    assert abs(lo - 0.375) <= 1e-13 and abs(hi - 0.375) <= 1e-13, (lo, hi)
