@@ -15,7 +15,9 @@
  * Parity pins (tests/test_oracle_*.py):  every function below is pinned by at least
  * one of p1..p13 of DESIGN.md section 3.  "parity unpinned": the two-stream growth
  * rate (not in the paper) and the internals of the authors' own FFT solver (reading
- * P1 is pinned only by the closed forms p10/p11 and the physics pin p12).
+ * P1 is pinned only by the closed forms p10/p11 and the physics pin p12); for the NEXT rows at the end of
+ * this file: E from the dG potential (reading U), sigma for k = 1 (reading T) and which quantities the single
+ * precision mode keeps in fp64 (reading W) are readings pinned by convergence / closed forms only.
  *
  * Layout of f (reading E): flat index n = n_0 + D_0 (n_1 + D_1 (n_2 + ...)),
  * axis order x_1..x_dx, v_1..v_dv (x_1 fastest), per-axis node index
