@@ -55,7 +55,11 @@ template <> struct Vec<2> {
 #endif
 // cells loaded ahead of the one being computed (loads in flight per thread = U * K1 * VEC values)
 template <int K1> struct Unroll {
+#ifdef SLDG_REAL_FLOAT
+    static constexpr int U = (K1 == 3) ? 8 : 4;            // measured: cfg2 (k=2) prefers 8 cells in flight, cfg4 (k=1) 4
+#else
     static constexpr int U = (K1 == 1) ? SLDG_WALK_U1 : (K1 == 2) ? SLDG_WALK_U2 : (K1 == 3) ? SLDG_WALK_U3 : (K1 == 4) ? SLDG_WALK_U4 : 2;
+#endif
 };
 
 // MODE 0: one shift per thread (x-sweep, shift indexed by a digit of the outer index)
@@ -188,9 +192,10 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_walk)(sldg_ctx* c, const void* fin, void*
     // Measured on B200: one value per thread (64-bit loads, more threads, more loads in
     // flight) beats 128-bit loads except for x-sweeps of degree >= 2, where the thread count is ample either way.
 #ifdef SLDG_REAL_FLOAT
-    // fp32 (measured on cfg2 / cfg4): 64-bit loads win on every slow axis except the FIRST velocity axis
-    // (inner == X, one shift entry per value), where one value per thread is 1.5x faster.
-    int vec = (g.mode == 1 && g.inner == g.smod) ? 1 : 2;
+    // fp32 (measured on cfg2 / cfg4 with smooth fields): 64-bit loads win on every slow axis.  (With a field that is
+    // round-off noise of random sign neighbouring x nodes get different s and the paired store splits: 2x slower,
+    // physically irrelevant.)
+    int vec = 2;
 #else
     int vec = (g.mode == 0 && g.K1 >= 3) ? 2 : 1;
 #endif
