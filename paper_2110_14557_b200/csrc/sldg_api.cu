@@ -36,7 +36,7 @@ void sldg_ev_end(sldg_ctx* c)
 }
 
 // ------------------------------------------------------------------ layout of the workspace
-struct WsLayout { size_t f2, vS, vAB, Wv, rho, E, part, cplx[6], red, phi, cg_info, total; long long part_cap; };
+struct WsLayout { size_t f2, vS, vAB, vS2, vAB2, Wv, rho, E, part, cplx[6], red, phi, cg_info, total; long long part_cap; };
 
 static WsLayout ws_layout(const sldg_ctx* c)
 {
@@ -47,6 +47,8 @@ static WsLayout ws_layout(const sldg_ctx* c)
     L.f2 = take((size_t)c->nf * c->esize);
     L.vS = take(X * 4);
     L.vAB = take(X * NN2 * 8);
+    L.vS2 = take(X * 4);
+    L.vAB2 = take(X * NN2 * 8);
     L.Wv = take((size_t)c->V * 8);
     L.rho = take(X * 8);
     L.E = take(X * 8 * c->dx);
@@ -127,6 +129,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
+    c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
@@ -235,6 +238,7 @@ extern "C" int sldg_set_workspace(sldg_ctx* c, void* dev, size_t bytes)
     char* b = (char*)dev;
     c->ws = b; c->ws_bytes = bytes;
     c->f2 = (double*)(b + L.f2); c->vS = (int*)(b + L.vS); c->vAB = (double*)(b + L.vAB);
+    c->vS2 = (int*)(b + L.vS2); c->vAB2 = (double*)(b + L.vAB2);
     c->Wv = (double*)(b + L.Wv); c->rho = (double*)(b + L.rho); c->E = (double*)(b + L.E);
     c->part = (double*)(b + L.part); c->part_cap = L.part_cap;
     for (int i = 0; i < 6; i++) c->cplx[i] = (double*)(b + L.cplx[i]);
@@ -536,19 +540,35 @@ extern "C" int sldg_advect_x(sldg_ctx* c, double* f, double dt)
 }
 
 struct VPrep { const double* E; double dt; };
-static int vprep(sldg_ctx* c, int i, void* arg)
+static int vtable_into(sldg_ctx* c, const VPrep* p, int i, int* S, double* AB)
 {
-    VPrep* p = (VPrep*)arg;
     const int a = c->dx + i;
     sldg_ev_begin(c, KIND_TABLE, a);
-    cudaError_t e = sldg_launch_vtable(c, p->E + (long long)i * c->X, p->dt, c->h[a], c->cells[a], c->vS, c->vAB);
+    cudaError_t e = sldg_launch_vtable(c, p->E + (long long)i * c->X, p->dt, c->h[a], c->cells[a], S, AB);
     sldg_ev_end(c);
     c->launches++;
     if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
     return SLDG_OK;
 }
+static int vprep(sldg_ctx* c, int i, void* arg) { return vtable_into(c, (VPrep*)arg, i, c->vS, c->vAB); }
+struct VPrepOff { VPrep p; int first; };
+static int vprep_off(sldg_ctx* c, int i, void* arg)
+{
+    VPrepOff* o = (VPrepOff*)arg;
+    return vtable_into(c, &o->p, o->first + i, c->vS, c->vAB);
+}
 
-// v-sweeps on (*cur, *oth): dx slow-axis sweeps, each flips the pair.
+// the fused v_1+v_2 pass (sldg_sweep_fusedv.cu) is planned when its shape rules hold
+static bool fusedv_possible(const sldg_ctx* c)
+{
+    if (!c->opt_fuse_v || c->dx < 2) return false;
+    return c->prec == SLDG_F32 ? sldg_fusedv_shape_f32(c, nullptr, nullptr) : sldg_fusedv_shape_f64(c, nullptr, nullptr);
+}
+// buffer flips of one v advection
+static int v_flips(const sldg_ctx* c) { return fusedv_possible(c) ? c->dx - 1 : c->dx; }
+
+// v-sweeps on (*cur, *oth): v_1 and v_2 in one fused out-of-place pass when the shape allows, every other sweep a
+// slow-axis walk; each pass flips the pair.
 static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt)
 {
     int axes[3];
@@ -558,6 +578,23 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         tabs[i].S = c->vS; tabs[i].AB = c->vAB; tabs[i].strideIdx = 1; tabs[i].strideM = c->X;
     }
     VPrep p = {E, dt};
+    if (fusedv_possible(c)) {
+        int r;
+        if ((r = vtable_into(c, &p, 0, c->vS, c->vAB))) return r;
+        if ((r = vtable_into(c, &p, 1, c->vS2, c->vAB2))) return r;
+        ShiftTable t2 = tabs[1];
+        t2.S = c->vS2; t2.AB = c->vAB2;
+        sldg_ev_begin(c, KIND_FUSED, 100 + c->dx);             // axis field >= 100: fused pass over axes a, a+1
+        cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
+                                            : sldg_launch_sweep_fusedv_f64(c, *cur, *oth, tabs[0], t2);
+        sldg_ev_end(c);
+        c->launches++;
+        if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+        double* t = *cur; *cur = *oth; *oth = t;
+        if (c->dx == 2) return SLDG_OK;
+        VPrepOff o = {p, 2};
+        return run_sweeps(c, cur, oth, axes + 2, tabs + 2, c->dx - 2, false, vprep_off, &o);
+    }
     return run_sweeps(c, cur, oth, axes, tabs, c->dx, false, vprep, &p);
 }
 
@@ -665,7 +702,7 @@ static int step_cost(const sldg_ctx* c, bool flip_total, int* p1)
 {
     int best = 1 << 30;
     for (int q1 = 0; q1 < 2; q1++) {
-        const int q2 = (q1 + c->dx + (flip_total ? 1 : 0)) & 1;
+        const int q2 = (q1 + v_flips(c) + (flip_total ? 1 : 0)) & 1;
         XPlan a = x_plan(c, q1 != 0), b = x_plan(c, q2 != 0);
         if (a.ok && b.ok && a.passes + b.passes < best) { best = a.passes + b.passes; if (p1) *p1 = q1; }
     }
@@ -933,7 +970,7 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
         if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
             c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
-            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2; for (int a = 0; a < nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
+            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2, a0 = r.axis >= 100 ? r.axis - 100 : 0; for (int a = a0; a < a0 + nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
         }
         c->ev_free.push_back(r);
     }
@@ -970,6 +1007,12 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "cell_rows")) { if (value < 0 || value > 1024) return SLDG_EINVAL; c->opt_cell_rows = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_cell_bytes = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_stages")) { if (value < 2 || value > 6) return SLDG_EINVAL; c->opt_cell_stages = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv_wx = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv_stages")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv_stages = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv_inflight")) { if (value < 1024 || value > 220 * 1024) return SLDG_EINVAL; c->opt_fv_inflight = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv_ppb")) { if (value < 0 || value > (1 << 20)) return SLDG_EINVAL; c->opt_fv_ppb = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv_l2")) { if (value < 0 || value > 3) return SLDG_EINVAL; c->opt_fv_l2 = (int)value; return SLDG_OK; }
     if (!strcmp(name, "rho_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_rho_vec = (int)value; return SLDG_OK; }
     if (!strcmp(name, "rho_blocks")) { if (value < 1 || value > 64) return SLDG_EINVAL; c->opt_rho_blocks = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_walk_vec = (int)value; return SLDG_OK; }

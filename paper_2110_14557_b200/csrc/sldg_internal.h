@@ -101,6 +101,7 @@ struct sldg_ctx {
     char* ws; size_t ws_bytes;
     double* f2;                     // second f buffer
     int* vS; double* vAB;           // v-sweep tables [X], [2 K1^2][X]
+    int* vS2; double* vAB2;         // second v-sweep table (the fused v_1+v_2 pass needs both at once)
     double* Wv;                     // [V]
     double* rho; double* E;         // [X], [dx][X]
     double* part; long long part_cap;   // rho partial sums
@@ -142,6 +143,12 @@ struct sldg_ctx {
     int opt_cell_rows;              // fused cell kernel: x_2 cells per chunk (0 = from opt_cell_bytes)
     int opt_cell_bytes;             // fused cell kernel: target bytes of one input stage (all planes of the block)
     int opt_cell_stages;            // fused cell kernel: input stages (2..6)
+    int opt_fuse_v;                 // 1: v_1 and v_2 sweeps in one pass when the shape allows (sldg_sweep_fusedv.cu)
+    int opt_fv_wx;                  // fused v kernel: x nodes per tile (0 = auto: 128-byte rows if the threads allow)
+    int opt_fv_stages;              // fused v kernel: ring depth (0 = from opt_fv_inflight)
+    int opt_fv_inflight;            // fused v kernel: bytes in flight per SM to aim for
+    int opt_fv_ppb;                 // fused v kernel: planes per block (0 = auto)
+    int opt_fv_l2;                  // fused v kernel: L2 promotion of the tensor map (0 none, 1 64 B, 2 128 B, 3 256 B)
     int opt_rho_vec;                // 0 = auto (2 when aligned), 1
     int opt_rho_blocks;             // rho kernel: 128-thread blocks per SM to aim for
 };
@@ -165,6 +172,10 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
 cudaError_t sldg_launch_sweep_fused3_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 cudaError_t sldg_launch_sweep_fused3_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
+bool sldg_fusedv_shape_f64(const sldg_ctx* c, int* wx_out, int* threads_out);
+bool sldg_fusedv_shape_f32(const sldg_ctx* c, int* wx_out, int* threads_out);
+cudaError_t sldg_launch_sweep_fusedv_f64(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2);
+cudaError_t sldg_launch_sweep_fusedv_f32(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2);
 SLDG_DECL_SWEEPS(_f64)
 SLDG_DECL_SWEEPS(_f32)
 cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,

@@ -1,0 +1,329 @@
+// sldg_sweep_fusedv.cu -- the v_1 AND v_2 sweeps of a v advection in ONE pass over f, sm_100a.
+//
+// eq. (3), reading B, applied twice in the order v_1, v_2 (E does not change during the v sweeps):
+//     u_i <- A(alpha) u_{(i-s) mod N} + B(alpha) u_{(i-s-1) mod N},   delta = -E_d(x) dt / h_{v_d}  per x node.
+// 16 B (fp64) of HBM traffic per value for TWO sweeps instead of 32 B.
+//
+//   f is seen as [planes q][D_2 = N_2 (k+1) rows][D_1 = N_1 (k+1) rows][X]  (X = all x nodes, contiguous; v_1 is the
+//   fastest velocity axis, v_2 the next; q runs over everything above v_2).  Every shift of both sweeps is that of
+//   the x node, so a thread that owns one x node keeps A_1, B_1, A_2, B_2 of that node in registers.
+//   A block owns a tile of WX consecutive x nodes and ALL of v_1, and walks along v_2 (and on through `ppb`
+//   consecutive planes: the rows of a tile are one arithmetic sequence in memory, and the tables do not change).
+//   One 3-d TMA tensor copy (box WX x D_1 x 1) per v_2 row brings [D_1][WX] into a ring of shared-memory stages;
+//   thread 0 issues them between its own rows (two rows behind the consumers' releases, so it rarely waits),
+//   full/empty mbarriers pace the ring, no __syncthreads in the loop.
+//   A thread owns one (x node, v_1 cell): per v_2 row it reads the k+1 rows of its two v_1 donor cells from shared
+//   memory (lanes run over x: conflict free) and applies A_1, B_1; after the k+1 rows of a v_2 cell it holds the
+//   v_1-swept (k+1)^2 block, combines it with the previous block by A_2, B_2 (register walk, as in
+//   sldg_sweep_walk.cu) and stores output cell (j + s_2 + 1) mod N_2 straight from registers (lanes over x:
+//   coalesced WX * 8 B pieces).  The first block closes the periodic wrap: kept in registers for k <= 1, streamed
+//   in once more (k+1 extra rows per plane, 1/N_2 of the reads) for k = 2.
+//
+// Arithmetic per value is identical (same operands, same order) to sweep_walk_kernel on v_1 then on v_2, so the
+// fused and the unfused plans agree bit for bit.  Out of place only; degree <= 2; D_1 <= 256 (one TMA box);
+// X * sizeof(real) a multiple of 16.
+#include <cuda.h>
+
+#include "sldg_async.h"
+#include "sldg_internal.h"
+#include "sldg_real.h"
+
+namespace {
+
+using namespace sldg_async;
+
+struct FVParams {
+    real* fout;
+    long long X, planes;
+    int N1, N2, WX, stages, ppb, ntiles;
+    uint32_t stage_bytes;         // ring slot stride (>= D_1 * WX * sizeof(real), multiple of 128)
+    ShiftTable t1, t2;
+};
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+template <int K1> struct FVTraits {
+    static constexpr bool KEEP = (K1 <= 2);        // first v_2 block kept in registers (else streamed in again)
+    // threads per block.  Registers are split over the 4 SM sub-partitions: 16 warps leave 128 registers per thread
+    // (what the (k+1)^2 blocks and four tables of k = 2 need), 20 warps 96.
+    static constexpr int MAXT = (K1 <= 2) ? 640 : 512;
+};
+
+template <int K1>
+__global__ void __launch_bounds__(FVTraits<K1>::MAXT)
+    sweep_fusedv_kernel(const __grid_constant__ CUtensorMap tmap, const FVParams P)
+{
+    constexpr int NN = K1 * K1;
+    constexpr bool KEEP = FVTraits<K1>::KEEP;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int ST = P.stages, WX = P.WX, N1 = P.N1, N2 = P.N2;
+    const int D1 = N1 * K1, D2 = N2 * K1;
+    const uint32_t ring_s = smem_u32(smem_raw);
+    const uint32_t full_s = ring_s + (uint32_t)ST * P.stage_bytes;      // ST full barriers, then ST empty barriers
+    const uint32_t empty_s = full_s + (uint32_t)ST * 8u;
+
+    const int t = threadIdx.x;
+    const int NTR = (int)blockDim.x;                                    // whole warps
+    const int LAG = ST >= 4 ? 2 : 1;                                    // the producer refills the slot of row i - LAG
+    const int DEP = ST - LAG;                                           // rows in flight ahead of the consumers
+    const int tile = (int)(blockIdx.x % (unsigned)P.ntiles);
+    const int chunk = (int)(blockIdx.x / (unsigned)P.ntiles);
+    const long long q0 = (long long)chunk * P.ppb;
+    const int nq = (int)min((long long)P.ppb, P.planes - q0);
+    const long long x0 = (long long)tile * WX;
+    const int RP = D2 + (KEEP ? 0 : K1);                                // rows streamed per plane
+    const int total = nq * RP;
+
+    if (t == 0) {
+        for (int s = 0; s < ST; s++) { mbar_init(full_s + 8u * s, 1); mbar_init(empty_s + 8u * s, NTR / 32); }
+        mbar_init_fence();
+    }
+    __syncthreads();
+
+    // ---------------- producer (thread 0, between its own rows): one tensor copy per v_2 row
+    const uint32_t row_bytes = (uint32_t)D1 * (uint32_t)WX * (uint32_t)sizeof(real);
+    int pst = 0, pn = 0, pr = 0, pi = 0;
+    long long prow0 = q0 * D2;                                          // first row of the producer's current plane
+    auto produce = [&]() {
+        if (pi >= total) return;
+        if (pn > 0) mbar_wait(empty_s + 8u * pst, (uint32_t)((pn - 1) & 1));
+        mbar_expect_tx(full_s + 8u * pst, row_bytes);
+        const int rr = (pr >= D2) ? pr - D2 : pr;
+        tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + rr), full_s + 8u * pst);
+        if (++pst == ST) { pst = 0; pn++; }
+        if (++pr == RP) { pr = 0; prow0 += D2; }
+        pi++;
+    };
+    if (t == 0)
+        for (int i = 0; i < DEP; i++) produce();
+
+    // ---------------- consumers
+    const int c = t / WX, x = t - c * WX;
+    const bool active = (c < N1) && (x0 + x < P.X);
+    real A1[NN], B1[NN], A2[NN], B2[NN];
+    int s1 = 0, s2 = 0;
+    bool cp1 = false, cp2 = false;
+#pragma unroll
+    for (int m = 0; m < NN; m++) { A1[m] = B1[m] = A2[m] = B2[m] = 0; }
+    if (active) {
+        const long long idx = x0 + x;
+        const int sv1 = __ldg(P.t1.S + idx), sv2 = __ldg(P.t2.S + idx);
+        cp1 = (sv1 & SLDG_COPY_BIT) != 0; s1 = sv1 & SLDG_S_MASK;
+        cp2 = (sv2 & SLDG_COPY_BIT) != 0; s2 = sv2 & SLDG_S_MASK;
+        const real* ab1 = static_cast<const real*>(P.t1.AB) + idx * P.t1.strideIdx;
+        const real* ab2 = static_cast<const real*>(P.t2.AB) + idx * P.t2.strideIdx;
+#pragma unroll
+        for (int m = 0; m < NN; m++) {
+            A1[m] = __ldg(ab1 + m * P.t1.strideM); B1[m] = __ldg(ab1 + (NN + m) * P.t1.strideM);
+            A2[m] = __ldg(ab2 + m * P.t2.strideM); B2[m] = __ldg(ab2 + (NN + m) * P.t2.strideM);
+        }
+    }
+    int ia = 0, ib = 0;
+    if (active) {
+        ia = c - s1; if (ia < 0) ia += N1;
+        ib = ia - 1; if (ib < 0) ib += N1;
+    }
+    const int oa = ia * K1 * WX + x, ob = ib * K1 * WX + x;           // donor rows inside a stage, in values
+    const real* const ring = reinterpret_cast<const real*>(smem_raw);
+    const int stage_vals = (int)(P.stage_bytes / sizeof(real));
+    const bool warp_lead = (t & 31) == 0;
+
+    int st = 0;
+    uint32_t ph = 0;
+    // one v_2 row of the ring -> the k+1 v_1-swept values of this thread's cell
+    auto swept_row = [&](real (&g)[K1]) {
+        if (t == 0) produce();
+        mbar_wait(full_s + 8u * st, ph);
+        const real* stage = ring + (size_t)st * stage_vals;
+        real a[K1], b[K1];
+#pragma unroll
+        for (int m = 0; m < K1; m++) { a[m] = stage[oa + m * WX]; b[m] = stage[ob + m * WX]; }
+        __syncwarp();
+        if (warp_lead) mbar_arrive(empty_s + 8u * st);
+#pragma unroll
+        for (int j = 0; j < K1; j++) {
+            real acc = 0;
+#pragma unroll
+            for (int m = 0; m < K1; m++) acc += A1[j * K1 + m] * a[m];
+#pragma unroll
+            for (int m = 0; m < K1; m++) acc += B1[j * K1 + m] * b[m];
+            g[j] = cp1 ? a[j] : acc;
+        }
+        if (++st == ST) { st = 0; ph ^= 1u; }
+    };
+
+    const long long X = P.X;
+    const long long rowX = (long long)D1 * X;                          // one v_2 row of a plane, in values
+    for (int iq = 0; iq < nq; iq++) {
+        real* const oplane = P.fout + (q0 + iq) * (long long)D2 * rowX + (long long)(c * K1) * X + x0 + x;
+        real first[KEEP ? NN : 1], prev[NN];
+        int io2 = s2 + 1; if (io2 >= N2) io2 -= N2;                    // output v_2 cell of the current donor pair
+        for (int jc = 0; jc <= N2; jc++) {
+            real nxt[NN];                                              // [j2][j1]
+            if (!KEEP || jc < N2) {
+#pragma unroll
+                for (int j2 = 0; j2 < K1; j2++) {
+                    real g[K1];
+                    swept_row(g);
+#pragma unroll
+                    for (int j1 = 0; j1 < K1; j1++) nxt[j2 * K1 + j1] = g[j1];
+                }
+            } else {
+#pragma unroll
+                for (int m = 0; m < NN; m++) nxt[m] = first[KEEP ? m : 0];
+            }
+            if (jc == 0) {
+                if (KEEP) {
+#pragma unroll
+                    for (int m = 0; m < NN; m++) first[KEEP ? m : 0] = nxt[m];
+                }
+            } else {
+                if (active) {
+                    real* o = oplane + (long long)(io2 * K1) * rowX;
+#pragma unroll
+                    for (int j2 = 0; j2 < K1; j2++)
+#pragma unroll
+                        for (int j1 = 0; j1 < K1; j1++) {
+                            real acc = 0;
+#pragma unroll
+                            for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
+#pragma unroll
+                            for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * prev[l * K1 + j1];
+                            __stcs(o + j2 * rowX + (long long)j1 * X, cp2 ? nxt[j2 * K1 + j1] : acc);
+                        }
+                }
+                if (++io2 == N2) io2 = 0;
+            }
+#pragma unroll
+            for (int m = 0; m < NN; m++) prev[m] = nxt[m];
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiled encode_fn()
+{
+    static EncodeTiled fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiled>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+template <int K1>
+cudaError_t launch(sldg_ctx* c, const CUtensorMap& tm, const FVParams& P, int threads, size_t smem)
+{
+    auto kern = sweep_fusedv_kernel<K1>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const long long nchunks = (P.planes + P.ppb - 1) / P.ppb;
+    const long long grid = nchunks * P.ntiles;
+    if (grid > 0x7fffffffLL) return cudaErrorNotSupported;
+    kern<<<(unsigned)grid, threads, smem, c->stream>>>(tm, P);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// The shape rules of the fused v_1+v_2 pass.  wx / threads / stage_bytes of the launch are returned when non-null.
+bool SLDG_SFX(sldg_fusedv_shape)(const sldg_ctx* c, int* wx_out, int* threads_out)
+{
+    const int K1 = c->K1;
+    if (c->dx < 2 || K1 > 3) return false;
+    const long long D1 = c->D[c->dx];
+    if (D1 > 256 || c->cells[c->dx] < 1) return false;
+    if ((c->X * (long long)sizeof(real)) & 15) return false;
+    const int cap = (K1 <= 2) ? FVTraits<1>::MAXT : FVTraits<3>::MAXT;  // threads allowed
+    // x nodes per tile: rows of 128 B when the thread budget allows, else 64 B; never below 32 B
+    int wx = c->opt_fv_wx > 0 ? c->opt_fv_wx : (int)(128 / sizeof(real));
+    while (wx * (int)sizeof(real) > 32 && (long long)wx * c->cells[c->dx] > cap) wx /= 2;
+    if ((long long)wx * c->cells[c->dx] > cap) return false;
+    if ((wx * (int)sizeof(real)) & 15) return false;
+    if (wx > 256) return false;
+    if (wx_out) *wx_out = wx;
+    if (threads_out) *threads_out = (int)(((long long)wx * c->cells[c->dx] + 31) / 32 * 32);
+    return true;
+}
+
+// t1, t2: the shift tables of v_1 and v_2 (one entry per x node).  cudaErrorNotSupported when the shape does not fit.
+cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1,
+                                               const ShiftTable& t2)
+{
+    int wx = 0, threads = 0;
+    if (fin == fout || !SLDG_SFX(sldg_fusedv_shape)(c, &wx, &threads)) return cudaErrorNotSupported;
+    if ((((uintptr_t)fin) | ((uintptr_t)fout)) & 15) return cudaErrorNotSupported;
+    EncodeTiled enc = encode_fn();
+    if (!enc) return cudaErrorNotSupported;
+    const int K1 = c->K1, a1 = c->dx, a2 = c->dx + 1;
+    const long long D1 = c->D[a1], D2 = c->D[a2];
+    const long long planes = c->V / (D1 * D2);
+    const long long rows = D2 * planes;
+    if (c->X >= (1LL << 31) || rows >= (1LL << 31)) return cudaErrorNotSupported;
+
+    FVParams P;
+    P.fout = static_cast<real*>(fout);
+    P.X = c->X; P.planes = planes; P.N1 = c->cells[a1]; P.N2 = c->cells[a2]; P.WX = wx;
+    P.ntiles = (int)((c->X + wx - 1) / wx);
+    P.stage_bytes = (uint32_t)((D1 * wx * sizeof(real) + 127) / 128 * 128);
+    // ring depth: about opt_fv_inflight bytes in flight per SM
+    const size_t regs_blocks = (K1 <= 2) ? (size_t)(65536 / 96) / threads : 1;
+    size_t bps = regs_blocks < 1 ? 1 : regs_blocks;
+    if (bps > 4) bps = 4;
+    int stages = c->opt_fv_stages > 0 ? c->opt_fv_stages : (int)((size_t)c->opt_fv_inflight / bps / P.stage_bytes);
+    if (stages < 3) stages = 3;
+    if (stages > 24) stages = 24;
+    auto smem_of = [&](int st) { return (size_t)st * P.stage_bytes + 16 * (size_t)st + 128; };
+    while (stages > 2 && smem_of(stages) > 227 * 1024) stages--;
+    if (smem_of(stages) > 227 * 1024) return cudaErrorNotSupported;
+    P.stages = stages;
+    // planes per block: long walks (tables and pipeline fill amortised), yet enough blocks to fill the GPU evenly
+    long long ppb = c->opt_fv_ppb > 0 ? c->opt_fv_ppb : 1;
+    if (c->opt_fv_ppb <= 0) {
+        const long long slots = (long long)c->sm_count * (long long)bps;
+        while (ppb < planes && D2 * ppb < 512 && (planes / (ppb * 2)) * P.ntiles >= 8 * slots) ppb *= 2;
+    }
+    if (ppb > planes) ppb = planes;
+    P.ppb = (int)ppb;
+    P.t1 = t1; P.t2 = t2;
+
+    CUtensorMap tm;
+    const cuuint64_t gdim[3] = {(cuuint64_t)c->X, (cuuint64_t)D1, (cuuint64_t)rows};
+    const cuuint64_t gstr[2] = {(cuuint64_t)c->X * sizeof(real), (cuuint64_t)c->X * D1 * sizeof(real)};
+    const cuuint32_t box[3] = {(cuuint32_t)wx, (cuuint32_t)D1, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUtensorMapDataType dt = sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const CUtensorMapL2promotion l2 = c->opt_fv_l2 == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
+                                    : c->opt_fv_l2 == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
+                                    : c->opt_fv_l2 == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                                        : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
+    if (enc(&tm, dt, 3, const_cast<void*>(fin), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, l2, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorNotSupported;
+    const size_t smem = smem_of(stages);
+    switch (K1) {
+    case 1: return launch<1>(c, tm, P, threads, smem);
+    case 2: return launch<2>(c, tm, P, threads, smem);
+    case 3: return launch<3>(c, tm, P, threads, smem);
+    }
+    return cudaErrorNotSupported;
+}
