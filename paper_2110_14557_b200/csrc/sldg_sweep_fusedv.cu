@@ -24,6 +24,8 @@
 // X * sizeof(real) a multiple of 16.
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "sldg_async.h"
 #include "sldg_internal.h"
 #include "sldg_real.h"
@@ -56,6 +58,11 @@ template <int K1> struct FVTraits {
     // threads per block.  Registers are split over the 4 SM sub-partitions: 16 warps leave 128 registers per thread
     // (what the (k+1)^2 blocks and four tables of k = 2 need), 20 warps 96.
     static constexpr int MAXT = (K1 <= 2) ? 640 : 512;
+    // k = 2: A_2, B_2 of the tile's x nodes live in shared memory (rows [A_2[j][.] | B_2[j][.]], one padded record per
+    // x node, read as 2-value vectors: lanes of equal x broadcast, different x fall on different banks); with all four
+    // tables in registers the kernel spills (ncu: a third of the issue slots stalled on local loads).
+    static constexpr bool T2S = (K1 >= 3);
+    static constexpr int PAD = 2 * K1 * K1 + 4;
 };
 
 template <int K1>
@@ -64,7 +71,9 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
 {
     constexpr int NN = K1 * K1;
     constexpr bool KEEP = FVTraits<K1>::KEEP;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr bool T2S = FVTraits<K1>::T2S;
+    constexpr int PAD = FVTraits<K1>::PAD;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
     const int ST = P.stages, WX = P.WX, N1 = P.N1, N2 = P.N2;
     const int D1 = N1 * K1, D2 = N2 * K1;
     const uint32_t ring_s = smem_u32(smem_raw);
@@ -97,7 +106,7 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
         if (pi >= total) return;
         if (pn > 0) mbar_wait(empty_s + 8u * pst, (uint32_t)((pn - 1) & 1));
         mbar_expect_tx(full_s + 8u * pst, row_bytes);
-        const int rr = (pr >= D2) ? pr - D2 : pr;
+        const int rr = (pr >= D2) ? pr - D2 : pr;                       // k = 2: rows 0..k of the plane once more
         tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + rr), full_s + 8u * pst);
         if (++pst == ST) { pst = 0; pn++; }
         if (++pr == RP) { pr = 0; prow0 += D2; }
@@ -132,81 +141,123 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
         ia = c - s1; if (ia < 0) ia += N1;
         ib = ia - 1; if (ib < 0) ib += N1;
     }
-    const int oa = ia * K1 * WX + x, ob = ib * K1 * WX + x;           // donor rows inside a stage, in values
+    real* const tab2 = reinterpret_cast<real*>(smem_raw + (size_t)ST * P.stage_bytes + 16 * (size_t)ST) + x * PAD;
+    if (T2S) {
+        if (c == 0) {
+#pragma unroll
+            for (int j = 0; j < K1; j++)
+#pragma unroll
+                for (int l = 0; l < K1; l++) { tab2[j * 2 * K1 + l] = A2[j * K1 + l]; tab2[j * 2 * K1 + K1 + l] = B2[j * K1 + l]; }
+        }
+        __syncthreads();
+    }
+    // the alpha == 0 copy selects are compiled out for warps none of whose x nodes has the copy bit (the usual case)
+    const bool anycp = __any_sync(0xffffffffu, cp1 || cp2);
+
     const real* const ring = reinterpret_cast<const real*>(smem_raw);
+    const real* const pa0 = ring + ia * K1 * WX + x;                    // donor rows of stage 0
+    const real* const pb0 = ring + ib * K1 * WX + x;
     const int stage_vals = (int)(P.stage_bytes / sizeof(real));
     const bool warp_lead = (t & 31) == 0;
-
-    int st = 0;
-    uint32_t ph = 0;
-    // one v_2 row of the ring -> the k+1 v_1-swept values of this thread's cell
-    auto swept_row = [&](real (&g)[K1]) {
-        if (t == 0) produce();
-        mbar_wait(full_s + 8u * st, ph);
-        const real* stage = ring + (size_t)st * stage_vals;
-        real a[K1], b[K1];
-#pragma unroll
-        for (int m = 0; m < K1; m++) { a[m] = stage[oa + m * WX]; b[m] = stage[ob + m * WX]; }
-        __syncwarp();
-        if (warp_lead) mbar_arrive(empty_s + 8u * st);
-#pragma unroll
-        for (int j = 0; j < K1; j++) {
-            real acc = 0;
-#pragma unroll
-            for (int m = 0; m < K1; m++) acc += A1[j * K1 + m] * a[m];
-#pragma unroll
-            for (int m = 0; m < K1; m++) acc += B1[j * K1 + m] * b[m];
-            g[j] = cp1 ? a[j] : acc;
-        }
-        if (++st == ST) { st = 0; ph ^= 1u; }
-    };
-
     const long long X = P.X;
     const long long rowX = (long long)D1 * X;                          // one v_2 row of a plane, in values
-    for (int iq = 0; iq < nq; iq++) {
-        real* const oplane = P.fout + (q0 + iq) * (long long)D2 * rowX + (long long)(c * K1) * X + x0 + x;
-        real first[KEEP ? NN : 1], prev[NN];
-        int io2 = s2 + 1; if (io2 >= N2) io2 -= N2;                    // output v_2 cell of the current donor pair
-        for (int jc = 0; jc <= N2; jc++) {
-            real nxt[NN];                                              // [j2][j1]
-            if (!KEEP || jc < N2) {
+    const long long cellX = (long long)K1 * rowX, planeX = (long long)D2 * rowX;
+
+    int st = 0, soff = 0;                                              // ring slot of the next row, its offset in values
+    uint32_t ph = 0, fbar = full_s;
+
+    auto body = [&](auto cpt) {
+        constexpr bool CP = decltype(cpt)::value;
+        // one v_2 row of the ring -> the k+1 v_1-swept values of this thread's cell
+        auto swept_row = [&](real* g) {
+            if (t == 0) produce();
+            mbar_wait(fbar, ph);
+            real a[K1], b[K1];
 #pragma unroll
-                for (int j2 = 0; j2 < K1; j2++) {
-                    real g[K1];
-                    swept_row(g);
+            for (int m = 0; m < K1; m++) { a[m] = pa0[soff + m * WX]; b[m] = pb0[soff + m * WX]; }
+            __syncwarp();
+            if (warp_lead) mbar_arrive(fbar + 8u * (uint32_t)ST);
 #pragma unroll
-                    for (int j1 = 0; j1 < K1; j1++) nxt[j2 * K1 + j1] = g[j1];
-                }
-            } else {
+            for (int j = 0; j < K1; j++) {
+                real acc = 0;
 #pragma unroll
-                for (int m = 0; m < NN; m++) nxt[m] = first[KEEP ? m : 0];
+                for (int m = 0; m < K1; m++) acc += A1[j * K1 + m] * a[m];
+#pragma unroll
+                for (int m = 0; m < K1; m++) acc += B1[j * K1 + m] * b[m];
+                g[j] = (CP && cp1) ? a[j] : acc;
             }
-            if (jc == 0) {
-                if (KEEP) {
+            st++; soff += stage_vals; fbar += 8u;
+            if (st == ST) { st = 0; soff = 0; fbar = full_s; ph ^= 1u; }
+        };
+        // output cell *o <- A_2 nxt + B_2 prev   (blocks are [j2][j1])
+        auto emit = [&](real* o, const real (&nxt)[NN], const real (&prev)[NN]) {
 #pragma unroll
-                    for (int m = 0; m < NN; m++) first[KEEP ? m : 0] = nxt[m];
+            for (int j2 = 0; j2 < K1; j2++) {
+                real ab[2 * K1];                                       // A_2[j2][.] then B_2[j2][.]
+                if (T2S) {
+#pragma unroll
+                    for (int l = 0; l < K1; l++) {                      // 2 K1 is even: whole 2-value vectors
+                        const real2 v = *reinterpret_cast<const real2*>(tab2 + j2 * 2 * K1 + 2 * l);
+                        ab[2 * l] = v.x; ab[2 * l + 1] = v.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int l = 0; l < K1; l++) { ab[l] = A2[j2 * K1 + l]; ab[K1 + l] = B2[j2 * K1 + l]; }
                 }
-            } else {
-                if (active) {
-                    real* o = oplane + (long long)(io2 * K1) * rowX;
+                real* p = o;
 #pragma unroll
-                    for (int j2 = 0; j2 < K1; j2++)
+                for (int j1 = 0; j1 < K1; j1++) {
+                    real acc = 0;
 #pragma unroll
-                        for (int j1 = 0; j1 < K1; j1++) {
-                            real acc = 0;
+                    for (int l = 0; l < K1; l++) acc += ab[l] * nxt[l * K1 + j1];
 #pragma unroll
-                            for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
-#pragma unroll
-                            for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * prev[l * K1 + j1];
-                            __stcs(o + j2 * rowX + (long long)j1 * X, cp2 ? nxt[j2 * K1 + j1] : acc);
-                        }
+                    for (int l = 0; l < K1; l++) acc += ab[K1 + l] * prev[l * K1 + j1];
+                    const real r = (CP && cp2) ? nxt[j2 * K1 + j1] : acc;
+                    if (active) __stcs(p, r);
+                    p += X;
                 }
-                if (++io2 == N2) io2 = 0;
+                o += rowX;
             }
+        };
+
+        for (int iq = 0; iq < nq; iq++) {
+            real* const oplane = P.fout + (q0 + iq) * planeX + (long long)(c * K1) * X + x0 + x;
+            int io2 = s2 + 1; if (io2 >= N2) io2 -= N2;                // output v_2 cell of the current donor pair
+            real* o = oplane + (long long)io2 * cellX;
+            real u[2][NN], first[KEEP ? NN : 1];
+            auto get = [&](real (&dst)[NN], int jc) {                  // v_1-swept block of v_2 cell jc (N_2 = cell 0 again)
+                if (!KEEP || jc < N2) {
 #pragma unroll
-            for (int m = 0; m < NN; m++) prev[m] = nxt[m];
+                    for (int j2 = 0; j2 < K1; j2++) swept_row(&dst[j2 * K1]);
+                } else {
+#pragma unroll
+                    for (int m = 0; m < NN; m++) dst[m] = first[KEEP ? m : 0];
+                }
+            };
+            auto step = [&](real (&nxt)[NN], const real (&prev)[NN], int jc) {
+                get(nxt, jc);
+                emit(o, nxt, prev);
+                o += cellX;
+                if (++io2 == N2) { io2 = 0; o -= planeX; }
+            };
+            get(u[0], 0);
+            if (KEEP) {
+#pragma unroll
+                for (int m = 0; m < NN; m++) first[KEEP ? m : 0] = u[0][m];
+            }
+            // two cells per trip so that the blocks alternate between u[0] and u[1] without register moves
+#pragma unroll 1
+            for (int jc = 1; jc <= N2; jc += 2) {
+                step(u[1], u[0], jc);
+                if (jc + 1 > N2) {                                      // odd N_2: the pair ends on u[1]; not reached again
+                    break;
+                }
+                step(u[0], u[1], jc + 1);
+            }
         }
-    }
+    };
+    if (anycp) body(std::true_type{});
+    else body(std::false_type{});
 }
 
 typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -284,7 +335,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     P.fout = static_cast<real*>(fout);
     P.X = c->X; P.planes = planes; P.N1 = c->cells[a1]; P.N2 = c->cells[a2]; P.WX = wx;
     P.ntiles = (int)((c->X + wx - 1) / wx);
-    P.stage_bytes = (uint32_t)((D1 * wx * sizeof(real) + 127) / 128 * 128);
+    P.stage_bytes = (uint32_t)((D1 * wx * sizeof(real) + 1023) / 1024 * 1024);
     // ring depth: about opt_fv_inflight bytes in flight per SM
     const size_t regs_blocks = (K1 <= 2) ? (size_t)(65536 / 96) / threads : 1;
     size_t bps = regs_blocks < 1 ? 1 : regs_blocks;
@@ -292,7 +343,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     int stages = c->opt_fv_stages > 0 ? c->opt_fv_stages : (int)((size_t)c->opt_fv_inflight / bps / P.stage_bytes);
     if (stages < 3) stages = 3;
     if (stages > 24) stages = 24;
-    auto smem_of = [&](int st) { return (size_t)st * P.stage_bytes + 16 * (size_t)st + 128; };
+    auto smem_of = [&](int st) { return (size_t)st * P.stage_bytes + 16 * (size_t)st + (size_t)wx * (2 * K1 * K1 + 4) * sizeof(real) + 128; };
     while (stages > 2 && smem_of(stages) > 227 * 1024) stages--;
     if (smem_of(stages) > 227 * 1024) return cudaErrorNotSupported;
     P.stages = stages;
