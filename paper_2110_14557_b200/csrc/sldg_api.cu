@@ -562,7 +562,13 @@ static int vprep_off(sldg_ctx* c, int i, void* arg)
 static bool fusedv_possible(const sldg_ctx* c)
 {
     if (!c->opt_fuse_v || c->dx < 2) return false;
-    return c->prec == SLDG_F32 ? sldg_fusedv_shape_f32(c, nullptr, nullptr) : sldg_fusedv_shape_f64(c, nullptr, nullptr);
+    int wx = 0;
+    if (!(c->prec == SLDG_F32 ? sldg_fusedv_shape_f32(c, &wx, nullptr) : sldg_fusedv_shape_f64(c, &wx, nullptr))) return false;
+    if (c->opt_fuse_v == 2) return true;
+    // auto: a block walks all of v_2 serially, so the pass pays only when its independent walks (x tiles times planes
+    // above v_2) fill the GPU; small problems (BASELINE config 1: 16 tiles) are faster with two wide walk launches
+    const long long walks = ((c->X + wx - 1) / wx) * (c->V / (c->D[c->dx] * c->D[c->dx + 1]));
+    return walks >= 2LL * c->sm_count;
 }
 // buffer flips of one v advection
 static int v_flips(const sldg_ctx* c) { return fusedv_possible(c) ? c->dx - 1 : c->dx; }
@@ -1007,7 +1013,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "cell_rows")) { if (value < 0 || value > 1024) return SLDG_EINVAL; c->opt_cell_rows = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_cell_bytes = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_stages")) { if (value < 2 || value > 6) return SLDG_EINVAL; c->opt_cell_stages = (int)value; return SLDG_OK; }
-    if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv_wx = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_stages")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_inflight")) { if (value < 1024 || value > 220 * 1024) return SLDG_EINVAL; c->opt_fv_inflight = (int)value; return SLDG_OK; }

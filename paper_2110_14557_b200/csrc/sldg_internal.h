@@ -143,7 +143,7 @@ struct sldg_ctx {
     int opt_cell_rows;              // fused cell kernel: x_2 cells per chunk (0 = from opt_cell_bytes)
     int opt_cell_bytes;             // fused cell kernel: target bytes of one input stage (all planes of the block)
     int opt_cell_stages;            // fused cell kernel: input stages (2..6)
-    int opt_fuse_v;                 // 1: v_1 and v_2 sweeps in one pass when the shape allows (sldg_sweep_fusedv.cu)
+    int opt_fuse_v;                 // v_1 and v_2 sweeps in one pass (sldg_sweep_fusedv.cu): 0 never, 1 when the shape allows and the walks fill the GPU, 2 whenever the shape allows
     int opt_fv_wx;                  // fused v kernel: x nodes per tile (0 = auto: 128-byte rows if the threads allow)
     int opt_fv_stages;              // fused v kernel: ring depth (0 = from opt_fv_inflight)
     int opt_fv_inflight;            // fused v kernel: bytes in flight per SM to aim for

@@ -437,10 +437,15 @@ def test_step_with_and_without_fused3_agree_bitwise(P, cfg):
 
 @pytest.mark.parametrize("cfg", [small_cfgs()[1], small_cfgs()[3], small_cfgs()[4]], ids=lambda c: c["name"])
 @pytest.mark.parametrize("n", [1, 2, 3, 4])
-def test_steps_equals_repeated_step_bitwise(P, cfg, n):
-    """sldg_steps may alternate buffers between steps (one-pass x half steps for dim_x = 3): same bits, result in f."""
+@pytest.mark.parametrize("fuse_v", [0, 2])
+def test_steps_equals_repeated_step_bitwise(P, cfg, n, fuse_v):
+    """sldg_steps may alternate buffers between steps: same bits, result in f.  It saves passes exactly when a single
+    step, which must end in f, cannot use its one-pass plans: dim_x = 3 with three separate v sweeps (odd flips: only one
+    of the two x half steps can be the fused x_1+x_2+x_3 pass), dim_x = 2 with the fused v_1+v_2 pass (odd flips again).
+    fuse_v = 2: these small grids are below the auto rule's size."""
     g, o = pair_of_cfg(P, cfg)
     g.set_option("graph", 0)
+    g.set_option("fuse_v", fuse_v)
     f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
     fa, fb = f0.to(g.device).contiguous(), f0.to(g.device).contiguous()
     n0 = g.launch_count()
@@ -450,7 +455,8 @@ def test_steps_equals_repeated_step_bitwise(P, cfg, n):
     g.steps(fb, cfg["dt"], n)
     n2 = g.launch_count()
     assert torch.equal(fa, fb)
-    if cfg["dim_x"] == 3 and n >= 2:
+    odd_v_flips = (cfg["dim_x"] == 3) == (fuse_v == 0)
+    if odd_v_flips and n >= 2:
         assert n2 - n1 < n1 - n0                                    # fewer passes
     else:
         assert n2 - n1 == n1 - n0
