@@ -590,7 +590,7 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         if ((r = vtable_into(c, &p, 1, c->vS2, c->vAB2))) return r;
         ShiftTable t2 = tabs[1];
         t2.S = c->vS2; t2.AB = c->vAB2;
-        sldg_ev_begin(c, KIND_FUSED, 100 + c->dx);             // axis field >= 100: fused pass over axes a, a+1
+        sldg_ev_begin(c, KIND_FUSEDV, c->dx);                  // axis field: first of the two fused axes
         cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
                                             : sldg_launch_sweep_fusedv_f64(c, *cur, *oth, tabs[0], t2);
         sldg_ev_end(c);
@@ -976,7 +976,8 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
         if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
             c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
-            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2, a0 = r.axis >= 100 ? r.axis - 100 : 0; for (int a = a0; a < a0 + nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
+            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2; for (int a = 0; a < nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
+            if (r.kind == KIND_FUSEDV) { for (int a = r.axis; a < r.axis + 2; a++) { c->a_launch[a]++; c->a_ms[a] += t / 2; } }
         }
         c->ev_free.push_back(r);
     }
