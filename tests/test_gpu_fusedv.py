@@ -162,3 +162,29 @@ def test_steps_with_and_without_fused_v_agree_bitwise(P, cfg, n):
     assert outs[1][1] <= outs[0][1] and outs[2][1] <= outs[3][1]
     if n >= 3 or cfg["dim_x"] == 3:
         assert outs[2][1] < outs[3][1]
+
+
+@pytest.mark.parametrize("geom", [(2, 2, [5, 3, 7, 4], 1), (2, 2, [6, 4, 5, 3], 2), (3, 3, [4, 3, 5, 3, 4, 2], 1)],
+                         ids=lambda g: f"{g[0]}x{g[1]}v-k{g[3]}")
+def test_fused_v_pass_stays_inside_the_field(P, geom):
+    """Canary bands around the caller's f (compute-sanitizer is not available on the GPU pool): the fused pass, whose
+    ragged last x tile is zero-filled by the tensor copy and whose stores are predicated per thread, must not touch a
+    byte outside f; an out-of-range store into the workspace copy would break the bitwise plan equivalence above."""
+    dx, dv, cells, k = geom
+    g, o = make_pair(P, dx, dv, cells, k)
+    g.set_option("fuse_v", 2); g.set_option("graph", 0)
+    n = int(np.prod(o.shape))
+    guard = 4096
+    big = torch.full((n + 2 * guard,), float("nan"), dtype=torch.float64, device=g.device)
+    f = big[guard:guard + n].view(o.shape)
+    f0 = W.random_field(o.shape, seed=3)
+    f.copy_(f0)
+    E = W.random_E(dx, o.xshape, seed=9, amplitude=25.0).to(g.device)
+    g.advect_v(f, E, 0.1)
+    g.steps(f, 0.05, 3)
+    assert bool(torch.isnan(big[:guard]).all()) and bool(torch.isnan(big[guard + n:]).all())
+    assert bool(torch.isfinite(f).all())
+    want = o.advect_v(f0.numpy(), E.cpu().numpy(), 0.1)
+    for _ in range(3):
+        want, _, _ = o.step(want, 0.05)
+    assert rel_inf(f.cpu().numpy(), want) <= 1e-10
