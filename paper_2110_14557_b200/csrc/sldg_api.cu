@@ -566,8 +566,10 @@ static bool fusedv_possible(const sldg_ctx* c)
     if (!(c->prec == SLDG_F32 ? sldg_fusedv_shape_f32(c, &wx, nullptr) : sldg_fusedv_shape_f64(c, &wx, nullptr))) return false;
     if (c->opt_fuse_v == 2) return true;
     // single precision: a thread moves half the bytes per row for the same per-row work, and the tile rows shrink to
-    // 32-64 bytes; measured (cfg2/4/5) the pass is then no faster than two walks: not planned automatically
-    if (c->prec == SLDG_F32) return false;
+    // 32-64 bytes.  Measured: a small loss for dim_x = 2 (cfg2 7.73 against 7.66 ms per step), a small gain for dim_x = 3
+    // (cfg4 35.4 against 36.4, cfg5 57.7 against 59.3: the even number of v flips also lets every x half step of a
+    // single step be the one-pass x_1+x_2+x_3 sweep)
+    if (c->prec == SLDG_F32 && c->dx < 3) return false;
     // auto: a block walks all of v_2 serially, so the pass pays only when its independent walks (x tiles times planes
     // above v_2) fill the GPU; small problems (BASELINE config 1: 16 tiles) are faster with two wide walk launches
     const long long walks = ((c->X + wx - 1) / wx) * (c->V / (c->D[c->dx] * c->D[c->dx + 1]));

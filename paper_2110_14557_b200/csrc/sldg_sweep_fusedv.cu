@@ -9,7 +9,8 @@
 //   the x node, so a thread that owns one x node keeps A_1, B_1, A_2, B_2 of that node in registers.
 //   A block owns a tile of WX consecutive x nodes and ALL of v_1, and walks along v_2 (and on through `ppb`
 //   consecutive planes: the rows of a tile are one arithmetic sequence in memory, and the tables do not change).
-//   One 3-d TMA tensor copy (box WX x D_1 x 1) per v_2 row brings [D_1][WX] into a ring of shared-memory stages;
+//   One 3-d TMA tensor copy (box WX x D_1 x RPS; RPS = k+1 rows = a whole v_2 cell at k <= 1, one row at k = 2) brings
+//   [RPS][D_1][WX] into a slot of a ring of shared-memory stages;
 //   thread 0 issues them between its own rows (two rows behind the consumers' releases, so it rarely waits),
 //   full/empty mbarriers pace the ring, no __syncthreads in the loop.
 //   A thread owns one (x node, v_1 cell): per v_2 row it reads the k+1 rows of its two v_1 donor cells from shared
@@ -63,6 +64,9 @@ template <int K1> struct FVTraits {
     // tables in registers the kernel spills (ncu: a third of the issue slots stalled on local loads).
     static constexpr bool T2S = (K1 >= 3);
     static constexpr int PAD = 2 * K1 * K1 + 4;
+    // v_2 rows per tensor copy (= per ring slot).  Measured: a whole cell per copy is faster at k = 1 (cfg3 3.6 -> 3.0 ms:
+    // half the barrier traffic), a row per copy at k = 2 (cfg2 4.3 against 5.0 ms with 36 KB copies).
+    static constexpr int RPS = (K1 == 3) ? 1 : K1;
 };
 
 template <int K1>
@@ -73,6 +77,7 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     constexpr bool KEEP = FVTraits<K1>::KEEP;
     constexpr bool T2S = FVTraits<K1>::T2S;
     constexpr int PAD = FVTraits<K1>::PAD;
+    constexpr int RPS = FVTraits<K1>::RPS, SPC = K1 / RPS;             // rows per ring slot, slots per v_2 cell
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const int ST = P.stages, WX = P.WX, N1 = P.N1, N2 = P.N2;
     const int D1 = N1 * K1, D2 = N2 * K1;
@@ -89,8 +94,8 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     const long long q0 = (long long)chunk * P.ppb;
     const int nq = (int)min((long long)P.ppb, P.planes - q0);
     const long long x0 = (long long)tile * WX;
-    const int RP = D2 + (KEEP ? 0 : K1);                                // rows streamed per plane
-    const int total = nq * RP;
+    const int CPP = N2 + (KEEP ? 0 : 1);                                // v_2 cells streamed per plane
+    const int total = nq * CPP * SPC;                                   // ring slots this block streams
 
     if (t == 0) {
         for (int s = 0; s < ST; s++) { mbar_init(full_s + 8u * s, 1); mbar_init(empty_s + 8u * s, NTR / 32); }
@@ -98,18 +103,19 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     }
     __syncthreads();
 
-    // ---------------- producer (thread 0, between its own rows): one tensor copy per v_2 row
-    const uint32_t row_bytes = (uint32_t)D1 * (uint32_t)WX * (uint32_t)sizeof(real);
-    int pst = 0, pn = 0, pr = 0, pi = 0;
+    // ---------------- producer (thread 0, between its own rows): one tensor copy (box WX x D_1 x RPS) per ring slot
+    const uint32_t slot_bytes = (uint32_t)RPS * (uint32_t)D1 * (uint32_t)WX * (uint32_t)sizeof(real);
+    int pst = 0, pn = 0, pc = 0, psub = 0, pi = 0;
     long long prow0 = q0 * D2;                                          // first row of the producer's current plane
     auto produce = [&]() {
         if (pi >= total) return;
         if (pn > 0) mbar_wait(empty_s + 8u * pst, (uint32_t)((pn - 1) & 1));
-        mbar_expect_tx(full_s + 8u * pst, row_bytes);
-        const int rr = (pr >= D2) ? pr - D2 : pr;                       // k = 2: rows 0..k of the plane once more
-        tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + rr), full_s + 8u * pst);
+        mbar_expect_tx(full_s + 8u * pst, slot_bytes);
+        const int cc = (pc >= N2) ? 0 : pc;                             // k = 2: cell 0 of the plane once more
+        tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + cc * K1 + psub * RPS),
+                    full_s + 8u * pst);
         if (++pst == ST) { pst = 0; pn++; }
-        if (++pr == RP) { pr = 0; prow0 += D2; }
+        if (++psub == SPC) { psub = 0; if (++pc == CPP) { pc = 0; prow0 += D2; } }
         pi++;
     };
     if (t == 0)
@@ -168,26 +174,37 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
 
     auto body = [&](auto cpt) {
         constexpr bool CP = decltype(cpt)::value;
-        // one v_2 row of the ring -> the k+1 v_1-swept values of this thread's cell
-        auto swept_row = [&](real* g) {
-            if (t == 0) produce();
-            mbar_wait(fbar, ph);
-            real a[K1], b[K1];
+        // one v_2 cell of the ring -> the v_1-swept (k+1)^2 block [j2][j1] of this thread's v_1 cell
+        auto swept_cell = [&](real* g) {
+            const int rowvals = D1 * WX;
 #pragma unroll
-            for (int m = 0; m < K1; m++) { a[m] = pa0[soff + m * WX]; b[m] = pb0[soff + m * WX]; }
-            __syncwarp();
-            if (warp_lead) mbar_arrive(fbar + 8u * (uint32_t)ST);
+            for (int j2 = 0; j2 < K1; j2++) {
+                const int jr = j2 % RPS;                                // row inside the ring slot
+                if (jr == 0) {
+                    if (t == 0) produce();
+                    mbar_wait(fbar, ph);
+                }
+                real a[K1], b[K1];
 #pragma unroll
-            for (int j = 0; j < K1; j++) {
-                real acc = 0;
+                for (int m = 0; m < K1; m++) { a[m] = pa0[soff + jr * rowvals + m * WX]; b[m] = pb0[soff + jr * rowvals + m * WX]; }
+                if (jr == RPS - 1) {                                    // the slot is read: hand it back
+                    __syncwarp();
+                    if (warp_lead) mbar_arrive(fbar + 8u * (uint32_t)ST);
+                }
 #pragma unroll
-                for (int m = 0; m < K1; m++) acc += A1[j * K1 + m] * a[m];
+                for (int j = 0; j < K1; j++) {
+                    real acc = 0;
 #pragma unroll
-                for (int m = 0; m < K1; m++) acc += B1[j * K1 + m] * b[m];
-                g[j] = (CP && cp1) ? a[j] : acc;
+                    for (int m = 0; m < K1; m++) acc += A1[j * K1 + m] * a[m];
+#pragma unroll
+                    for (int m = 0; m < K1; m++) acc += B1[j * K1 + m] * b[m];
+                    g[j2 * K1 + j] = (CP && cp1) ? a[j] : acc;
+                }
+                if (jr == RPS - 1) {
+                    st++; soff += stage_vals; fbar += 8u;
+                    if (st == ST) { st = 0; soff = 0; fbar = full_s; ph ^= 1u; }
+                }
             }
-            st++; soff += stage_vals; fbar += 8u;
-            if (st == ST) { st = 0; soff = 0; fbar = full_s; ph ^= 1u; }
         };
         // output cell *o <- A_2 nxt + B_2 prev   (blocks are [j2][j1])
         auto emit = [&](real* o, const real (&nxt)[NN], const real (&prev)[NN]) {
@@ -227,8 +244,7 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
             real u[2][NN], first[KEEP ? NN : 1];
             auto get = [&](real (&dst)[NN], int jc) {                  // v_1-swept block of v_2 cell jc (N_2 = cell 0 again)
                 if (!KEEP || jc < N2) {
-#pragma unroll
-                    for (int j2 = 0; j2 < K1; j2++) swept_row(&dst[j2 * K1]);
+                    swept_cell(dst);
                 } else {
 #pragma unroll
                     for (int m = 0; m < NN; m++) dst[m] = first[KEEP ? m : 0];
@@ -335,12 +351,13 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     P.fout = static_cast<real*>(fout);
     P.X = c->X; P.planes = planes; P.N1 = c->cells[a1]; P.N2 = c->cells[a2]; P.WX = wx;
     P.ntiles = (int)((c->X + wx - 1) / wx);
-    P.stage_bytes = (uint32_t)((D1 * wx * sizeof(real) + 1023) / 1024 * 1024);
+    const int rps = K1 == 3 ? 1 : K1;                                   // FVTraits<K1>::RPS
+    P.stage_bytes = (uint32_t)(((size_t)rps * D1 * wx * sizeof(real) + 1023) / 1024 * 1024);
     // ring depth: about opt_fv_inflight bytes in flight per SM
     const size_t regs_blocks = (K1 <= 2) ? (size_t)(65536 / 96) / threads : 1;
     size_t bps = regs_blocks < 1 ? 1 : regs_blocks;
     if (bps > 4) bps = 4;
-    int stages = c->opt_fv_stages > 0 ? c->opt_fv_stages : (int)((size_t)c->opt_fv_inflight / bps / P.stage_bytes);
+    int stages = c->opt_fv_stages > 0 ? c->opt_fv_stages : (int)((size_t)c->opt_fv_inflight * (K1 <= 2 ? 4 : 3) / 3 / bps / P.stage_bytes);   // measured: 96 KB at k <= 1, 72 KB at k = 2
     if (stages < 3) stages = 3;
     if (stages > 24) stages = 24;
     auto smem_of = [&](int st) { return (size_t)st * P.stage_bytes + 16 * (size_t)st + (size_t)wx * (2 * K1 * K1 + 4) * sizeof(real) + 128; };
@@ -360,7 +377,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     CUtensorMap tm;
     const cuuint64_t gdim[3] = {(cuuint64_t)c->X, (cuuint64_t)D1, (cuuint64_t)rows};
     const cuuint64_t gstr[2] = {(cuuint64_t)c->X * sizeof(real), (cuuint64_t)c->X * D1 * sizeof(real)};
-    const cuuint32_t box[3] = {(cuuint32_t)wx, (cuuint32_t)D1, 1u};
+    const cuuint32_t box[3] = {(cuuint32_t)wx, (cuuint32_t)D1, (cuuint32_t)rps};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUtensorMapDataType dt = sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     const CUtensorMapL2promotion l2 = c->opt_fv_l2 == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
