@@ -129,7 +129,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
-    c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2;
+    c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
@@ -707,6 +707,29 @@ extern "C" int sldg_sipg_matrices(int degree, double sigma, double* hostM, doubl
     return SLDG_OK;
 }
 
+// Two consecutive x half steps with the same time increment (the second of a Strang step and the first of the next
+// one) as ONE pass of the fused cell kernel applying the sweep pair twice (sldg_sweep_fused_cell.cu, DBL).
+static bool x_double_possible(const sldg_ctx* c)
+{
+    if (!c->opt_x_double || !c->opt_fuse_x || c->dx != 2 || c->K1 > 3 || c->opt_fused_impl == 2) return false;
+    if (c->cells[0] > 128 || ((c->K1 * c->D[0] * (long long)c->esize) & 15)) return false;
+    return (size_t)(2 + 1) * c->K1 * c->D[0] * c->esize + (size_t)2 * 2 * c->K1 * c->D[0] * c->esize + 64 <= 227 * 1024;
+}
+static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
+{
+    ShiftTable tabs[3];
+    int r = build_x_tables(c, tau, tabs);
+    if (r) return r;
+    sldg_ev_begin(c, KIND_FUSED, 4);                           // axis field 4: the pair twice (4 sweeps)
+    cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1])
+                                        : sldg_launch_sweep_fused_cell2_f64(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+    sldg_ev_end(c);
+    c->launches++;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+    double* t = *cur; *cur = *oth; *oth = t;
+    return SLDG_OK;
+}
+
 // passes over f of one Strang step whose total number of buffer flips has parity `flip_total`; *p1 = flip parity of
 // the first x half step that achieves it
 static int step_cost(const sldg_ctx* c, bool flip_total, int* p1)
@@ -813,6 +836,21 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
     ShiftTable tabs[3];
     if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;      // fills tab_safe, which the plans depend on
     double *cur = f, *oth = c->f2;
+    if (nsteps >= 2 && x_double_possible(c)) {
+        // x(dt/2) | rho, E, v(dt) | x(dt/2) x(dt/2) as one pass | rho, E, v(dt) | ... | x(dt/2): the same sweeps in the
+        // same order as nsteps single steps.  The last half step restores the buffer parity.
+        if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, true))) return r;
+        for (int s = 0; s < nsteps; s++) {
+            if ((r = sldg_density(c, cur, c->rho))) return r;
+            if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
+            if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;
+            if (s < nsteps - 1) r = advect_x_double(c, &cur, &oth, dt / 2.0);
+            else r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f);
+            if (r) return r;
+        }
+        if (cur != f) return copy_back(c, f, cur);              // unreachable by construction
+        return SLDG_OK;
+    }
     for (int s = 0; s < nsteps; s++) {
         bool flip;
         if (s == nsteps - 1) flip = (cur != f);                 // the last step ends in f
@@ -981,7 +1019,7 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
         if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
             c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
-            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2; for (int a = 0; a < nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
+            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2, rep = r.axis == 4 ? 2 : 1; for (int a = 0; a < nf; a++) { c->a_launch[a] += rep; c->a_ms[a] += t / nf; } }
             if (r.kind == KIND_FUSEDV) { for (int a = r.axis; a < r.axis + 2; a++) { c->a_launch[a]++; c->a_ms[a] += t / 2; } }
         }
         c->ev_free.push_back(r);
@@ -1019,6 +1057,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "cell_rows")) { if (value < 0 || value > 1024) return SLDG_EINVAL; c->opt_cell_rows = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_cell_bytes = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_stages")) { if (value < 2 || value > 6) return SLDG_EINVAL; c->opt_cell_stages = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "x_double")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_double = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv_wx = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_stages")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv_stages = (int)value; return SLDG_OK; }

@@ -143,6 +143,7 @@ struct sldg_ctx {
     int opt_cell_rows;              // fused cell kernel: x_2 cells per chunk (0 = from opt_cell_bytes)
     int opt_cell_bytes;             // fused cell kernel: target bytes of one input stage (all planes of the block)
     int opt_cell_stages;            // fused cell kernel: input stages (2..6)
+    int opt_x_double;               // 1: sldg_steps merges the x half steps of consecutive Strang steps into one pass (dim_x = 2, degree <= 2)
     int opt_fuse_v;                 // v_1 and v_2 sweeps in one pass (sldg_sweep_fusedv.cu): 0 never, 1 when the shape allows and the walks fill the GPU, 2 whenever the shape allows
     int opt_fv_wx;                  // fused v kernel: x nodes per tile (0 = auto: 128-byte rows if the threads allow)
     int opt_fv_stages;              // fused v kernel: ring depth (0 = from opt_fv_inflight)
@@ -169,7 +170,9 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
     cudaError_t sldg_launch_sweep_line##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g,           \
                                             const ShiftTable& t);                                                   \
     cudaError_t sldg_launch_sweep_fused_cell##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,    \
-                                                  const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
+                                                  const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1); \
+    cudaError_t sldg_launch_sweep_fused_cell2##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,   \
+                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
 cudaError_t sldg_launch_sweep_fused3_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 cudaError_t sldg_launch_sweep_fused3_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 bool sldg_fusedv_shape_f64(const sldg_ctx* c, int* wx_out, int* threads_out);

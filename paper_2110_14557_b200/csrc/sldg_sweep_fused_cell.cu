@@ -68,7 +68,14 @@ template <int K1> struct CellV {
     }
 };
 
-template <int K1, int MINB>
+// DBL: the sweep pair is applied TWICE (x_1, x_2, x_1, x_2 with the same tables): the second x half step of a Strang
+// step followed by the first x half step of the next one (same time increment, nothing in between), in one pass.
+// The first pair's output cells go to a shared "mid" stage in the layout of an input chunk instead of to global
+// memory; after a block barrier the same threads read them as the donors of the second x_1 sweep and run a second
+// x_2 walk (its own previous / first block).  The first pair emits its cells in cyclic order starting at cell
+// s_2 + 1, which is all a periodic walk needs, so the second pair's outputs trail by one cell and the wrap cell joins
+// the last group.  Same operands and order as two launches of the single pass: bit-identical.
+template <int K1, int MINB, bool DBL>
 __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellParams P)
 {
     constexpr int NN = K1 * K1;
@@ -77,9 +84,12 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     const int PC = CR * K1 * D0;                       // doubles of one plane's chunk
     const int SS = P.PB * PC;                          // doubles of one stage
     real* const sin_ = reinterpret_cast<real*>(smem_raw);
-    real* const sout = sin_ + (size_t)ST * SS;
+    const int PCO = DBL ? (CR + 1) * K1 * D0 : PC;      // doubles of one plane's output group (DBL: + the wrap cell)
+    const int SSO = P.PB * PCO;                        // doubles of one output stage
+    real* const smid = sin_ + (size_t)ST * SS;         // DBL: the first pair's output group, read back as input
+    real* const sout = smid + (DBL ? SS : 0);
     const uint32_t sin_s = smem_u32(sin_), sout_s = smem_u32(sout);
-    const uint32_t bars_s = (smem_u32(sout + (size_t)OST * SS) + 7u) & ~7u;
+    const uint32_t bars_s = (smem_u32(sout + (size_t)OST * SSO) + 7u) & ~7u;
 
     const int t = threadIdx.x;
     const int pl = t / N0, i = t - pl * N0;
@@ -172,6 +182,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     // the x_1-swept first cell closes the periodic wrap at the end of the walk: in registers for k <= 2, parked in
     // shared memory (one column per thread, conflict free) for k = 3 where the four matrices fill the register file
     constexpr bool FS = K1 >= 4;
+    static_assert(!(DBL && K1 >= 4), "the double pass keeps both walks in registers: degree <= 2");
     real* const first_s = reinterpret_cast<real*>(smem_raw + (((size_t)(ST + OST) * SS * sizeof(real) + 8 * ST + 31) & ~(size_t)15));
     real first[FS ? 1 : NN], prev[NN];
     // chunk 0: cell 0 alone
@@ -185,8 +196,28 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     __syncthreads();
     issue_load(ST);
 
+    // output cell <- A_2 nxt + B_2 prev, its k+1 rows written at `orow` (row stride D0)
+    auto emit = [&](real* orow, const real (&nxt)[NN], const real (&prv)[NN]) {
+#pragma unroll
+        for (int j2 = 0; j2 < K1; j2++) {
+            CellV<K1> r;
+#pragma unroll
+            for (int j1 = 0; j1 < K1; j1++) {
+                real acc = 0;
+#pragma unroll
+                for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
+#pragma unroll
+                for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * prv[l * K1 + j1];
+                r.v[j1] = cp2 ? nxt[j2 * K1 + j1] : acc;
+            }
+            r.store(orow + j2 * D0);
+        }
+    };
+
     const int H = (N1 + CR - 1) / CR;                  // output groups of CR cells
-    int io0 = s2 + 1; if (io0 >= N1) io0 -= N1;        // first output cell of the group
+    int io0 = s2 + 1; if (io0 >= N1) io0 -= N1;        // first output cell of the group (of the first pair)
+    int io2 = io0 + s2 + 1; if (io2 >= N1) io2 -= N1;  // DBL: first output cell of the second pair's next group
+    real first2[DBL ? NN : 1], prev2[DBL ? NN : 1];
     for (int h = 0; h < H; h++) {
         const int j = h + 1;                           // input chunk that feeds this group
         const int st = j % ST;
@@ -194,7 +225,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         const int nout = min(CR, N1 - h * CR);
         if (nin > 0) mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
         const real* ibase = sin_ + st * SS + pl * PC;
-        real* obase = sout + (h & 1) * SS + pl * PC + i * K1;
+        real* obase = (DBL ? smid : sout + (h & 1) * SS) + pl * PC + i * K1;
         for (int e = 0; e < nout; e++) {
             real nxt[NN];
             if (e < nin) swept(ibase + e * K1 * D0, nxt);
@@ -205,43 +236,56 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
                     else nxt[m] = first[m];
                 }
             }
-#pragma unroll
-            for (int j2 = 0; j2 < K1; j2++) {
-                CellV<K1> r;
-#pragma unroll
-                for (int j1 = 0; j1 < K1; j1++) {
-                    real acc = 0;
-#pragma unroll
-                    for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
-#pragma unroll
-                    for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * prev[l * K1 + j1];
-                    r.v[j1] = cp2 ? nxt[j2 * K1 + j1] : acc;
-                }
-                r.store(obase + (e * K1 + j2) * D0);
-            }
+            emit(obase + e * K1 * D0, nxt, prev);
 #pragma unroll
             for (int m = 0; m < NN; m++) prev[m] = nxt[m];
+        }
+        int ncells = nout;                             // cells the leader stores for this group
+        if constexpr (DBL) {
+            __syncthreads();                           // the mid stage is complete, the input stage is free
+            issue_load(j + ST);
+            real* o2 = sout + (h & 1) * SSO + pl * PCO + i * K1;
+            ncells = 0;
+            for (int e = 0; e < nout; e++) {
+                real nxt2[NN];
+                swept(smid + pl * PC + e * K1 * D0, nxt2);
+                if (h == 0 && e == 0) {
+#pragma unroll
+                    for (int m = 0; m < NN; m++) first2[DBL ? m : 0] = nxt2[m];
+                } else {
+                    emit(o2 + ncells * K1 * D0, nxt2, prev2);
+                    ncells++;
+                }
+#pragma unroll
+                for (int m = 0; m < NN; m++) prev2[DBL ? m : 0] = nxt2[m];
+            }
+            if (h == H - 1) {                          // the periodic wrap of the second walk
+                emit(o2 + ncells * K1 * D0, first2, prev2);
+                ncells++;
+            }
         }
         fence_async_smem();                            // generic-proxy writes of the output stage -> async proxy
         if (leader) bulk_wait_read<0>();               // the store of group h-1 has left its output stage
         __syncthreads();
-        if (leader) {
-            const uint32_t src = sout_s + (uint32_t)((h & 1) * SS + pl * PC) * (uint32_t)sizeof(real);
-            const int n1 = min(nout, N1 - io0);
-            bulk_store(gout + (long long)io0 * K1 * D0, src, (uint32_t)n1 * cell_bytes);
-            if (nout > n1) bulk_store(gout, src + (uint32_t)n1 * cell_bytes, (uint32_t)(nout - n1) * cell_bytes);
+        if (leader && ncells > 0) {
+            const uint32_t src = sout_s + (uint32_t)((h & 1) * SSO + pl * PCO) * (uint32_t)sizeof(real);
+            const int ofirst = DBL ? io2 : io0;
+            const int n1 = min(ncells, N1 - ofirst);
+            bulk_store(gout + (long long)ofirst * K1 * D0, src, (uint32_t)n1 * cell_bytes);
+            if (ncells > n1) bulk_store(gout, src + (uint32_t)n1 * cell_bytes, (uint32_t)(ncells - n1) * cell_bytes);
             bulk_commit();
         }
-        issue_load(j + ST);
+        if constexpr (!DBL) issue_load(j + ST);
         io0 += CR; if (io0 >= N1) io0 -= N1;
+        io2 += ncells; if (io2 >= N1) io2 -= N1;
     }
     if (leader) bulk_wait_read<0>();                   // shared memory must outlive the bulk stores reading it
 }
 
-template <int K1, int MINB>
+template <int K1, int MINB, bool DBL>
 cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem)
 {
-    auto kern = sweep_fused_cell_kernel<K1, MINB>;
+    auto kern = sweep_fused_cell_kernel<K1, MINB, DBL>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long grid = (P.planes + P.PB - 1) / P.PB;
@@ -254,14 +298,15 @@ cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem)
 
 // g0, g1: geometry of axis 0 and axis 1.  Returns cudaErrorNotSupported when the shape does not fit (the caller
 // falls back to the node-per-thread fused kernel, then to separate sweeps).
-cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,
-                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+static cudaError_t launch_cell(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0, const SweepGeom& g1,
+                               const ShiftTable& t0, const ShiftTable& t1, bool dbl)
 {
     if (g1.outer == 0) return cudaSuccess;
     const long long D0 = (long long)g0.N * g0.K1, D1 = (long long)g1.N * g1.K1;
     const int K1 = g0.K1;
     if (fin == fout || g1.inner != D0 || g0.mode != 0 || g1.mode != 0 || g0.sdiv % D1 != 0) return cudaErrorNotSupported;
     if (K1 > 4 || (((long long)K1 * D0 * sizeof(real)) & 15) || g0.N > 128) return cudaErrorNotSupported;
+    if (dbl && K1 > 3) return cudaErrorNotSupported;
     if ((((uintptr_t)fin) | ((uintptr_t)fout)) & 15) return cudaErrorNotSupported;
     CellParams P;
     P.fin = static_cast<const real*>(fin); P.fout = static_cast<real*>(fout); P.planes = g1.outer;
@@ -278,6 +323,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin,
     int stages = c->opt_cell_stages;
     const size_t smem_max = 227 * 1024;
     auto smem_of = [&](long long pb, long long cr, int st) {
+        if (dbl) return (size_t)(st + 1) * pb * cr * cellb + (size_t)OST * pb * (cr + 1) * cellb + 8 * st + 48;
         return (size_t)(st + OST) * pb * cr * cellb + 8 * st + 48 + (K1 >= 4 ? (size_t)pb * g0.N * K1 * K1 * sizeof(real) : 0);
     };
     while (smem_of(PB, CR, stages) > smem_max && CR > 1) CR--;
@@ -290,11 +336,32 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin,
     P.t0 = t0; P.t1 = t1;
     const int threads = (int)(PB * g0.N);
     const size_t smem = smem_of(PB, CR, stages);
+    if (dbl) {
+        switch (K1) {
+        case 1: return launch<1, 4, true>(c, P, threads, smem);
+        case 2: return launch<2, 4, true>(c, P, threads, smem);
+        case 3: return launch<3, 2, true>(c, P, threads, smem);
+        }
+        return cudaErrorNotSupported;
+    }
     switch (K1) {
-    case 1: return launch<1, 4>(c, P, threads, smem);
-    case 2: return launch<2, 4>(c, P, threads, smem);
-    case 3: return launch<3, 3>(c, P, threads, smem);
-    case 4: return launch<4, 2>(c, P, threads, smem);
+    case 1: return launch<1, 4, false>(c, P, threads, smem);
+    case 2: return launch<2, 4, false>(c, P, threads, smem);
+    case 3: return launch<3, 3, false>(c, P, threads, smem);
+    case 4: return launch<4, 2, false>(c, P, threads, smem);
     }
     return cudaErrorNotSupported;
+}
+
+cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,
+                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+{
+    return launch_cell(c, fin, fout, g0, g1, t0, t1, false);
+}
+
+// The sweep pair applied twice (x_1, x_2, x_1, x_2) in one pass: two consecutive x half steps with the same tables.
+cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell2)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,
+                                                    const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+{
+    return launch_cell(c, fin, fout, g0, g1, t0, t1, true);
 }

@@ -1,0 +1,95 @@
+"""GPU tests of the double x half step (sweep_fused_cell_kernel<..., DBL>; inside a run of Strang steps the
+second x half step of a step is followed directly by the first x half step of the next one, with the same time
+increment).  `sldg_steps` runs the two as one pass that applies the sweep pair twice in the order x_1, x_2, x_1, x_2:
+same operands and order as two passes, so the result must be BIT-IDENTICAL to the plan without it (and to repeated
+`sldg_step` calls), and match the oracle within the 10-step bar.
+"""
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from oracle import oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+def rel_inf(g, o):
+    return float(np.abs(g.astype(np.float64) - o.astype(np.float64)).max() / np.abs(o).max())
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2110_14557_b200 as pkg
+    if not torch.cuda.is_available():
+        pytest.fail("gpu test without a CUDA device")
+    return pkg
+
+
+def dom_of(dx, dv):
+    dom = []
+    for a in range(dx + dv):
+        dom += [0.0, 1.0 + a] if a < dx else [-2.0 - a, 2.0 + a]
+    return dom
+
+
+# (dim_x, dim_v, cells, degree)
+XD_GEOMS = [
+    (2, 2, [6, 5, 4, 3], 1),
+    (2, 2, [8, 7, 3, 4], 2),          # 7 x_2 cells: ragged groups
+    (2, 2, [4, 1, 3, 2], 1),          # a single x_2 cell: every donor is the cell itself
+    (2, 2, [4, 2, 2, 3], 2),          # two x_2 cells
+    (2, 2, [8, 9, 3, 2], 0),          # degree 0 (D_0 = 8: bulk-copy rule holds)
+    (2, 3, [6, 4, 3, 2, 2], 1),       # 2x3v
+    (2, 2, [64, 5, 2, 2], 2),         # D_0 = 192 as in BASELINE cfg2
+    (2, 2, [6, 5, 4, 3], 3),          # degree 3: no double pass (registers) -> plain plan
+    (2, 2, [5, 4, 3, 2], 0),          # D_0 = 5: rows not a multiple of 16 B -> plain plan
+]
+
+
+@pytest.mark.parametrize("geom", XD_GEOMS, ids=lambda g: f"{g[0]}x{g[1]}v-{'x'.join(map(str, g[2]))}-k{g[3]}")
+@pytest.mark.parametrize("dt", [0.05, 0.9])                     # |x shift| < 1 cell / up to ~10 cells (wraps)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_steps_with_double_x_pass_are_bitwise_the_plain_plan(P, geom, dt, prec):
+    dx, dv, cells, k = geom
+    dom = dom_of(dx, dv)
+    o = O.Oracle(dx, dv, cells, k, dom, threads=O.lib().orc_max_threads())
+    f0 = W.random_field(o.shape, seed=41 + k)
+    if prec == "f32":
+        f0 = f0.to(torch.float32)
+    outs = []
+    # (x_double, fuse_v, cell_rows, cell_threads, nsteps)
+    for xd, fv, rows, thr, n in ((0, 0, 0, 64, 4), (1, 0, 0, 64, 4), (1, 2, 1, 128, 4), (1, 2, 3, 32, 4), (1, 0, 2, 64, 4)):
+        g = P.Sldg(dx, dv, cells, k, dom, precision=prec)
+        g.set_option("graph", 0); g.set_option("x_double", xd); g.set_option("fuse_v", fv)
+        g.set_option("cell_rows", rows); g.set_option("cell_threads", thr)
+        fg = f0.to(g.device).contiguous()
+        n0 = g.launch_count()
+        g.steps(fg, dt, n)
+        outs.append((fg.cpu().numpy(), g.launch_count() - n0))
+    for x, _ in outs[1:]:
+        assert np.array_equal(outs[0][0], x)
+    doubled = k <= 2 and (cells[0] * (k + 1) * (k + 1) * (8 if prec == "f64" else 4)) % 16 == 0
+    if doubled:
+        assert outs[1][1] < outs[0][1]                              # the merged passes really ran
+    else:
+        assert outs[1][1] == outs[0][1]
+    if prec == "f64":
+        want = f0.numpy()
+        for _ in range(4):
+            want, _, _ = o.step(want, dt)
+        assert rel_inf(outs[0][0], want) <= 1e-10
+
+
+@pytest.mark.parametrize("n", [2, 3, 5])
+def test_steps_equal_repeated_single_steps_with_the_double_pass(P, n):
+    cfg = W.scaled(W.CONFIGS[1], [12, 10, 8, 8])
+    o = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], threads=1)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    g.set_option("graph", 0)
+    fa, fb = f0.to(g.device).contiguous(), f0.to(g.device).contiguous()
+    for _ in range(n):
+        g.step(fa, cfg["dt"])
+    g.steps(fb, cfg["dt"], n)
+    assert torch.equal(fa, fb)
