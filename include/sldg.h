@@ -178,11 +178,12 @@ int sldg_advect_axis(sldg_ctx* ctx, double* f, int axis, const double* delta_hos
  * With timing on, every kernel launch is bracketed by CUDA events on the context's stream.
  * Kinds: 0 = sweep along axis 0 (TMA/SMEM kernel), 1 = sweep along a slow axis, 2 = rho,
  * 3 = Poisson/E, 4 = shift tables, 5 = copies, 6 = fused x pass (x_1+x_2, or x_1+x_2+x_3 for dim_x = 3, in one
- * launch), 7 = fused v_1+v_2 pass (one launch); the per-axis figures of sldg_timing_axis book an equal share of a
+ * launch), 7 = fused v_1+v_2 pass (one launch), 8 = double x half step (x_1+x_2 applied twice in one launch, inside
+ * sldg_steps); the per-axis figures of sldg_timing_axis book an equal share of a
  * fused launch's time on each of its axes.  sldg_timing_read synchronises, adds the elapsed
  * times of all events recorded since the last read, and returns per kind the number of launches
  * and the total milliseconds (arrays of SLDG_NKINDS entries, host). */
-#define SLDG_NKINDS 8
+#define SLDG_NKINDS 9
 int sldg_timing_enable(sldg_ctx* ctx, int on);
 int sldg_timing_read(sldg_ctx* ctx, long long* launches, double* ms);
 /* total kernel launches enqueued by this context since creation */

@@ -9,9 +9,9 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = "libsldg_b200.so"
 
-NKINDS = 8
+NKINDS = 9
 MAX_DIM = 6
-KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x", "sweep_fused_v"]
+KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x", "sweep_fused_v", "sweep_fused_x_double"]
 
 _vp, _dp, _ip, _ll = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_longlong
 _llp = C.POINTER(C.c_longlong)

@@ -720,7 +720,7 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
     ShiftTable tabs[3];
     int r = build_x_tables(c, tau, tabs);
     if (r) return r;
-    sldg_ev_begin(c, KIND_FUSED, 4);                           // axis field 4: the pair twice (4 sweeps)
+    sldg_ev_begin(c, KIND_FUSEDX2, 0);
     cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1])
                                         : sldg_launch_sweep_fused_cell2_f64(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
     sldg_ev_end(c);
@@ -836,7 +836,9 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
     ShiftTable tabs[3];
     if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;      // fills tab_safe, which the plans depend on
     double *cur = f, *oth = c->f2;
-    if (nsteps >= 2 && x_double_possible(c)) {
+    // n - 1 merged passes save n - 1 passes over f; restoring the buffer parity at the end costs one of them back when
+    // the number of flips is odd (2 steps with an even number of v flips: nothing gained, the plain plan runs)
+    if (x_double_possible(c) && (nsteps >= 3 || (nsteps == 2 && (v_flips(c) & 1)))) {
         // x(dt/2) | rho, E, v(dt) | x(dt/2) x(dt/2) as one pass | rho, E, v(dt) | ... | x(dt/2): the same sweeps in the
         // same order as nsteps single steps.  The last half step restores the buffer parity.
         if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, true))) return r;
@@ -1019,7 +1021,8 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
         if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
             c->t_launch[r.kind]++; c->t_ms[r.kind] += t;
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
-            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2, rep = r.axis == 4 ? 2 : 1; for (int a = 0; a < nf; a++) { c->a_launch[a] += rep; c->a_ms[a] += t / nf; } }
+            if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2; for (int a = 0; a < nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
+            if (r.kind == KIND_FUSEDX2) { for (int a = 0; a < 2; a++) { c->a_launch[a] += 2; c->a_ms[a] += t / 2; } }   // four sweeps
             if (r.kind == KIND_FUSEDV) { for (int a = r.axis; a < r.axis + 2; a++) { c->a_launch[a]++; c->a_ms[a] += t / 2; } }
         }
         c->ev_free.push_back(r);

@@ -457,7 +457,8 @@ def test_steps_equals_repeated_step_bitwise(P, cfg, n, fuse_v):
     assert torch.equal(fa, fb)
     odd_v_flips = (cfg["dim_x"] == 3) == (fuse_v == 0)
     # dim_x = 2: sldg_steps also merges the x half steps of consecutive steps into one pass (tests/test_gpu_xdouble.py)
-    if (odd_v_flips or cfg["dim_x"] == 2) and n >= 2:
+    merged = cfg["dim_x"] == 2 and (n >= 3 or (n == 2 and fuse_v == 2))
+    if (odd_v_flips and n >= 2) or merged:
         assert n2 - n1 < n1 - n0                                    # fewer passes
     else:
         assert n2 - n1 == n1 - n0
