@@ -38,7 +38,7 @@ using namespace sldg_async;
 struct FVParams {
     real* fout;
     long long X, planes;
-    int N1, N2, WX, stages, ppb, ntiles;
+    int N1, N2, WX, stages, ppb, ntiles, cps;
     uint32_t stage_bytes;         // ring slot stride (>= D_1 * WX * sizeof(real), multiple of 128)
     ShiftTable t1, t2;
 };
@@ -95,7 +95,10 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     const int nq = (int)min((long long)P.ppb, P.planes - q0);
     const long long x0 = (long long)tile * WX;
     const int CPP = N2 + (KEEP ? 0 : 1);                                // v_2 cells streamed per plane
-    const int total = nq * CPP * SPC;                                   // ring slots this block streams
+    // k <= 1: a ring slot holds `cps` whole v_2 cells; the block's cells are one run of rows, so the last slot may reach
+    // past it (into the next plane, or zero-filled past the end of f) and is simply not read to the end
+    const int cps = (RPS == K1) ? P.cps : 1;
+    const int total = (RPS == K1) ? (nq * CPP + cps - 1) / cps : nq * CPP * SPC;   // ring slots this block streams
 
     if (t == 0) {
         for (int s = 0; s < ST; s++) { mbar_init(full_s + 8u * s, 1); mbar_init(empty_s + 8u * s, NTR / 32); }
@@ -104,18 +107,23 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     __syncthreads();
 
     // ---------------- producer (thread 0, between its own rows): one tensor copy (box WX x D_1 x RPS) per ring slot
-    const uint32_t slot_bytes = (uint32_t)RPS * (uint32_t)D1 * (uint32_t)WX * (uint32_t)sizeof(real);
+    const uint32_t slot_bytes = (uint32_t)(RPS * cps) * (uint32_t)D1 * (uint32_t)WX * (uint32_t)sizeof(real);
     int pst = 0, pn = 0, pc = 0, psub = 0, pi = 0;
     long long prow0 = q0 * D2;                                          // first row of the producer's current plane
     auto produce = [&]() {
         if (pi >= total) return;
         if (pn > 0) mbar_wait(empty_s + 8u * pst, (uint32_t)((pn - 1) & 1));
         mbar_expect_tx(full_s + 8u * pst, slot_bytes);
-        const int cc = (pc >= N2) ? 0 : pc;                             // k = 2: cell 0 of the plane once more
-        tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + cc * K1 + psub * RPS),
-                    full_s + 8u * pst);
+        if constexpr (RPS == K1) {
+            tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + (long long)pi * (K1 * cps)),
+                        full_s + 8u * pst);
+        } else {
+            const int cc = (pc >= N2) ? 0 : pc;                         // k = 2: cell 0 of the plane once more
+            tma_load_3d(ring_s + (uint32_t)pst * P.stage_bytes, &tmap, (int)x0, 0, (int)(prow0 + cc * K1 + psub * RPS),
+                        full_s + 8u * pst);
+            if (++psub == SPC) { psub = 0; if (++pc == CPP) { pc = 0; prow0 += D2; } }
+        }
         if (++pst == ST) { pst = 0; pn++; }
-        if (++psub == SPC) { psub = 0; if (++pc == CPP) { pc = 0; prow0 += D2; } }
         pi++;
     };
     if (t == 0)
@@ -169,6 +177,7 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     const long long rowX = (long long)D1 * X;                          // one v_2 row of a plane, in values
     const long long cellX = (long long)K1 * rowX, planeX = (long long)D2 * rowX;
 
+    int csub = 0;                                                      // cell inside the current ring slot (k <= 1)
     int st = 0, soff = 0;                                              // ring slot of the next row, its offset in values
     uint32_t ph = 0, fbar = full_s;
 
@@ -179,15 +188,17 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
             const int rowvals = D1 * WX;
 #pragma unroll
             for (int j2 = 0; j2 < K1; j2++) {
-                const int jr = j2 % RPS;                                // row inside the ring slot
-                if (jr == 0) {
+                const int jr = j2 % RPS;                                // row inside the ring slot (of its cell)
+                if (jr == 0 && csub == 0) {
                     if (t == 0) produce();
                     mbar_wait(fbar, ph);
                 }
+                const int ro = soff + (csub * RPS + jr) * rowvals;
                 real a[K1], b[K1];
 #pragma unroll
-                for (int m = 0; m < K1; m++) { a[m] = pa0[soff + jr * rowvals + m * WX]; b[m] = pb0[soff + jr * rowvals + m * WX]; }
-                if (jr == RPS - 1) {                                    // the slot is read: hand it back
+                for (int m = 0; m < K1; m++) { a[m] = pa0[ro + m * WX]; b[m] = pb0[ro + m * WX]; }
+                const bool last = jr == RPS - 1 && csub == cps - 1;
+                if (last) {                                             // the slot is read: hand it back
                     __syncwarp();
                     if (warp_lead) mbar_arrive(fbar + 8u * (uint32_t)ST);
                 }
@@ -200,11 +211,12 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
                     for (int m = 0; m < K1; m++) acc += B1[j * K1 + m] * b[m];
                     g[j2 * K1 + j] = (CP && cp1) ? a[j] : acc;
                 }
-                if (jr == RPS - 1) {
+                if (last) {
                     st++; soff += stage_vals; fbar += 8u;
                     if (st == ST) { st = 0; soff = 0; fbar = full_s; ph ^= 1u; }
                 }
             }
+            if (RPS == K1) { if (++csub == cps) csub = 0; }
         };
         // output cell *o <- A_2 nxt + B_2 prev   (blocks are [j2][j1])
         auto emit = [&](real* o, const real (&nxt)[NN], const real (&prev)[NN]) {
@@ -353,7 +365,10 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     P.fout = static_cast<real*>(fout);
     P.X = c->X; P.planes = planes; P.N1 = c->cells[a1]; P.N2 = c->cells[a2]; P.WX = wx;
     P.ntiles = (int)((c->X + wx - 1) / wx);
-    const int rps = K1 == 3 ? 1 : K1;                                   // FVTraits<K1>::RPS
+    int cps = (K1 == 3) ? 1 : (c->opt_fv_cps > 0 ? c->opt_fv_cps : 1);   // v_2 cells per tensor copy (k <= 1)
+    if (cps > c->cells[a2]) cps = c->cells[a2];
+    P.cps = cps;
+    const int rps = (K1 == 3 ? 1 : K1) * cps;                           // rows per ring slot
     P.stage_bytes = (uint32_t)(((size_t)rps * D1 * wx * sizeof(real) + 1023) / 1024 * 1024);
     // ring depth: about opt_fv_inflight bytes in flight per SM
     const size_t regs_blocks = (K1 <= 2) ? (size_t)(65536 / 96) / threads : 1;

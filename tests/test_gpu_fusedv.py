@@ -56,9 +56,9 @@ FV_GEOMS = [
 
 def run_plans(g, f0, E, dt, plans):
     outs = []
-    for fuse, wx, stages, ppb, l2, _ in plans:
+    for fuse, wx, stages, ppb, l2, cps in plans:
         g.set_option("fuse_v", fuse); g.set_option("fv_wx", wx); g.set_option("fv_stages", stages)
-        g.set_option("fv_ppb", ppb); g.set_option("fv_l2", l2)
+        g.set_option("fv_ppb", ppb); g.set_option("fv_l2", l2); g.set_option("fv_cps", cps)
         fg = f0.to(g.device).contiguous()
         n0 = g.launch_count()
         g.advect_v(fg, E, dt)
@@ -66,9 +66,9 @@ def run_plans(g, f0, E, dt, plans):
     return outs
 
 
-# (fuse_v: 0 never, 1 auto, 2 whenever the shape allows; fv_wx, fv_stages, fv_ppb, fv_l2, unused)
-PLANS = ((0, 0, 0, 0, 2, 0), (2, 0, 0, 0, 2, 0), (2, 2, 3, 1, 0, 0), (2, 4, 5, 2, 1, 0), (2, 8, 2, 3, 3, 0), (2, 16, 9, 0, 2, 0),
-         (2, 0, 4, 0, 2, 0), (1, 0, 0, 0, 2, 0))
+# (fuse_v: 0 never, 1 auto, 2 whenever the shape allows; fv_wx, fv_stages, fv_ppb, fv_l2, fv_cps: v_2 cells per copy)
+PLANS = ((0, 0, 0, 0, 2, 1), (2, 0, 0, 0, 2, 1), (2, 2, 3, 1, 0, 2), (2, 4, 5, 2, 1, 3), (2, 8, 2, 3, 3, 1), (2, 16, 9, 0, 2, 4),
+         (2, 0, 4, 0, 2, 2), (1, 0, 0, 0, 2, 1))
 
 
 @pytest.mark.parametrize("geom", FV_GEOMS, ids=lambda g: f"{g[0]}x{g[1]}v-{'x'.join(map(str, g[2]))}-k{g[3]}")
@@ -124,7 +124,7 @@ def test_fused_v_single_precision_agrees_bitwise_and_matches_fp32_oracle(P, geom
     dt = 0.1
     hv = (2 * (2.0 + dx)) / cells[dx]
     E = W.random_E(dx, o.xshape, seed=6, amplitude=2.5 * hv / dt)
-    outs = run_plans(g, f0, E.to(g.device), dt, ((0, 0, 0, 0, 2, 0), (2, 0, 0, 0, 2, 0), (2, 4, 3, 1, 0, 0), (2, 8, 6, 2, 2, 0), (2, 0, 5, 0, 2, 0)))
+    outs = run_plans(g, f0, E.to(g.device), dt, ((0, 0, 0, 0, 2, 1), (2, 0, 0, 0, 2, 1), (2, 4, 3, 1, 0, 2), (2, 8, 6, 2, 2, 3), (2, 0, 5, 0, 2, 2)))
     for x, _ in outs[1:]:
         assert np.array_equal(outs[0][0], x)
     assert outs[1][1] < outs[0][1]
