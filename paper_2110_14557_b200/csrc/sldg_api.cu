@@ -576,11 +576,13 @@ static bool fusedv_possible(const sldg_ctx* c)
     return walks >= 2LL * c->sm_count;
 }
 // buffer flips of one v advection
-static int v_flips(const sldg_ctx* c) { return fusedv_possible(c) ? c->dx - 1 : c->dx; }
+static int v_flips(const sldg_ctx* c, bool fuse) { return fuse ? c->dx - 1 : c->dx; }
+static int v_flips(const sldg_ctx* c) { return v_flips(c, fusedv_possible(c)); }
 
 // v-sweeps on (*cur, *oth): v_1 and v_2 in one fused out-of-place pass when the shape allows, every other sweep a
 // slow-axis walk; each pass flips the pair.
-static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt)
+// fuse: 1 = the fused pass when the shape allows, 0 = separate walks (a plan may veto the fused pass: step_best)
+static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt, bool fuse = true)
 {
     int axes[3];
     ShiftTable tabs[3];
@@ -589,7 +591,7 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         tabs[i].S = c->vS; tabs[i].AB = c->vAB; tabs[i].strideIdx = 1; tabs[i].strideM = c->X;
     }
     VPrep p = {E, dt};
-    if (fusedv_possible(c)) {
+    if (fuse && fusedv_possible(c)) {
         int r;
         if ((r = vtable_into(c, &p, 0, c->vS, c->vAB))) return r;
         if ((r = vtable_into(c, &p, 1, c->vS2, c->vAB2))) return r;
@@ -732,15 +734,29 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
 
 // passes over f of one Strang step whose total number of buffer flips has parity `flip_total`; *p1 = flip parity of
 // the first x half step that achieves it
-static int step_cost(const sldg_ctx* c, bool flip_total, int* p1)
+static int step_cost(const sldg_ctx* c, bool flip_total, int* p1, bool fuse_v)
 {
     int best = 1 << 30;
     for (int q1 = 0; q1 < 2; q1++) {
-        const int q2 = (q1 + v_flips(c) + (flip_total ? 1 : 0)) & 1;
+        const int q2 = (q1 + v_flips(c, fuse_v) + (flip_total ? 1 : 0)) & 1;
         XPlan a = x_plan(c, q1 != 0), b = x_plan(c, q2 != 0);
         if (a.ok && b.ok && a.passes + b.passes < best) { best = a.passes + b.passes; if (p1) *p1 = q1; }
     }
     return best;
+}
+// The cheapest plan of one Strang step in tenths of a pass over f: x passes as above, v_1+v_2 as two walks (20) or as
+// the fused pass (13: measured 1.3 walk passes).  For dim_x = 2 a single step that must end in its own buffer is
+// cheaper WITHOUT the fused v pass (its odd flip would cost a two-pass in-place x half step: 43 against 40).
+static int step_best(const sldg_ctx* c, bool flip_total, int* p1, bool* fuse_v)
+{
+    int p_off = 0, p_on = 0;
+    const int off = 10 * step_cost(c, flip_total, &p_off, false) + 10 * c->dx;
+    int on = 1 << 30;
+    if (fusedv_possible(c)) on = 10 * step_cost(c, flip_total, &p_on, true) + 13 + 10 * (c->dx - 2);
+    const bool use = on < off || (c->opt_fuse_v == 2 && on < (1 << 30));       // forced: tests
+    if (p1) *p1 = use ? p_on : p_off;
+    if (fuse_v) *fuse_v = use;
+    return use ? on : off;
 }
 
 // One Strang step on the pair (*cur, *oth).  The dx v-sweeps flip the pair dx times; the two x half steps choose
@@ -753,11 +769,12 @@ static int step_core(sldg_ctx* c, double** cur, double** oth, double dt, bool fl
     ShiftTable tabs[3];
     if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;
     int p1 = 0;
-    step_cost(c, flip_total, &p1);
+    bool fuse_v = false;
+    step_best(c, flip_total, &p1, &fuse_v);
     if ((r = advect_x_impl(c, cur, oth, dt / 2.0, p1 != 0))) return r;
     if ((r = sldg_density(c, *cur, c->rho))) return r;
     if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
-    if ((r = advect_v_impl(c, cur, oth, c->E, dt))) return r;
+    if ((r = advect_v_impl(c, cur, oth, c->E, dt, fuse_v))) return r;
     const bool want_other = flip_total;                       // where the step has to end, relative to `start`
     const bool now_other = (*cur != start);
     return advect_x_impl(c, cur, oth, dt / 2.0, now_other != want_other);
@@ -856,7 +873,7 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
     for (int s = 0; s < nsteps; s++) {
         bool flip;
         if (s == nsteps - 1) flip = (cur != f);                 // the last step ends in f
-        else flip = step_cost(c, true, nullptr) < step_cost(c, false, nullptr);
+        else flip = step_best(c, true, nullptr, nullptr) < step_best(c, false, nullptr, nullptr);
         if ((r = step_core(c, &cur, &oth, dt, flip))) return r;
     }
     if (cur != f) return copy_back(c, f, cur);                  // unreachable by construction
