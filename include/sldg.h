@@ -192,6 +192,15 @@ long long sldg_launch_count(const sldg_ctx* ctx);
  * SLDG_MAX_DIM entries (host).  Filled by sldg_timing_read; this call does not synchronise. */
 int sldg_timing_axis(const sldg_ctx* ctx, long long* launches, double* ms);
 
+/* Host-only (no CUDA device needed): the plan of one sldg_step (nsteps == 0) or of sldg_steps(nsteps) for a problem
+ * of this shape, obtained by running the library's planning code with every launch replaced by a counter.
+ * shifts_below_one: 1 = every x shift is 0 or -1 cell (|v| dt/2 < h_x: slow-axis x sweeps may then run in place),
+ * fuse_v / x_double: the options of the same names (sldg_set_option).  counts (host, 6 entries) = passes over f of
+ * the x sweeps, passes of the v sweeps, rho passes, field solves, whole-array device copies, kernel launches counted
+ * by sldg_launch_count.  A fused or merged launch is ONE pass.  Returns 0 or a negative code. */
+int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
+                    int shifts_below_one, int fuse_v, int x_double, long long* counts);
+
 /* Tuning knob (affects speed only, never results): see DESIGN.md section 5. */
 int sldg_set_option(sldg_ctx* ctx, const char* name, long long value);
 

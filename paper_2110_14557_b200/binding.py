@@ -56,6 +56,8 @@ EXPORTS = {
     "sldg_cg_info": (C.c_int, [_vp, _ip, _dp]),
     "sldg_last_phi": (_vp, [_vp]),
     "sldg_sipg_matrices": (C.c_int, [C.c_int, C.c_double, _dp, _dp]),
+    "sldg_plan_query": (C.c_int, [C.c_int, C.c_int, _ip, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                  C.POINTER(C.c_longlong)]),
 }
 
 _lib = None
@@ -115,6 +117,16 @@ def sipg_matrices(degree, sigma=0.0):
     M, B = np.empty((degree + 1, degree + 1)), np.empty((degree + 1, degree + 1))
     _check(lib().sldg_sipg_matrices(int(degree), float(sigma), M.ctypes.data_as(_dp), B.ctypes.data_as(_dp)))
     return M, B
+
+
+def plan_query(dim_x, dim_v, cells, degree, nsteps, precision="f64", shifts_below_one=True, fuse_v=1, x_double=1):
+    """sldg_plan_query (host-only call): passes over f that sldg_step (nsteps == 0) / sldg_steps(nsteps) would launch.
+    -> dict(x_passes, v_passes, rho_passes, field_solves, copies, launches)"""
+    cells_c = (C.c_int * len(cells))(*[int(c) for c in cells])
+    out = (C.c_longlong * 6)()
+    _check(lib().sldg_plan_query(int(dim_x), int(dim_v), cells_c, int(degree), 1 if precision == "f32" else 0, int(nsteps),
+                                 1 if shifts_below_one else 0, int(fuse_v), int(x_double), out))
+    return dict(zip(("x_passes", "v_passes", "rho_passes", "field_solves", "copies", "launches"), [int(v) for v in out]))
 
 
 def gauss_legendre(degree):

@@ -96,7 +96,8 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
                                 int precision)
 {
     if (!out || !cells || !domain) return SLDG_EINVAL;
-    if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
+    const int dry_bit = precision & SLDG_DRY_BIT_INTERNAL;
+    if ((precision & ~SLDG_DRY_BIT_INTERNAL) != SLDG_F64 && (precision & ~SLDG_DRY_BIT_INTERNAL) != SLDG_F32) return SLDG_EINVAL;
     if (dim_x < 1 || dim_x > 3 || dim_v < dim_x || dim_v > 3) return SLDG_EINVAL;
     if (degree < 0 || degree > SLDG_MAX_DEGREE) return SLDG_EINVAL;
     const int d = dim_x + dim_v;
@@ -106,8 +107,10 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     }
     sldg_ctx* c = new (std::nothrow) sldg_ctx();
     if (!c) return SLDG_ENOMEM;
+    c->dry = false; c->dry_safe = 0; c->dry_x = c->dry_v = c->dry_rho = c->dry_field = c->dry_copies = 0;
     c->dx = dim_x; c->dv = dim_v; c->d = d; c->k = degree; c->K1 = degree + 1;
-    c->prec = precision; c->esize = precision == SLDG_F32 ? 4 : 8;
+    c->prec = precision & ~SLDG_DRY_BIT_INTERNAL; c->esize = c->prec == SLDG_F32 ? 4 : 8;
+    (void)dry_bit;
     c->nf = 1; c->X = 1; c->V = 1;
     for (int a = 0; a < d; a++) {
         c->cells[a] = cells[a];
@@ -134,6 +137,8 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
     c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
+
+    if (precision & SLDG_DRY_BIT_INTERNAL) { *out = c; return SLDG_OK; }   // sldg_plan_query: host fields only
 
     // device side: needs a CUDA device.  Without one the context is unusable -> fail loudly.
     int dev = 0;
@@ -320,6 +325,12 @@ static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scrat
 {
     SweepGeom g = geom_of(c, axis);
     cudaError_t e;
+    if (c->dry) {
+        if (g.inner != 1 && fin == fout && !inplace_walk_ok) return SLDG_EINVAL;
+        (axis < c->dx ? c->dry_x : c->dry_v)++;
+        c->launches++;
+        return SLDG_OK;
+    }
     if (g.inner == 1) {
         // contiguous lines: per-warp TMA pipelines; block-wide tiles when a line is too long for a warp's ring;
         // the (uncoalesced) register walk when it does not even fit a block's shared memory
@@ -355,6 +366,7 @@ static int run_sweep(sldg_ctx* c, const double* fin, double* fout, double* scrat
 
 static int copy_back(sldg_ctx* c, double* dst, const double* src)
 {
+    if (c->dry) { c->dry_copies++; return SLDG_OK; }
     sldg_ev_begin(c, KIND_COPY, -1);
     cudaError_t e = cudaMemcpyAsync(dst, src, (size_t)c->nf * c->esize, cudaMemcpyDeviceToDevice, c->stream);
     sldg_ev_end(c);
@@ -395,6 +407,10 @@ static int run_sweeps(sldg_ctx* c, double** cur, double** oth, const int* axes, 
 static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
 {
     const long long NN2 = 2LL * c->K1 * c->K1;
+    if (c->dry) {
+        for (int a = 0; a < c->dx; a++) { c->tab_safe[a] = c->dry_safe != 0; c->tab_anycp[a] = false; tabs[a] = ShiftTable(); }
+        return SLDG_OK;
+    }
     for (int a = 0; a < c->dx; a++) {
         const int b = c->dx + a;
         if (!c->tab_valid[a] || c->tab_tau[a] != dt) {
@@ -495,6 +511,12 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     XPlan p = x_plan(c, flip);
     if (!p.ok) return SLDG_EINVAL;          // cannot happen: the unfused plan reaches either parity
     int a = 0;
+    if (c->dry && (p.fused3 || p.fused)) {
+        c->dry_x++; c->launches++;
+        double* t = *cur; *cur = *oth; *oth = t;
+        if (p.fused3) return SLDG_OK;
+        a = 2;
+    } else
     if (p.fused3) {
         SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
         sldg_ev_begin(c, KIND_FUSED, 3);                       // axis field of a fused event = number of fused axes
@@ -507,7 +529,7 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
         double* t = *cur; *cur = *oth; *oth = t;
         return SLDG_OK;
     }
-    if (p.fused) {
+    if (p.fused && !c->dry) {
         sldg_ev_begin(c, KIND_FUSED, 0);
         cudaError_t e = cudaErrorNotSupported;
         if (c->opt_fused_impl != 2) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
@@ -543,6 +565,7 @@ struct VPrep { const double* E; double dt; };
 static int vtable_into(sldg_ctx* c, const VPrep* p, int i, int* S, double* AB)
 {
     const int a = c->dx + i;
+    if (c->dry) return SLDG_OK;
     sldg_ev_begin(c, KIND_TABLE, a);
     cudaError_t e = sldg_launch_vtable(c, p->E + (long long)i * c->X, p->dt, c->h[a], c->cells[a], S, AB);
     sldg_ev_end(c);
@@ -597,6 +620,13 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         if ((r = vtable_into(c, &p, 1, c->vS2, c->vAB2))) return r;
         ShiftTable t2 = tabs[1];
         t2.S = c->vS2; t2.AB = c->vAB2;
+        if (c->dry) {
+            c->dry_v++; c->launches++;
+            double* t = *cur; *cur = *oth; *oth = t;
+            if (c->dx == 2) return SLDG_OK;
+            VPrepOff o = {p, 2};
+            return run_sweeps(c, cur, oth, axes + 2, tabs + 2, c->dx - 2, false, vprep_off, &o);
+        }
         sldg_ev_begin(c, KIND_FUSEDV, c->dx);                  // axis field: first of the two fused axes
         cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
                                             : sldg_launch_sweep_fusedv_f64(c, *cur, *oth, tabs[0], t2);
@@ -629,6 +659,7 @@ extern "C" int sldg_density(sldg_ctx* c, const double* f, double* rho)
     int r = check_f(c, f);
     if (r) return r;
     if (!rho) return SLDG_EINVAL;
+    if (c->dry) { c->dry_rho++; return SLDG_OK; }
     sldg_ev_begin(c, KIND_RHO, -1);
     cudaError_t e = sldg_launch_density(c, f, rho);
     sldg_ev_end(c);
@@ -640,6 +671,7 @@ extern "C" int sldg_poisson(sldg_ctx* c, const double* rho, double* E)
 {
     if (!c || !rho || !E) return SLDG_EINVAL;
     if (!c->ws_ready) return SLDG_ENOWORKSPACE;
+    if (c->dry) { c->dry_field++; return SLDG_OK; }
     sldg_ev_begin(c, KIND_POISSON, -1);
     cudaError_t e = sldg_launch_poisson(c, rho, E);
     sldg_ev_end(c);
@@ -722,6 +754,7 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
     ShiftTable tabs[3];
     int r = build_x_tables(c, tau, tabs);
     if (r) return r;
+    if (c->dry) { c->dry_x++; c->launches++; double* t = *cur; *cur = *oth; *oth = t; return SLDG_OK; }
     sldg_ev_begin(c, KIND_FUSEDX2, 0);
     cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1])
                                         : sldg_launch_sweep_fused_cell2_f64(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
@@ -878,6 +911,33 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
     }
     if (cur != f) return copy_back(c, f, cur);                  // unreachable by construction
     return SLDG_OK;
+}
+
+// Host-only: run the planning code of sldg_step (nsteps == 0) or sldg_steps(nsteps) on a context without a device and
+// count what it would launch.  The same functions plan and launch (c->dry only replaces the launches), so the counts
+// are those of the real calls.
+extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
+                               int shifts_below_one, int fuse_v, int x_double, long long* counts)
+{
+    if (!counts || nsteps < 0 || fuse_v < 0 || fuse_v > 2 || x_double < 0 || x_double > 1) return SLDG_EINVAL;
+    if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
+    if (dim_x < 1 || dim_x > 3) return SLDG_EINVAL;
+    double dom[2 * SLDG_MAX_DIM];
+    for (int a = 0; a < SLDG_MAX_DIM; a++) { dom[2 * a] = 0.0; dom[2 * a + 1] = 1.0; }
+    sldg_ctx* c = nullptr;
+    int r = sldg_create_prec(&c, dim_x, dim_v, cells, degree, dom, precision | SLDG_DRY_BIT_INTERNAL);
+    if (r) return r;
+    c->dry = true; c->dry_safe = shifts_below_one; c->opt_graph = 0; c->opt_fuse_v = fuse_v; c->opt_x_double = x_double;
+    c->ws_ready = true;
+    // distinct, aligned, never dereferenced: the planner only compares and swaps them
+    double* f = reinterpret_cast<double*>((uintptr_t)0x10000);
+    c->f2 = reinterpret_cast<double*>((uintptr_t)0x20000);
+    c->rho = c->E = reinterpret_cast<double*>((uintptr_t)0x30000);
+    r = nsteps == 0 ? sldg_step(c, f, 0.1) : sldg_steps(c, f, 0.1, nsteps);
+    counts[0] = c->dry_x; counts[1] = c->dry_v; counts[2] = c->dry_rho; counts[3] = c->dry_field; counts[4] = c->dry_copies;
+    counts[5] = c->launches;
+    delete c;
+    return r;
 }
 
 extern "C" int sldg_step_host(sldg_ctx* c, double* f_host, double* f_dev, double* E_host, double dt, int nsteps)

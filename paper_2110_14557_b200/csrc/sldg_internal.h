@@ -15,6 +15,9 @@
 #define SLDG_MAXPOLY (2 * SLDG_MAX_DEGREE + 2)   // A_jl(alpha) has degree <= 2k+1
 
 // bit 30 of a table's s-entry marks alpha == 0 (pure copy, exact permutation)
+// sldg_create_prec(precision | this bit): host fields only, no device (the dry-run context of sldg_plan_query)
+#define SLDG_DRY_BIT_INTERNAL 0x100
+
 #define SLDG_COPY_BIT (1 << 30)
 #define SLDG_S_MASK (SLDG_COPY_BIT - 1)
 
@@ -112,6 +115,10 @@ struct sldg_ctx {
     int poisson_solver;             // 0 = FFT route (reading P1), 1 = CGdG
     double cg_tol, cg_sigma; int cg_maxiter;
     bool ws_ready;
+
+    // dry run (sldg_plan_query): the planning code runs unchanged, every launch site only counts what it would launch
+    bool dry; int dry_safe;
+    long long dry_x, dry_v, dry_rho, dry_field, dry_copies;   // passes over f by kind, field solves, device copies
 
     // instrumentation
     bool timing;

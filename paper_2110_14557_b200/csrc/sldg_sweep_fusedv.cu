@@ -333,7 +333,7 @@ bool SLDG_SFX(sldg_fusedv_shape)(const sldg_ctx* c, int* wx_out, int* threads_ou
     if (D1 > 256 || c->cells[c->dx] < 1) return false;
     if ((c->X * (long long)sizeof(real)) & 15) return false;
     // 32-bit tensor coordinates, and the driver's tensor-map encoder must be reachable (no libcuda link)
-    if (c->X >= (1LL << 31) || c->V / D1 >= (1LL << 31) || !encode_fn()) return false;
+    if (c->X >= (1LL << 31) || c->V / D1 >= (1LL << 31) || (!c->dry && !encode_fn())) return false;
     const int cap = (K1 <= 2) ? FVTraits<1>::MAXT : FVTraits<3>::MAXT;  // threads allowed
     // x nodes per tile: rows of 128 B when the thread budget allows, else 64 B; never below 32 B
     int wx = c->opt_fv_wx > 0 ? c->opt_fv_wx : (int)(128 / sizeof(real));

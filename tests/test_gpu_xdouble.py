@@ -93,3 +93,31 @@ def test_steps_equal_repeated_single_steps_with_the_double_pass(P, n):
         g.step(fa, cfg["dt"])
     g.steps(fb, cfg["dt"], n)
     assert torch.equal(fa, fb)
+
+
+@pytest.mark.parametrize("geom", [(2, 2, [12, 10, 8, 8], 2), (2, 3, [8, 8, 6, 6, 4], 1), (3, 3, [6, 4, 4, 6, 4, 4], 1)],
+                         ids=lambda g: f"{g[0]}x{g[1]}v-k{g[3]}")
+@pytest.mark.parametrize("n", [0, 2, 5])
+@pytest.mark.parametrize("fuse_v,x_double", [(0, 0), (2, 0), (2, 1), (0, 1)])
+def test_plan_query_counts_are_those_of_the_real_calls(P, geom, n, fuse_v, x_double):
+    """The host-only sldg_plan_query (tests/test_plan.py checks its budgets on the CPU) must report exactly the sweep
+    launches the real sldg_step / sldg_steps make: per-kind launch counts from the library's event instrumentation."""
+    dx, dv, cells, k = geom
+    dom = dom_of(dx, dv)
+    g = P.Sldg(dx, dv, cells, k, dom)
+    g.set_option("graph", 0); g.set_option("fuse_v", fuse_v); g.set_option("x_double", x_double)
+    f = W.random_field(g.shape, seed=2).to(g.device).contiguous()
+    dt = 0.01                                                      # every x shift below one cell
+    g.timing_enable(True); g.timing_read()
+    if n == 0:
+        g.step(f, dt)
+    else:
+        g.steps(f, dt, n)
+    kinds, _ = g.timing_read()
+    g.timing_enable(False)
+    want = P.plan_query(dx, dv, cells, k, n, shifts_below_one=True, fuse_v=fuse_v, x_double=x_double)
+    sweeps = sum(v[0] for name, v in kinds.items() if name.startswith("sweep"))
+    assert sweeps == want["x_passes"] + want["v_passes"]
+    assert kinds["sweep_fused_v"][0] + kinds["sweep_slow_axis"][0] >= want["v_passes"]
+    assert kinds["copies"][0] == dx                                # only the x shift-table uploads (one event per axis)
+    assert kinds["rho"][0] == max(1, n)
