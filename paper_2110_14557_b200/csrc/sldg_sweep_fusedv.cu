@@ -21,7 +21,7 @@
 //   in once more (k+1 extra rows per plane, 1/N_2 of the reads) for k = 2.
 //
 // Arithmetic per value is identical (same operands, same order) to sweep_walk_kernel on v_1 then on v_2, so the
-// fused and the unfused plans agree bit for bit.  Out of place only; degree <= 2; D_1 <= 256 (one TMA box);
+// fused and the unfused plans agree bit for bit.  Out of place only; degree <= 3; D_1 <= 256 (one TMA box);
 // X * sizeof(real) a multiple of 16.
 #include <cuda.h>
 
@@ -58,15 +58,15 @@ template <int K1> struct FVTraits {
     static constexpr bool KEEP = (K1 <= 2);        // first v_2 block kept in registers (else streamed in again)
     // threads per block.  Registers are split over the 4 SM sub-partitions: 16 warps leave 128 registers per thread
     // (what the (k+1)^2 blocks and four tables of k = 2 need), 20 warps 96.
-    static constexpr int MAXT = (K1 <= 2) ? 640 : 512;
+    static constexpr int MAXT = (K1 <= 2) ? 640 : (K1 == 3) ? 512 : 256;   // k = 3: 8 warps, up to 255 registers
     // k = 2: A_2, B_2 of the tile's x nodes live in shared memory (rows [A_2[j][.] | B_2[j][.]], one padded record per
     // x node, read as 2-value vectors: lanes of equal x broadcast, different x fall on different banks); with all four
     // tables in registers the kernel spills (ncu: a third of the issue slots stalled on local loads).
     static constexpr bool T2S = (K1 >= 3);
-    static constexpr int PAD = 2 * K1 * K1 + 4;
+    static constexpr int PAD = 2 * K1 * K1 + (K1 == 4 ? 6 : 4);        // record stride = 12 banks mod 32: conflict free
     // v_2 rows per tensor copy (= per ring slot).  Measured: a whole cell per copy is faster at k = 1 (cfg3 3.6 -> 3.0 ms:
     // half the barrier traffic), a row per copy at k = 2 (cfg2 4.3 against 5.0 ms with 36 KB copies).
-    static constexpr int RPS = (K1 == 3) ? 1 : K1;
+    static constexpr int RPS = (K1 >= 3) ? 1 : K1;
 };
 
 template <int K1>
@@ -328,15 +328,22 @@ cudaError_t launch(sldg_ctx* c, const CUtensorMap& tm, const FVParams& P, int th
 bool SLDG_SFX(sldg_fusedv_shape)(const sldg_ctx* c, int* wx_out, int* threads_out)
 {
     const int K1 = c->K1;
-    if (c->dx < 2 || K1 > 3) return false;
+    if (c->dx < 2 || K1 > 4) return false;
     const long long D1 = c->D[c->dx];
     if (D1 > 256 || c->cells[c->dx] < 1) return false;
     if ((c->X * (long long)sizeof(real)) & 15) return false;
     // 32-bit tensor coordinates, and the driver's tensor-map encoder must be reachable (no libcuda link)
     if (c->X >= (1LL << 31) || c->V / D1 >= (1LL << 31) || (!c->dry && !encode_fn())) return false;
-    const int cap = (K1 <= 2) ? FVTraits<1>::MAXT : FVTraits<3>::MAXT;  // threads allowed
+    const int cap = (K1 <= 2) ? FVTraits<1>::MAXT : (K1 == 3) ? FVTraits<3>::MAXT : FVTraits<4>::MAXT;  // threads allowed
     // x nodes per tile: rows of 128 B when the thread budget allows, else 64 B; never below 32 B
     int wx = c->opt_fv_wx > 0 ? c->opt_fv_wx : (int)(128 / sizeof(real));
+    if (K1 == 4 && c->opt_fv_wx <= 0) {
+        // k = 3: one block of at most 256 threads per SM (212 registers): fill it -- as many x nodes as fit, whole 16 B
+        const int q16 = 16 / (int)sizeof(real);
+        wx = (int)(cap / c->cells[c->dx]) / q16 * q16;
+        if (wx > 256 / (int)sizeof(real)) wx = 256 / (int)sizeof(real);
+        if (wx < 32 / (int)sizeof(real)) wx = 32 / (int)sizeof(real);
+    }
     while (wx * (int)sizeof(real) > 32 && (long long)wx * c->cells[c->dx] > cap) wx /= 2;
     if ((long long)wx * c->cells[c->dx] > cap) return false;
     if ((wx * (int)sizeof(real)) & 15) return false;
@@ -365,10 +372,10 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     P.fout = static_cast<real*>(fout);
     P.X = c->X; P.planes = planes; P.N1 = c->cells[a1]; P.N2 = c->cells[a2]; P.WX = wx;
     P.ntiles = (int)((c->X + wx - 1) / wx);
-    int cps = (K1 == 3) ? 1 : (c->opt_fv_cps > 0 ? c->opt_fv_cps : 1);   // v_2 cells per tensor copy (k <= 1)
+    int cps = (K1 >= 3) ? 1 : (c->opt_fv_cps > 0 ? c->opt_fv_cps : 1);   // v_2 cells per tensor copy (k <= 1)
     if (cps > c->cells[a2]) cps = c->cells[a2];
     P.cps = cps;
-    const int rps = (K1 == 3 ? 1 : K1) * cps;                           // rows per ring slot
+    const int rps = (K1 >= 3 ? 1 : K1) * cps;                           // rows per ring slot
     P.stage_bytes = (uint32_t)(((size_t)rps * D1 * wx * sizeof(real) + 1023) / 1024 * 1024);
     // ring depth: about opt_fv_inflight bytes in flight per SM
     const size_t regs_blocks = (K1 <= 2) ? (size_t)(65536 / 96) / threads : 1;
@@ -377,7 +384,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     int stages = c->opt_fv_stages > 0 ? c->opt_fv_stages : (int)((size_t)c->opt_fv_inflight * (K1 <= 2 ? 4 : 3) / 3 / bps / P.stage_bytes);   // measured: 96 KB at k <= 1, 72 KB at k = 2
     if (stages < 3) stages = 3;
     if (stages > 24) stages = 24;
-    auto smem_of = [&](int st) { return (size_t)st * P.stage_bytes + 16 * (size_t)st + (size_t)wx * (2 * K1 * K1 + 4) * sizeof(real) + 128; };
+    auto smem_of = [&](int st) { return (size_t)st * P.stage_bytes + 16 * (size_t)st + (size_t)wx * (2 * K1 * K1 + 6) * sizeof(real) + 128; };
     while (stages > 2 && smem_of(stages) > 227 * 1024) stages--;
     if (smem_of(stages) > 227 * 1024) return cudaErrorNotSupported;
     P.stages = stages;
@@ -409,6 +416,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     case 1: return launch<1>(c, tm, P, threads, smem);
     case 2: return launch<2>(c, tm, P, threads, smem);
     case 3: return launch<3>(c, tm, P, threads, smem);
+    case 4: return launch<4>(c, tm, P, threads, smem);
     }
     return cudaErrorNotSupported;
 }

@@ -54,9 +54,13 @@ def test_options_change_the_budget_as_documented():
     assert (r["x_passes"], r["v_passes"], r["copies"]) == (4, 2, 0)
 
 
-def test_degree_three_has_no_merged_passes():
+def test_degree_three_fuses_v_but_not_the_x_half_steps():
+    """k = 3 (the paper's default order): the fused v pass exists (256-thread blocks), the double x half step
+    does not (two walk states of (k+1)^2 values do not fit the register file) -> sldg_steps alternates buffers."""
     cfg = {c["name"]: c for c in W.NEXT_CONFIGS}["bot_5d_k3_16"]
     r = q(cfg, 10)
+    assert (r["x_passes"], r["v_passes"], r["copies"]) == (20, 10, 0)
+    r = q(cfg, 10, fuse_v=0)
     assert (r["x_passes"], r["v_passes"], r["copies"]) == (20, 20, 0)
 
 
