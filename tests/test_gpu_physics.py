@@ -73,3 +73,29 @@ def test_linear_landau_damping_rate_fp64_fp32_and_cgdg(P):
     _, ecg, _ = run(P, "f64", "cg")
     gcg, wcg, _ = damping_fit(t, ecg, 0.1)
     assert abs(gcg + 0.1533) < 0.06 * 0.1533 and abs(wcg - 1.4156) < 0.03 * 1.4156, (gcg, wcg)
+
+
+def test_merged_plans_reproduce_the_step_by_step_run_bitwise(P):
+    """The same Landau run advanced by ONE sldg_steps call (double x half steps, fused v_1+v_2 passes, alternating
+    buffers: 3.4e8 values, so the automatic plan rules apply) must give the bits of 60 separate sldg_step calls, and
+    conserve mass; the field of the last step must be the one the step-by-step run saw."""
+    cfg = dict(name="landau2x2v", dim_x=2, dim_v=2, cells=[32, 32, 64, 64], degree=2,
+               domain=[0, 4 * math.pi, 0, 4 * math.pi, -6, 6, -6, 6], dt=0.1, ic="landau",
+               ic_args=dict(eps=0.01, k=0.5, axes=[0]))
+    g = P.Sldg(2, 2, cfg["cells"], 2, cfg["domain"])
+    f0 = W.initial_data(cfg, [g.node_coords(a) for a in range(4)], device=g.device)
+    fa, fb = f0.clone(), f0.clone()
+    m0 = g.mass(fa)
+    n0 = g.launch_count()
+    for _ in range(60):
+        g.step(fa, 0.1)
+    Ea = g.last_E().clone()
+    n1 = g.launch_count()
+    g.steps(fb, 0.1, 60)
+    n2 = g.launch_count()
+    assert torch.equal(fa, fb)
+    assert torch.equal(Ea, g.last_E())
+    assert abs(g.mass(fb) - m0) / abs(m0) < 1e-12
+    assert (n2 - n1) < (n1 - n0) - 100                            # 59 merged x passes and 60 fused v passes fewer
+    want = P.plan_query(2, 2, cfg["cells"], 2, 60)
+    assert (want["x_passes"], want["v_passes"], want["copies"]) == (62, 60, 0)
