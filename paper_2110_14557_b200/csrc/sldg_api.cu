@@ -92,12 +92,12 @@ cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double*
                                : sldg_launch_sweep_fused_cell_f64(c, fin, fout, g0, g1, t0, t1);
 }
 
-extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree, const double* domain,
-                                int precision)
+// host_only: the host fields only, no device (the dry-run context of sldg_plan_query)
+static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree, const double* domain,
+                       int precision, bool host_only)
 {
     if (!out || !cells || !domain) return SLDG_EINVAL;
-    const int dry_bit = precision & SLDG_DRY_BIT_INTERNAL;
-    if ((precision & ~SLDG_DRY_BIT_INTERNAL) != SLDG_F64 && (precision & ~SLDG_DRY_BIT_INTERNAL) != SLDG_F32) return SLDG_EINVAL;
+    if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
     if (dim_x < 1 || dim_x > 3 || dim_v < dim_x || dim_v > 3) return SLDG_EINVAL;
     if (degree < 0 || degree > SLDG_MAX_DEGREE) return SLDG_EINVAL;
     const int d = dim_x + dim_v;
@@ -109,8 +109,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     if (!c) return SLDG_ENOMEM;
     c->dry = false; c->dry_safe = 0; c->dry_x = c->dry_v = c->dry_rho = c->dry_field = c->dry_copies = 0;
     c->dx = dim_x; c->dv = dim_v; c->d = d; c->k = degree; c->K1 = degree + 1;
-    c->prec = precision & ~SLDG_DRY_BIT_INTERNAL; c->esize = c->prec == SLDG_F32 ? 4 : 8;
-    (void)dry_bit;
+    c->prec = precision; c->esize = precision == SLDG_F32 ? 4 : 8;
     c->nf = 1; c->X = 1; c->V = 1;
     for (int a = 0; a < d; a++) {
         c->cells[a] = cells[a];
@@ -138,7 +137,7 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
     c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
 
-    if (precision & SLDG_DRY_BIT_INTERNAL) { *out = c; return SLDG_OK; }   // sldg_plan_query: host fields only
+    if (host_only) { *out = c; return SLDG_OK; }                            // sldg_plan_query
 
     // device side: needs a CUDA device.  Without one the context is unusable -> fail loudly.
     int dev = 0;
@@ -195,6 +194,12 @@ extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int*
     }
     *out = c;
     return SLDG_OK;
+}
+
+extern "C" int sldg_create_prec(sldg_ctx** out, int dim_x, int dim_v, const int* cells, int degree, const double* domain,
+                                int precision)
+{
+    return create_impl(out, dim_x, dim_v, cells, degree, domain, precision, false);
 }
 
 extern "C" int sldg_destroy(sldg_ctx* c)
@@ -925,7 +930,7 @@ extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degre
     double dom[2 * SLDG_MAX_DIM];
     for (int a = 0; a < SLDG_MAX_DIM; a++) { dom[2 * a] = 0.0; dom[2 * a + 1] = 1.0; }
     sldg_ctx* c = nullptr;
-    int r = sldg_create_prec(&c, dim_x, dim_v, cells, degree, dom, precision | SLDG_DRY_BIT_INTERNAL);
+    int r = create_impl(&c, dim_x, dim_v, cells, degree, dom, precision, true);
     if (r) return r;
     c->dry = true; c->dry_safe = shifts_below_one; c->opt_graph = 0; c->opt_fuse_v = fuse_v; c->opt_x_double = x_double;
     c->ws_ready = true;

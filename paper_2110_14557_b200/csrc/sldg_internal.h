@@ -15,9 +15,6 @@
 #define SLDG_MAXPOLY (2 * SLDG_MAX_DEGREE + 2)   // A_jl(alpha) has degree <= 2k+1
 
 // bit 30 of a table's s-entry marks alpha == 0 (pure copy, exact permutation)
-// sldg_create_prec(precision | this bit): host fields only, no device (the dry-run context of sldg_plan_query)
-#define SLDG_DRY_BIT_INTERNAL 0x100
-
 #define SLDG_COPY_BIT (1 << 30)
 #define SLDG_S_MASK (SLDG_COPY_BIT - 1)
 
