@@ -190,3 +190,20 @@ def test_fused_v_pass_stays_inside_the_field(P, geom):
     for _ in range(3):
         want, _, _ = o.step(want, 0.05)
     assert rel_inf(f.cpu().numpy(), want) <= 1e-10
+
+
+def test_fused_v_pass_inside_a_captured_step_graph(P):
+    """The tensor map of the fused pass is a by-value kernel parameter built on the host at launch time: a Strang step
+    captured into a CUDA graph (option graph = 2) and replayed must give the bits of plain launches."""
+    cfg = W.scaled(W.CONFIGS[1], [12, 10, 8, 8])
+    o = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], threads=1)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    outs = []
+    for graph in (0, 2):
+        g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+        g.set_option("fuse_v", 2); g.set_option("graph", graph)
+        fg = f0.to(g.device).contiguous()
+        for _ in range(4):
+            g.step(fg, cfg["dt"])
+        outs.append(fg.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
