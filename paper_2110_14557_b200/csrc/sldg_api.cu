@@ -131,7 +131,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
-    c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
+    c->opt_poisson_small = 1; c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
@@ -1142,6 +1142,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "cell_rows")) { if (value < 0 || value > 1024) return SLDG_EINVAL; c->opt_cell_rows = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_cell_bytes = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_stages")) { if (value < 2 || value > 6) return SLDG_EINVAL; c->opt_cell_stages = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "poisson_small")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_poisson_small = (int)value; return SLDG_OK; }
     if (!strcmp(name, "x_double")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_double = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv_wx = (int)value; return SLDG_OK; }

@@ -191,6 +191,79 @@ __global__ void spectral_kernel(SpecParams P, int d, const double* __restrict__ 
     else { er[t] = -kd * ri[t] / k2; ei[t] = kd * rr[t] / k2; }
 }
 
+// Small x grids (X <= 1024 nodes, e.g. BASELINE config 1: 256): the whole solve in ONE single-block launch with the
+// six complex work arrays in shared memory, instead of 8 (dim_x = 2) or 15 (dim_x = 3) launches of a few microseconds
+// each.  Every output is the same fma chain over n = 0..D-1 as in apply_axis_kernel and the same spectral formula, so
+// the result is bit-identical to the multi-launch route.
+struct SmallParams { int dx; long long D[3]; const double* kap[3]; const double* fwdT[3]; const double* invT[3]; long long X; };
+
+template <bool HAS_IM, bool OUT_IM>
+__device__ __forceinline__ void small_axis(const double* __restrict__ inr, const double* __restrict__ ini,
+                                           const double* __restrict__ MT, long long D, long long inner, long long X,
+                                           double* __restrict__ outr, double* __restrict__ outi)
+{
+    for (long long t = threadIdx.x; t < X; t += blockDim.x) {
+        const long long pp = t % inner, m = (t / inner) % D, q = t / (inner * D);
+        const long long base = q * D * inner + pp;
+        double ar = 0.0, ai = 0.0;
+        for (long long n = 0; n < D; n++) {
+            const double mr = __ldg(MT + n * D + m), mi = __ldg(MT + D * D + n * D + m), vr = inr[base + n * inner];
+            ar = fma(mr, vr, ar); ai = fma(mi, vr, ai);
+            if (HAS_IM) {
+                const double vi = ini[base + n * inner];
+                ar = fma(-mi, vi, ar); ai = fma(mr, vi, ai);
+            }
+        }
+        outr[t] = ar;
+        if (OUT_IM) outi[t] = ai;
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(256) poisson_small_kernel(SmallParams P, const double* __restrict__ rho, double* __restrict__ E)
+{
+    extern __shared__ double sm_small[];
+    const long long X = P.X;
+    double *ar = sm_small, *ai = ar + X, *br = ai + X, *bi = br + X, *rr = bi + X, *ri = rr + X;
+    // forward: transfer to the equidistant grid + DFT, axis by axis (as sldg_launch_poisson)
+    const double* sr = rho; const double* si = nullptr;
+    long long inner = 1;
+    for (int a = 0; a < P.dx; a++) {
+        const bool last = (a == P.dx - 1);
+        double* dr = last ? rr : ((a & 1) ? br : ar);
+        double* di = last ? ri : ((a & 1) ? bi : ai);
+        if (si) small_axis<true, true>(sr, si, P.fwdT[a], P.D[a], inner, X, dr, di);
+        else small_axis<false, true>(sr, si, P.fwdT[a], P.D[a], inner, X, dr, di);
+        sr = dr; si = di; inner *= P.D[a];
+    }
+    for (int d = 0; d < P.dx; d++) {
+        for (long long t = threadIdx.x; t < X; t += blockDim.x) {
+            long long r = t;
+            double k2 = 0.0, kd = 0.0;
+            for (int a = 0; a < P.dx; a++) {
+                long long m = r % P.D[a]; r /= P.D[a];
+                double kap = P.kap[a][m];
+                k2 += kap * kap;
+                if (a == d) kd = (2 * m == P.D[a]) ? 0.0 : kap;
+            }
+            if (k2 == 0.0) { ar[t] = 0.0; ai[t] = 0.0; }
+            else { ar[t] = -kd * ri[t] / k2; ai[t] = kd * rr[t] / k2; }
+        }
+        __syncthreads();
+        double *pr = ar, *pi = ai, *qr = br, *qi = bi;
+        inner = 1;
+        for (int a = 0; a < P.dx; a++) {
+            const bool last = (a == P.dx - 1);
+            if (last) small_axis<true, false>(pr, pi, P.invT[a], P.D[a], inner, X, E + (long long)d * X, nullptr);
+            else small_axis<true, true>(pr, pi, P.invT[a], P.D[a], inner, X, qr, qi);
+            double* t2;
+            t2 = pr; pr = qr; qr = t2;
+            t2 = pi; pi = qi; qi = t2;
+            inner *= P.D[a];
+        }
+    }
+}
+
 // ------------------------------------------------------------------ diagnostics
 struct WgtParams { int nd; long long D[SLDG_MAX_DIM]; const double* w[SLDG_MAX_DIM]; long long total; };
 
@@ -303,6 +376,14 @@ cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho)
 cudaError_t sldg_launch_poisson(sldg_ctx* c, const double* rho, double* E)
 {
     const long long X = c->X;
+    if (X <= 1024 && c->opt_poisson_small) {
+        SmallParams S;
+        S.dx = c->dx; S.X = X;
+        for (int a = 0; a < c->dx; a++) { S.D[a] = c->D[a]; S.kap[a] = c->dKap[a]; S.fwdT[a] = c->dFwdT[a]; S.invT[a] = c->dInvT[a]; }
+        poisson_small_kernel<<<1, 256, (size_t)(6 * X * sizeof(double)), c->stream>>>(S, rho, E);
+        c->launches++;
+        return cudaGetLastError();
+    }
     const int block = 128;
     const unsigned grid = (unsigned)((X + block - 1) / block);
     double *ar = c->cplx[0], *ai = c->cplx[1], *br = c->cplx[2], *bi = c->cplx[3], *rr = c->cplx[4], *ri = c->cplx[5];

@@ -155,6 +155,7 @@ struct sldg_ctx {
     int opt_fv_ppb;                 // fused v kernel: planes per block (0 = auto)
     int opt_fv_cps;                 // fused v kernel, degree <= 1: v_2 cells per tensor copy
     int opt_fv_l2;                  // fused v kernel: L2 promotion of the tensor map (0 none, 1 64 B, 2 128 B, 3 256 B)
+    int opt_poisson_small;          // 1: x grids of up to 1024 nodes are solved by one single-block launch (FFT route)
     int opt_rho_vec;                // 0 = auto (2 when aligned), 1
     int opt_rho_blocks;             // rho kernel: 128-thread blocks per SM to aim for
 };

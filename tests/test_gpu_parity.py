@@ -488,3 +488,26 @@ def test_repeated_steps_are_bitwise_identical(P, geom, prec):
             ref = f
         else:
             assert torch.equal(ref, f), rep
+
+
+# --------------------------------------------------------------- single-launch Poisson solve of small x grids
+
+@pytest.mark.parametrize("geom", [(1, 1, [37, 5], 1), (2, 2, [8, 8, 4, 4], 1), (2, 2, [7, 5, 3, 3], 2), (2, 3, [6, 4, 3, 2, 2], 3),
+                                  (3, 3, [4, 3, 5, 2, 2, 2], 1), (3, 3, [3, 3, 2, 2, 2, 2], 2), (2, 2, [16, 16, 2, 2], 1)],
+                         ids=lambda g: f"{g[0]}x{g[1]}v-{'x'.join(map(str, g[2]))}-k{g[3]}")
+def test_small_grid_poisson_in_one_launch_is_bitwise_the_multi_launch_route(P, geom):
+    """X <= 1024 x nodes (BASELINE config 1: 256): one single-block launch with the work arrays in shared memory does the
+    per-axis DFTs, the spectral solve and the inverse transforms with the same fma chain per output as the tiled
+    kernels: same bits, 1 launch instead of 8 / 15; and the oracle's E within the bar."""
+    dx, dv, cells, k = geom
+    g, o = make_pair(P, dx, dv, cells, k)
+    rho = 1.0 + 0.3 * W.random_field(o.xshape, seed=8)
+    outs = []
+    for small in (1, 0):
+        g.set_option("poisson_small", small)
+        n0 = g.launch_count()
+        E = g.poisson(rho.to(g.device))
+        outs.append((E.cpu().numpy(), g.launch_count() - n0))
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert outs[0][1] == 1 and outs[1][1] == dx + dx * (1 + dx)
+    assert rel_inf(outs[0][0], o.poisson(rho.numpy())) <= 1e-12
