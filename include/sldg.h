@@ -95,7 +95,9 @@ int sldg_advect_x(sldg_ctx* ctx, double* f, double dt);
 
 /* a5+a6, steps 3a-3c: for d = 1..dim_x, f(x, v_d + E_d(x) dt), i.e. the same update
  * along v_d with delta = ((-E_d(x)) * dt) / h_{v_d} per x node (sign from eq. (1), reading H).
- * Velocity axes beyond dim_x are not advected (reading D).  E is [dim_x][X].  Result in f. */
+ * Velocity axes beyond dim_x are not advected (reading D).  E is [dim_x][X].  Result in f.
+ * E is the same for all sweeps, so the v_1 and v_2 sweeps may run as one pass over f (same
+ * arithmetic in the same order: bit-identical to separate sweeps; option fuse_v). */
 int sldg_advect_v(sldg_ctx* ctx, double* f, const double* E, double dt);
 
 /* a3: rho[x] = sum_v (prod_d h_{v_d} w_{j_d}) f[x,v]. */
@@ -134,9 +136,12 @@ const double* sldg_last_phi(const sldg_ctx* ctx);
  * B u_{i-1} + B^T u_{i+1}; sigma <= 0: default.  Host-only, needs no context or device. */
 int sldg_sipg_matrices(int degree, double sigma, double* hostM, double* hostB);
 
-/* nsteps Strang steps; the result is in f and equals nsteps calls of sldg_step bit for bit.  Consecutive
- * steps may keep their intermediate result in the workspace buffer, which lets every x half step of a
- * dim_x = 3 problem run as ONE fused pass (a single sldg_step needs one two-pass x half step to end in f). */
+/* nsteps Strang steps; the result is in f and equals nsteps calls of sldg_step bit for bit (the same 1-D
+ * sweeps in the same order).  What changes is the number of passes over f: consecutive steps may keep their
+ * intermediate result in the workspace buffer, and for dim_x = 2 the second x half step of a step and the
+ * first x half step of the next one (same time increment, nothing in between) run as ONE pass
+ * (option x_double).  f at the intermediate integer times is then not written out: call sldg_step when a
+ * per-step diagnostic needs it.  sldg_plan_query reports the pass budget of either call. */
 int sldg_steps(sldg_ctx* ctx, double* f, double dt, int nsteps);
 
 /* Same path driven from HOST memory: copies f_host (|f| doubles, pinned memory recommended) to
