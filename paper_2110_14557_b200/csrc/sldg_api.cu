@@ -86,10 +86,10 @@ cudaError_t sldg_launch_sweep_line(sldg_ctx* c, const double* fin, double* fout,
     return c->prec == SLDG_F32 ? sldg_launch_sweep_line_f32(c, fin, fout, g, t) : sldg_launch_sweep_line_f64(c, fin, fout, g, t);
 }
 cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
-                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy)
 {
-    return c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell_f32(c, fin, fout, g0, g1, t0, t1)
-                               : sldg_launch_sweep_fused_cell_f64(c, fin, fout, g0, g1, t0, t1);
+    return c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell_f32(c, fin, fout, g0, g1, t0, t1, any_copy)
+                               : sldg_launch_sweep_fused_cell_f64(c, fin, fout, g0, g1, t0, t1, any_copy);
 }
 
 // host_only: the host fields only, no device (the dry-run context of sldg_plan_query)
@@ -537,7 +537,7 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     if (p.fused && !c->dry) {
         sldg_ev_begin(c, KIND_FUSED, 0);
         cudaError_t e = cudaErrorNotSupported;
-        if (c->opt_fused_impl != 2) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        if (c->opt_fused_impl != 2) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], (c->tab_anycp[0] || c->tab_anycp[1]) ? 1 : 0);
         if (e == cudaErrorNotSupported && c->prec == SLDG_F64) e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
         sldg_ev_end(c);
         c->launches++;
@@ -760,9 +760,10 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
     int r = build_x_tables(c, tau, tabs);
     if (r) return r;
     if (c->dry) { c->dry_x++; c->launches++; double* t = *cur; *cur = *oth; *oth = t; return SLDG_OK; }
+    const int anycp = (c->tab_anycp[0] || c->tab_anycp[1]) ? 1 : 0;
     sldg_ev_begin(c, KIND_FUSEDX2, 0);
-    cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1])
-                                        : sldg_launch_sweep_fused_cell2_f64(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+    cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], anycp)
+                                        : sldg_launch_sweep_fused_cell2_f64(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], anycp);
     sldg_ev_end(c);
     c->launches++;
     if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }

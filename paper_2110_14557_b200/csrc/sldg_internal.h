@@ -176,9 +176,9 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
     cudaError_t sldg_launch_sweep_line##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g,           \
                                             const ShiftTable& t);                                                   \
     cudaError_t sldg_launch_sweep_fused_cell##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,    \
-                                                  const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1); \
+                                                  const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy); \
     cudaError_t sldg_launch_sweep_fused_cell2##sfx(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,   \
-                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
+                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy);
 cudaError_t sldg_launch_sweep_fused3_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 cudaError_t sldg_launch_sweep_fused3_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 bool sldg_fusedv_shape_f64(const sldg_ctx* c, int* wx_out, int* threads_out);
@@ -196,7 +196,7 @@ cudaError_t sldg_launch_sweep_tma(sldg_ctx* c, const double* fin, double* fout, 
 cudaError_t sldg_launch_sweep_fused(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
                                     const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
 cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
-                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
+                                         const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy);
 cudaError_t sldg_upload_poly(const ABPoly* p);
 cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB);
 cudaError_t sldg_launch_wv(sldg_ctx* c);

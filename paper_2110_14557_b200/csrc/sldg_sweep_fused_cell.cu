@@ -75,7 +75,8 @@ template <int K1> struct CellV {
 // x_2 walk (its own previous / first block).  The first pair emits its cells in cyclic order starting at cell
 // s_2 + 1, which is all a periodic walk needs, so the second pair's outputs trail by one cell and the wrap cell joins
 // the last group.  Same operands and order as two launches of the single pass: bit-identical.
-template <int K1, int MINB, bool DBL>
+// CPS = false: no entry of the two shift tables has alpha == 0 (the host knows): the copy selects are compiled out.
+template <int K1, int MINB, bool DBL, bool CPS>
 __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellParams P)
 {
     constexpr int NN = K1 * K1;
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
                 for (int m = 0; m < K1; m++) acc += A1[j1 * K1 + m] * a.v[m];
 #pragma unroll
                 for (int m = 0; m < K1; m++) acc += B1[j1 * K1 + m] * b.v[m];
-                N[j2 * K1 + j1] = cp1 ? a.v[j1] : acc;
+                N[j2 * K1 + j1] = (CPS && cp1) ? a.v[j1] : acc;
             }
         }
     };
@@ -208,7 +209,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
                 for (int l = 0; l < K1; l++) acc += A2[j2 * K1 + l] * nxt[l * K1 + j1];
 #pragma unroll
                 for (int l = 0; l < K1; l++) acc += B2[j2 * K1 + l] * prv[l * K1 + j1];
-                r.v[j1] = cp2 ? nxt[j2 * K1 + j1] : acc;
+                r.v[j1] = (CPS && cp2) ? nxt[j2 * K1 + j1] : acc;
             }
             r.store(orow + j2 * D0);
         }
@@ -217,7 +218,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
     const int H = (N1 + CR - 1) / CR;                  // output groups of CR cells
     int io0 = s2 + 1; if (io0 >= N1) io0 -= N1;        // first output cell of the group (of the first pair)
     int io2 = io0 + s2 + 1; if (io2 >= N1) io2 -= N1;  // DBL: first output cell of the second pair's next group
-    real first2[DBL ? NN : 1], prev2[DBL ? NN : 1];
+    real first2[DBL ? NN : 1], prev2[DBL ? NN : 1], alt2[DBL ? NN : 1], alt[NN];
     for (int h = 0; h < H; h++) {
         const int j = h + 1;                           // input chunk that feeds this group
         const int st = j % ST;
@@ -226,19 +227,26 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         if (nin > 0) mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
         const real* ibase = sin_ + st * SS + pl * PC;
         real* obase = (DBL ? smid : sout + (h & 1) * SS) + pl * PC + i * K1;
-        for (int e = 0; e < nout; e++) {
-            real nxt[NN];
-            if (e < nin) swept(ibase + e * K1 * D0, nxt);
+        // the walk alternates between `prev` and `alt` (two cells per trip: no register moves); an odd tail copies once
+        auto cell1 = [&](int e, real (&nx)[NN], const real (&pv)[NN]) {
+            if (e < nin) swept(ibase + e * K1 * D0, nx);
             else {
 #pragma unroll
                 for (int m = 0; m < NN; m++) {
-                    if constexpr (FS) nxt[m] = first_s[m * blockDim.x + t];
-                    else nxt[m] = first[m];
+                    if constexpr (FS) nx[m] = first_s[m * blockDim.x + t];
+                    else nx[m] = first[m];
                 }
             }
-            emit(obase + e * K1 * D0, nxt, prev);
+            emit(obase + e * K1 * D0, nx, pv);
+        };
+        {
+            int e = 0;
+            for (; e + 1 < nout; e += 2) { cell1(e, alt, prev); cell1(e + 1, prev, alt); }
+            if (e < nout) {
+                cell1(e, alt, prev);
 #pragma unroll
-            for (int m = 0; m < NN; m++) prev[m] = nxt[m];
+                for (int m = 0; m < NN; m++) prev[m] = alt[m];
+            }
         }
         int ncells = nout;                             // cells the leader stores for this group
         if constexpr (DBL) {
@@ -246,18 +254,23 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
             issue_load(j + ST);
             real* o2 = sout + (h & 1) * SSO + pl * PCO + i * K1;
             ncells = 0;
-            for (int e = 0; e < nout; e++) {
-                real nxt2[NN];
-                swept(smid + pl * PC + e * K1 * D0, nxt2);
-                if (h == 0 && e == 0) {
+            auto cell2 = [&](int e, real (&nx)[DBL ? NN : 1], const real (&pv)[DBL ? NN : 1]) {
+                swept(smid + pl * PC + e * K1 * D0, nx);
+                emit(o2 + ncells * K1 * D0, nx, pv);
+                ncells++;
+            };
+            int e = 0;
+            if (h == 0) {                              // the first cell of the second walk only initialises it
+                swept(smid + pl * PC, prev2);
 #pragma unroll
-                    for (int m = 0; m < NN; m++) first2[DBL ? m : 0] = nxt2[m];
-                } else {
-                    emit(o2 + ncells * K1 * D0, nxt2, prev2);
-                    ncells++;
-                }
+                for (int m = 0; m < NN; m++) first2[DBL ? m : 0] = prev2[DBL ? m : 0];
+                e = 1;
+            }
+            for (; e + 1 < nout; e += 2) { cell2(e, alt2, prev2); cell2(e + 1, prev2, alt2); }
+            if (e < nout) {
+                cell2(e, alt2, prev2);
 #pragma unroll
-                for (int m = 0; m < NN; m++) prev2[DBL ? m : 0] = nxt2[m];
+                for (int m = 0; m < NN; m++) prev2[DBL ? m : 0] = alt2[DBL ? m : 0];
             }
             if (h == H - 1) {                          // the periodic wrap of the second walk
                 emit(o2 + ncells * K1 * D0, first2, prev2);
@@ -283,9 +296,9 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
 }
 
 template <int K1, int MINB, bool DBL>
-cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem)
+cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem, bool any_copy)
 {
-    auto kern = sweep_fused_cell_kernel<K1, MINB, DBL>;
+    auto kern = any_copy ? sweep_fused_cell_kernel<K1, MINB, DBL, true> : sweep_fused_cell_kernel<K1, MINB, DBL, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long grid = (P.planes + P.PB - 1) / P.PB;
@@ -299,7 +312,7 @@ cudaError_t launch(sldg_ctx* c, const CellParams& P, int threads, size_t smem)
 // g0, g1: geometry of axis 0 and axis 1.  Returns cudaErrorNotSupported when the shape does not fit (the caller
 // falls back to the node-per-thread fused kernel, then to separate sweeps).
 static cudaError_t launch_cell(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0, const SweepGeom& g1,
-                               const ShiftTable& t0, const ShiftTable& t1, bool dbl)
+                               const ShiftTable& t0, const ShiftTable& t1, bool dbl, bool any_copy)
 {
     if (g1.outer == 0) return cudaSuccess;
     const long long D0 = (long long)g0.N * g0.K1, D1 = (long long)g1.N * g1.K1;
@@ -338,30 +351,30 @@ static cudaError_t launch_cell(sldg_ctx* c, const void* fin, void* fout, const S
     const size_t smem = smem_of(PB, CR, stages);
     if (dbl) {
         switch (K1) {
-        case 1: return launch<1, 4, true>(c, P, threads, smem);
-        case 2: return launch<2, 4, true>(c, P, threads, smem);
-        case 3: return launch<3, 2, true>(c, P, threads, smem);
+        case 1: return launch<1, 4, true>(c, P, threads, smem, any_copy);
+        case 2: return launch<2, 4, true>(c, P, threads, smem, any_copy);
+        case 3: return launch<3, 2, true>(c, P, threads, smem, any_copy);
         }
         return cudaErrorNotSupported;
     }
     switch (K1) {
-    case 1: return launch<1, 4, false>(c, P, threads, smem);
-    case 2: return launch<2, 4, false>(c, P, threads, smem);
-    case 3: return launch<3, 3, false>(c, P, threads, smem);
-    case 4: return launch<4, 2, false>(c, P, threads, smem);
+    case 1: return launch<1, 4, false>(c, P, threads, smem, any_copy);
+    case 2: return launch<2, 4, false>(c, P, threads, smem, any_copy);
+    case 3: return launch<3, 3, false>(c, P, threads, smem, any_copy);
+    case 4: return launch<4, 2, false>(c, P, threads, smem, any_copy);
     }
     return cudaErrorNotSupported;
 }
 
 cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,
-                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+                                                   const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy)
 {
-    return launch_cell(c, fin, fout, g0, g1, t0, t1, false);
+    return launch_cell(c, fin, fout, g0, g1, t0, t1, false, any_copy != 0);
 }
 
 // The sweep pair applied twice (x_1, x_2, x_1, x_2) in one pass: two consecutive x half steps with the same tables.
 cudaError_t SLDG_SFX(sldg_launch_sweep_fused_cell2)(sldg_ctx* c, const void* fin, void* fout, const SweepGeom& g0,
-                                                    const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1)
+                                                    const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy)
 {
-    return launch_cell(c, fin, fout, g0, g1, t0, t1, true);
+    return launch_cell(c, fin, fout, g0, g1, t0, t1, true, any_copy != 0);
 }
