@@ -193,10 +193,12 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     issue_load(ST);
 
     int io3 = s3 + 1; if (io3 >= N2) io3 -= N2;            // output x_3 cell of the current donor pair
-    for (int h = 0; h < N2; h++) {
+    // one step of the x_3 walk: nxt <- swept block of input cell h+1 (or the first one), output cell from (nxt, prv).
+    // The walk alternates between `prev` and `alt` (two steps per trip): no register moves between steps.
+    real alt[N3];
+    auto step3 = [&](int h, real (&nxt)[N3], const real (&prv)[N3]) {
         const int j = h + 1;
         const int st = j % ST;
-        real nxt[N3];
         if (j < N2) {
             if (active) {
                 mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
@@ -219,14 +221,12 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
 #pragma unroll
                         for (int l = 0; l < K1; l++) acc += A3[j3 * K1 + l] * nxt[(l * K1 + j2) * K1 + j1];
 #pragma unroll
-                        for (int l = 0; l < K1; l++) acc += B3[j3 * K1 + l] * prev[(l * K1 + j2) * K1 + j1];
+                        for (int l = 0; l < K1; l++) acc += B3[j3 * K1 + l] * prv[(l * K1 + j2) * K1 + j1];
                         r.v[j1] = (CP && cp3) ? nxt[(j3 * K1 + j2) * K1 + j1] : acc;
                     }
                     r.store(obase + j3 * OP + j2 * D0);
                 }
         }
-#pragma unroll
-        for (int m = 0; m < N3; m++) prev[m] = nxt[m];
         fence_async_smem();
         if (lead) bulk_wait_read<0>();                     // the stores of step h-1 have left their output stage
         __syncthreads();
@@ -239,6 +239,11 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
         }
         issue_load(j + ST);
         io3++; if (io3 >= N2) io3 = 0;
+    };
+    {
+        int h = 0;
+        for (; h + 1 < N2; h += 2) { step3(h, alt, prev); step3(h + 1, prev, alt); }
+        if (h < N2) step3(h, alt, prev);
     }
     if (lead) bulk_wait_read<0>();
 }

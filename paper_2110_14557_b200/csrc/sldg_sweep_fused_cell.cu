@@ -250,6 +250,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         }
         int ncells = nout;                             // cells the leader stores for this group
         if constexpr (DBL) {
+            fence_async_smem();                        // the generic-proxy reads of the input stage -> its refill by the async proxy
             __syncthreads();                           // the mid stage is complete, the input stage is free
             issue_load(j + ST);
             real* o2 = sout + (h & 1) * SSO + pl * PCO + i * K1;

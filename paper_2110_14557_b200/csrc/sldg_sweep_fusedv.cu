@@ -199,6 +199,11 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
                 for (int m = 0; m < K1; m++) { a[m] = pa0[ro + m * WX]; b[m] = pb0[ro + m * WX]; }
                 const bool last = jr == RPS - 1 && csub == cps - 1;
                 if (last) {                                             // the slot is read: hand it back
+                    // The slot is refilled by the ASYNC proxy (TMA) once every warp has arrived: the generic-proxy reads
+                    // above must be ordered before that write by a proxy fence.  Without it single lanes read a row of the
+                    // NEXT copy (seen at full size only, where long multi-plane walks let the warps drift apart: a few
+                    // wrong values per launch, caught by the mass check of tests/test_gpu_fullsize.py).
+                    fence_async_smem();
                     __syncwarp();
                     if (warp_lead) mbar_arrive(fbar + 8u * (uint32_t)ST);
                 }

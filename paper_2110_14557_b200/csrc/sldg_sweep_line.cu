@@ -255,6 +255,7 @@ __global__ void __launch_bounds__(WARPS * 32) sweep_line_kernel(const LineParams
             if (lane == 0) bulk_store(P.fout + c * chunk_vals, wbase_s + (uint32_t)((STAGES + ost) * cap) * (uint32_t)sizeof(real),
                                       (uint32_t)nval * (uint32_t)sizeof(real));
         } else {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy reads of sin_ -> a refill by the async proxy
             __syncwarp();
             real* gout = P.fout + c * chunk_vals;
             for (int t = lane; t < nval; t += 32) gout[t] = sout[t];

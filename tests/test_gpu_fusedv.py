@@ -207,3 +207,26 @@ def test_fused_v_pass_inside_a_captured_step_graph(P):
             g.step(fg, cfg["dt"])
         outs.append(fg.cpu().numpy())
     assert np.array_equal(outs[0], outs[1])
+
+
+def test_fused_v_ring_under_drift_long_multi_plane_walks(P):
+    """Regression for a cross-proxy write-after-read race: a ring slot read by the generic proxy was handed back to the
+    TMA (async proxy) without a proxy fence, so single lanes could read rows of the NEXT copy.  It needed warps that
+    drift apart (long walks over many planes, few ring slots, memory contention) and showed only at full size, as a
+    mass error of 1e-9 in tests/test_gpu_fullsize.py.  Here: 1.1 GB, 144 blocks walking 64 planes each, strong seeded
+    field, several ring depths; every run must give the bits of the separate walks."""
+    dx, dv, cells, k = 2, 3, [24, 24, 20, 12, 32], 1
+    g, o = make_pair(P, dx, dv, cells, k)
+    f0 = W.random_field(g.shape, seed=77, device=g.device)
+    hv = (2 * (2.0 + dx)) / cells[dx]
+    E = W.random_E(dx, g.xshape, seed=12, amplitude=3.0 * hv / 0.1, device=g.device)
+    g.set_option("fuse_v", 0)
+    want = f0.clone()
+    g.advect_v(want, E, 0.1)
+    g.set_option("fuse_v", 2)
+    for stages, ppb in ((3, 64), (4, 64), (8, 64), (3, 16), (0, 0)):
+        g.set_option("fv_stages", stages); g.set_option("fv_ppb", ppb)
+        for _ in range(4):
+            got = f0.clone()
+            g.advect_v(got, E, 0.1)
+            assert torch.equal(got, want), (stages, ppb, int((got != want).sum()))
