@@ -189,6 +189,7 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     }
 #pragma unroll
     for (int m = 0; m < N3; m++) prev[m] = first[m];
+    fence_async_smem();                                    // generic-proxy reads of stage 0 -> its refill by the async proxy
     __syncthreads();
     issue_load(ST);
 

@@ -194,6 +194,7 @@ __global__ void __launch_bounds__(128, MINB) sweep_fused_cell_kernel(const CellP
         if constexpr (FS) first_s[m * blockDim.x + t] = prev[m];
         else first[m] = prev[m];
     }
+    fence_async_smem();                                // generic-proxy reads of stage 0 -> its refill by the async proxy
     __syncthreads();
     issue_load(ST);
 
