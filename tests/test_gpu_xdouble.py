@@ -121,3 +121,25 @@ def test_plan_query_counts_are_those_of_the_real_calls(P, geom, n, fuse_v, x_dou
     assert kinds["sweep_fused_v"][0] + kinds["sweep_slow_axis"][0] >= want["v_passes"]
     assert kinds["copies"][0] == dx                                # only the x shift-table uploads (one event per axis)
     assert kinds["rho"][0] == max(1, n)
+
+
+@pytest.mark.parametrize("ci", [1, 2, 3], ids=lambda i: W.CONFIGS[i]["name"])
+def test_merged_steps_equal_single_steps_at_full_size(P, ci):
+    """BASELINE configs 2-4 at FULL size in the launch configuration bench.py times (sldg_steps: double x half steps,
+    fused v passes, alternating buffers): three merged steps, repeated, must give the bits of three sldg_step calls.
+    Long walks under memory contention are where a missing proxy fence once showed."""
+    cfg = W.CONFIGS[ci]
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    f0 = g.empty_field()
+    W.initial_data(cfg, [g.node_coords(a) for a in range(g.d)], device=f0.device, out=f0)
+    W.perturb_inplace(f0)
+    ref = f0.clone()
+    for _ in range(3):
+        g.step(ref, cfg["dt"])
+    m_ref = g.mass(ref)
+    for rep in range(3):
+        f = f0.clone()
+        g.steps(f, cfg["dt"], 3)
+        assert torch.equal(f, ref), (rep, int((f != ref).sum()))
+        del f
+    assert abs(m_ref - g.mass(f0)) <= 1e-12 * abs(m_ref)
