@@ -898,10 +898,15 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
         // x(dt/2) | rho, E, v(dt) | x(dt/2) x(dt/2) as one pass | rho, E, v(dt) | ... | x(dt/2): the same sweeps in the
         // same order as nsteps single steps.  The last half step restores the buffer parity.
         if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, true))) return r;
+        // The closing half step is one pass only if it may flip the buffers, i.e. if the flips before it are odd in
+        // number: 1 + nsteps * v_flips + (nsteps - 1).  With the fused v pass (one flip) that count is even: the LAST v
+        // advection then runs as two walks (one flip and 0.7 pass more) and the closing half step saves a whole pass.
+        const bool fused_v = fusedv_possible(c);
+        const bool last_v_walks = fused_v && ((1 + nsteps * v_flips(c, true) + (nsteps - 1)) % 2 == 0);
         for (int s = 0; s < nsteps; s++) {
             if ((r = sldg_density(c, cur, c->rho))) return r;
             if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
-            if ((r = advect_v_impl(c, &cur, &oth, c->E, dt))) return r;
+            if ((r = advect_v_impl(c, &cur, &oth, c->E, dt, !(last_v_walks && s == nsteps - 1)))) return r;
             if (s < nsteps - 1) r = advect_x_double(c, &cur, &oth, dt / 2.0);
             else r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f);
             if (r) return r;

@@ -98,4 +98,4 @@ def test_merged_plans_reproduce_the_step_by_step_run_bitwise(P):
     assert abs(g.mass(fb) - m0) / abs(m0) < 1e-12
     assert (n2 - n1) < (n1 - n0) - 100                            # 59 merged x passes and 60 fused v passes fewer
     want = P.plan_query(2, 2, cfg["cells"], 2, 60)
-    assert (want["x_passes"], want["v_passes"], want["copies"]) == (62, 60, 0)
+    assert (want["x_passes"], want["v_passes"], want["copies"]) == (61, 61, 0)

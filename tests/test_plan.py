@@ -29,10 +29,11 @@ def test_single_step_budget(name):
     assert (r["x_passes"], r["v_passes"], r["rho_passes"], r["field_solves"], r["copies"]) == (2, 2, 1, 1, 0)
 
 
-@pytest.mark.parametrize("name,x,v", [("cfg2", 12, 10), ("cfg3", 12, 10), ("cfg4", 20, 20), ("cfg5", 20, 20)])
+@pytest.mark.parametrize("name,x,v", [("cfg2", 11, 11), ("cfg3", 11, 11), ("cfg4", 20, 20), ("cfg5", 20, 20)])
 def test_ten_steps_budget(name, x, v):
-    """sldg_steps(10).  dim_x = 2: first half step 1 pass, 9 merged double half steps, closing half step 2 passes
-    (19 flips so far: it must not flip), 10 fused v passes.  dim_x = 3: 2 x passes and 2 v passes per step."""
+    """sldg_steps(10).  dim_x = 2: first half step 1 pass, 9 merged double half steps, 9 fused v passes and the last v
+    advection as two walks (so that the flips before the closing half step are odd and it is ONE pass).  dim_x = 3: 2 x
+    passes and 2 v passes per step."""
     r = q(CFG[name], 10)
     assert (r["x_passes"], r["v_passes"], r["rho_passes"], r["field_solves"], r["copies"]) == (x, v, 10, 10, 0)
 
@@ -50,8 +51,8 @@ def test_options_change_the_budget_as_documented():
     assert (r["x_passes"], r["v_passes"]) == (3, 1)
     r = q(c2, 10, precision="f32")               # single precision: no automatic fused v for dim_x = 2
     assert (r["x_passes"], r["v_passes"]) == (12, 20)
-    r = q(c2, 2)                                 # two steps: one merged pass, closing half step restores the parity
-    assert (r["x_passes"], r["v_passes"], r["copies"]) == (4, 2, 0)
+    r = q(c2, 2)                                 # two steps: one merged pass, the last v as walks, one-pass closing half step
+    assert (r["x_passes"], r["v_passes"], r["copies"]) == (3, 3, 0)
 
 
 def test_degree_three_fuses_v_but_not_the_x_half_steps():
