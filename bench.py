@@ -4,11 +4,13 @@
     python bench.py --gpus N --steps K --warmup W [--impl reference] [--config I]
 
 A "step" is one Strang step (3*d_x sweeps + rho + Poisson + shift tables) of the
-SLDG Vlasov-Poisson path on synthetic data of BASELINE.json configs[I] (default I=1: 4-d two-stream,
-64^4 cells, k=2, 192^4 values = 10.9 GB fp64).  Metric: effective HBM GB/s per 1-D advection sweep,
-2*|f|*8 B per sweep / time (BASELINE.json `metric`); `value` uses the WHOLE step time (rho, Poisson and
-table kernels included), `sweeps` lists the pure per-axis kernel figures from CUDA events on the launching
-stream.  Multi-GPU: the path does not shard in this build ("replicas only"): every rank
+SLDG Vlasov-Poisson path on synthetic data of BASELINE.json configs[I] (default I=4: cfg5, 6-d two-stream,
+24^3 x 20^3 cells, k=1, 48^3*40^3 values = 56.6 GB fp64: the largest configuration that fits one B200; the
+other four configs are run briefly in the same invocation and attached under `configs`).  Metric: effective
+HBM GB/s per 1-D advection sweep, 2*|f|*8 B per sweep / time (BASELINE.json `metric`); `value` uses the WHOLE
+step time (rho, Poisson and table kernels included).  Because fused / merged passes perform several sweeps per
+trip over f, the line also carries the PHYSICAL traffic (`physical_bytes_per_step`, `physical_frac`, and per
+launch kind under `kernels`): passes * 2*|f|*8 B + the rho read, over the measured copy rate.  Multi-GPU: the path does not shard in this build ("replicas only"): every rank
 runs an independent replica, value = total bytes of all ranks / max-over-ranks time.
 """
 import argparse
@@ -133,13 +135,13 @@ def oracle_sample_cfg(cfg, target_values=2.0e7):
     return W.scaled(cfg, cells)
 
 
-def time_oracle(cfg, steps, warmup, budget_s=25.0):
+def time_oracle(cfg, steps, warmup, budget_s=25.0, threads=None):
     """Time the oracle AS IT STANDS (oracle/sldg_oracle.c, all host threads) on a bounded sample.
     -> dict(value [GB/s effective per sweep], ms_per_step, cores, sample, steps)."""
     import workloads as W
     from oracle import oracle as O
     s = oracle_sample_cfg(cfg)
-    cores = O.lib().orc_max_threads()
+    cores = threads if threads else O.lib().orc_max_threads()
     o = O.Oracle(s["dim_x"], s["dim_v"], s["cells"], s["degree"], s["domain"], threads=cores)
     f = W.initial_data(s, [o.node_coords(a) for a in range(o.d)]).numpy()
     ostep = o.step
@@ -158,7 +160,7 @@ def time_oracle(cfg, steps, warmup, budget_s=25.0):
     value = sweeps_per_step(s) * sweep_bytes(s) / (ms * 1e-3) / 1e9
     return {"value": value, "unit": UNIT, "ms_per_step": ms, "cores": cores, "kind": "oracle", "steps": done,
             "sample": f"scaled replica of {cfg['name']}: cells {s['cells']} ({W.field_elems(s)} values), "
-                      f"{done} Strang step(s), all {cores} host threads"}
+                      f"{done} Strang step(s), {cores} host thread(s)"}
 
 
 def run_reference(args, cfg, rank, world):
@@ -194,20 +196,9 @@ def ncu_traffic(cfg_name, kernel):
     return None
 
 
-def run_ours(args, cfg, rank, world, local):
-    import torch
-    import workloads as W
-    import paper_2110_14557_b200 as P
-
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the SLDG path has no CPU fallback (use --impl reference "
-                         "to time the CPU oracle)")
-    dev = torch.device("cuda", local)
-    torch.cuda.set_device(dev)
-    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], device=dev, precision=args.dtype)
+def fill_initial(W, g, cfg, f, dtype, dev):
     coords = [g.node_coords(a) for a in range(g.d)]
-    f = g.empty_field()
-    if args.dtype == "f32":               # the generator works in fp64: fill slab by slab along the slowest axis
+    if dtype == "f32":                    # the generator works in fp64: fill slab by slab along the slowest axis
         D = f.shape[0]
         step = max(1, D // 8)
         for a in range(0, D, step):
@@ -215,71 +206,134 @@ def run_ours(args, cfg, rank, world, local):
             f[a:b].copy_(W.initial_data(cfg, coords[:-1] + [coords[-1][a:b]], device=dev))
     else:
         W.initial_data(cfg, coords, device=dev, out=f)
+
+
+SWEEP_KINDS_PREFIX = "sweep"
+
+
+def measure_config(args, cfg, dev, local, steps, warmup, headline):
+    """One workload on this rank's GPU: K Strang steps through sldg_steps (timed with CUDA events on the library's stream),
+    the same K steps as K sldg_step calls, and once more with events around every launch.
+    -> (dict of figures, ms of the timed region, effective bytes of the timed region, solver, field) ."""
+    import torch
+    import workloads as W
+    import paper_2110_14557_b200 as P
+
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], device=dev, precision=args.dtype)
+    f = g.empty_field()
+    fill_initial(W, g, cfg, f, args.dtype, dev)
     if args.poisson == "cg":
         g.set_poisson_solver(1, tol=1e-3)
     dt = cfg["dt"]
     nf = W.field_elems(cfg)
     nsweeps = sweeps_per_step(cfg)
     bytes_step = nsweeps * sweep_bytes(cfg)
+    pass_bytes = 2 * nf * ESIZE               # one pass over f: every value read once and written once
 
     # warm-up through the SAME entry point as the timed region (sldg_steps plans merged passes that single sldg_step calls
     # never launch: their kernels would otherwise be loaded -- CUDA loads a kernel lazily at its first launch -- inside the
     # timed region), then one single step for the kernels only that path uses
-    g.steps(f, dt, max(args.warmup, 3))
+    g.steps(f, dt, max(warmup, 3))
     g.step(f, dt)
     torch.cuda.synchronize(dev)
     # ---- timed region: K Strang steps, no instrumentation inside
     launches0 = g.launch_count()
     sampler = ClockSampler(local)
     sampler.start()
-    barrier()
+    if headline:
+        barrier()
     torch.cuda.synchronize(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(g.stream)
-    g.steps(f, dt, args.steps)                # K Strang steps through the multi-step entry point (sldg_steps)
+    g.steps(f, dt, steps)                     # K Strang steps through the multi-step entry point (sldg_steps)
     e1.record(g.stream)
     torch.cuda.synchronize(dev)
-    barrier()
+    if headline:
+        barrier()
     ms_total_local = e0.elapsed_time(e1)
     launches = g.launch_count() - launches0
     # ---- for comparison: the same K steps as K separate sldg_step calls (f at every integer time t_n is materialised in
     # the caller's buffer, as a per-step diagnostic would need; no merging of x half steps across steps)
     s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     s0.record(g.stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         g.step(f, dt)
     s1.record(g.stream)
     torch.cuda.synchronize(dev)
-    ms_single_calls = s0.elapsed_time(s1) / args.steps
+    ms_single_calls = s0.elapsed_time(s1) / steps
     # ---- the same K steps again with CUDA events around every launch (on the library's stream): per-kernel figures
     g.timing_enable(True)
     g.timing_read()
-    g.steps(f, dt, args.steps)
+    g.steps(f, dt, steps)
     kinds, axes = g.timing_read()
     g.timing_enable(False)
     clocks = sampler.stop()
-    ms_total, bytes_all = aggregate(ms_total_local, bytes_step * args.steps, device=dev)
-    ms_step = ms_total / args.steps
-    value = bytes_all / (ms_total * 1e-3) / 1e9
+    ms_step = ms_total_local / steps
 
     peak, peak_src = measured_peak()
-    # per-axis pure kernel figures (CUDA events around every sweep launch, on the launching stream)
+    # PHYSICAL traffic: every sweep launch (single, fused or merged) is one pass over f = |f| values read + |f| written;
+    # the rho launch reads f once.  This is what the HBM actually moves, and what the roofline fraction is taken of.
+    passes = {k: v for k, v in kinds.items() if k.startswith(SWEEP_KINDS_PREFIX) and v[0]}
+    n_pass = sum(n for n, _ in passes.values())
+    n_rho = kinds.get("rho", (0, 0.0))[0]
+    phys_step = (n_pass * pass_bytes + n_rho * nf * ESIZE) / steps
+    kernels = {}
+    for k, (n, ms) in passes.items():
+        gbs = pass_bytes / (ms / n * 1e-3) / 1e9
+        kernels[k] = {"launches": n, "avg_ms": ms / n, "physical_gbs": gbs, "frac_of_measured_peak": gbs / peak,
+                      "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS, "bytes_per_launch": pass_bytes}
+    if n_rho:
+        n, ms = kinds["rho"]
+        gbs = nf * ESIZE / (ms / n * 1e-3) / 1e9
+        kernels["rho"] = {"launches": n, "avg_ms": ms / n, "physical_gbs": gbs, "frac_of_measured_peak": gbs / peak,
+                          "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS, "bytes_per_launch": nf * ESIZE}
+    # EFFECTIVE per-axis figures (BASELINE.json's metric: 2*|f|*8 B per 1-D sweep / time): a fused or merged launch books
+    # an equal share of its time on each sweep it performs, so these exceed the HBM peak by the fusion factor
     sweeps = {}
     names = [f"x{a + 1}" for a in range(cfg["dim_x"])] + [f"v{a + 1}" for a in range(cfg["dim_v"])]
     for a, (n, ms) in enumerate(axes):
         if n:
             gbs = sweep_bytes(cfg) / (ms / n * 1e-3) / 1e9
-            sweeps[names[a]] = {"launches": n, "ms": ms / n, "gbs": gbs, "pct_of_measured_peak": 100 * gbs / peak,
-                                "pct_of_nominal_8TBs": 100 * gbs / NOMINAL_HBM_GBS}
-    # dominant kernel = the one with the largest share of the step
-    kn, (kl, kms) = max(((k, v) for k, v in kinds.items() if k.startswith("sweep")), key=lambda kv: kv[1][1])
-    achieved = sweep_bytes(cfg) / (kms / kl * 1e-3) / 1e9
+            sweeps[names[a]] = {"sweeps": n, "ms_share": ms / n, "effective_gbs": gbs}
+    # dominant kernel = the sweep kind with the largest share of the step
+    kn, (kl, kms) = max(passes.items(), key=lambda kv: kv[1][1])
+    achieved = pass_bytes / (kms / kl * 1e-3) / 1e9
     tr = ncu_traffic(cfg["name"], kn)
     roofline = {"bound": "hbm", "kernel": kn, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": tr.get("traffic_bytes_per_launch") if tr else None,
-                "algorithmic_bytes_per_launch": sweep_bytes(cfg), "peak_source": peak_src,
-                "launches": kl, "avg_ms": kms / kl, "timed_by": "CUDA events around every launch, K steps run right after the timed region", "share_of_step": kms / sum(v[1] for v in kinds.values())}
-    parts = {k: {"launches": n, "ms_per_step": ms / args.steps} for k, (n, ms) in kinds.items() if n}
+                "traffic_source": (tr.get("source") if tr else None),
+                "algorithmic_bytes_per_launch": pass_bytes, "peak_source": peak_src,
+                "launches": kl, "avg_ms": kms / kl,
+                "timed_by": "CUDA events around every launch, K steps run right after the timed region",
+                "share_of_step": kms / sum(v[1] for v in kinds.values())}
+    parts = {k: {"launches": n, "ms_per_step": ms / steps} for k, (n, ms) in kinds.items() if n}
+    res = {"workload": cfg["name"], "values": nf, "bytes_f": nf * ESIZE, "ms_per_step": ms_step,
+           "single_step_ms": ms_single_calls,
+           "effective_gbs_per_sweep": bytes_step / (ms_step * 1e-3) / 1e9,
+           "passes_per_step": n_pass / steps, "rho_passes_per_step": n_rho / steps,
+           "physical_bytes_per_step": phys_step, "physical_gbs": phys_step / (ms_step * 1e-3) / 1e9,
+           "physical_frac": phys_step / (ms_step * 1e-3) / 1e9 / peak,
+           "kernels": kernels, "sweeps_effective": sweeps, "parts": parts, "roofline": roofline, "clocks": clocks,
+           "gpu_launches": launches, "steps": steps}
+    return res, ms_total_local, bytes_step * steps, g, f
+
+
+def run_ours(args, cfg, rank, world, local):
+    import torch
+    import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SLDG path has no CPU fallback (use --impl reference "
+                         "to time the CPU oracle)")
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    res, ms_total_local, bytes_local, g, f = measure_config(args, cfg, dev, local, args.steps, args.warmup, True)
+    ms_total, bytes_all = aggregate(ms_total_local, bytes_local, device=dev)
+    ms_step = ms_total / args.steps
+    value = bytes_all / (ms_total * 1e-3) / 1e9
+    peak, _ = measured_peak()
+    nf, dt = res["values"], cfg["dt"]
+    parts = res["parts"]
     # the paper's own figure (PAPER.md:201-203): F * sizeof(fp) * dof / time per step, F = 20 for 3x3v and 14 otherwise,
     # where its step holds a second rho/E evaluation for the diagnostics (PAPER.md:199): one measured rho pass and one
     # field solve are added to our step time.  Context only (the paper: 727 GB/s on A100 for 2x3v fp64, 626 GB/s for 3x3v).
@@ -293,25 +347,33 @@ def run_ours(args, cfg, rank, world, local):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
         "data": "synthetic",
-        "config": {"workload": cfg["name"], "values": nf, "bytes_f": nf * ESIZE, "sweeps_per_step": nsweeps,
+        "config": {"workload": cfg["name"], "values": nf, "bytes_f": nf * ESIZE, "sweeps_per_step": sweeps_per_step(cfg),
                    "dt": dt, "poisson": args.poisson,
                    "steps_api": "sldg_steps: K Strang steps in one call, bit-identical to K sldg_step calls; the x half "
-                                "steps of consecutive steps share one pass (dim_x = 2), so f at the intermediate integer "
-                                "times is not written out (no per-step diagnostics inside the timed region)", "l2": "inputs larger than L2 (no flush needed)" if nf * ESIZE > 2 * 126e6 else
+                                "steps of consecutive steps share one pass, so f at the intermediate integer "
+                                "times is not written out (no per-step diagnostics inside the timed region)",
+                   "l2": "inputs larger than L2 (no flush needed)" if nf * ESIZE > 2 * 126e6 else
                    "array fits in L2: numbers are L2-resident, launch-bound",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "value_is": "EFFECTIVE bandwidth per 1-D sweep (BASELINE.json metric): sweeps_per_step * 2*|f|*8 B / step time; fused "
+                    "and merged passes perform several sweeps per trip over f, so it exceeds the HBM peak. The bytes the "
+                    "HBM really moves are physical_bytes_per_step; physical_frac is their rate over the measured copy rate",
         "pct_of_measured_peak": 100 * value / world / peak, "pct_of_nominal_8TBs": 100 * value / world / NOMINAL_HBM_GBS,
-        "single_step_calls": {"ms_per_step": ms_single_calls, "note": "K separate sldg_step calls, each ending in the caller's buffer"},
+        "physical_bytes_per_step": res["physical_bytes_per_step"], "physical_gbs": res["physical_gbs"],
+        "physical_frac": res["physical_frac"], "passes_per_step": res["passes_per_step"],
+        "single_step_calls": {"ms_per_step": res["single_step_ms"], "note": "K separate sldg_step calls, each ending in the caller's buffer"},
         "paper_style": paper_style,
-        "sweeps": sweeps, "parts": parts, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
+        "kernels": res["kernels"], "sweeps_effective": res["sweeps_effective"], "parts": parts, "roofline": res["roofline"],
+        "clocks": res["clocks"], "gpu_launches": res["gpu_launches"],
     }
 
     # end to end through the C-ABI with HOST buffers (sldg_step_host): H2D of f, one Strang step, D2H of f, per step
+    bytes_step = sweeps_per_step(cfg) * sweep_bytes(cfg)
     if rank == 0 or world > 1:
         try:
             fh = torch.empty(g.shape, dtype=f.dtype, pin_memory=True)
             fh.copy_(f)
-            nrep = max(1, min(args.steps, 3))
+            nrep = max(1, min(args.steps, 2 if nf * ESIZE > 2e10 else 3))
             g.step_host(fh, f, dt, nsteps=1)                    # warm-up
             torch.cuda.synchronize(dev)
             t0 = time.perf_counter()
@@ -327,9 +389,41 @@ def run_ours(args, cfg, rank, world, local):
         except Exception as ex:                                  # e.g. not enough pinned host memory
             line["e2e"] = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
 
+    # the other BASELINE.json configs, briefly, in the same invocation (rank 0, single GPU): one block per config
+    if rank == 0 and world == 1 and args.all_configs and not args.workload and not args.cells:
+        g.close()
+        del g, f
+        torch.cuda.empty_cache()
+        others = {}
+        for i, oc in enumerate(W.CONFIGS):
+            if oc["name"] == cfg["name"]:
+                continue
+            try:
+                r, _, _, g2, f2 = measure_config(args, oc, dev, local, min(args.steps, 10), 3, False)
+                g2.close()
+                del g2, f2
+                torch.cuda.empty_cache()
+                rf = r["roofline"]
+                others[oc["name"]] = {"ms_per_step": r["ms_per_step"], "single_step_ms": r["single_step_ms"],
+                                      "effective_gbs_per_sweep": r["effective_gbs_per_sweep"],
+                                      "passes_per_step": r["passes_per_step"],
+                                      "physical_bytes_per_step": r["physical_bytes_per_step"],
+                                      "physical_gbs": r["physical_gbs"], "physical_frac": r["physical_frac"],
+                                      "roofline": {"kernel": rf["kernel"], "frac": rf["frac"], "avg_ms": rf["avg_ms"],
+                                                   "achieved": rf["achieved"]},
+                                      "kernels": {k: {"avg_ms": v["avg_ms"], "frac_of_measured_peak": v["frac_of_measured_peak"],
+                                                      "launches": v["launches"]} for k, v in r["kernels"].items()},
+                                      "clocks": r["clocks"], "steps": r["steps"],
+                                      "note": "L2-resident, launch-bound" if r["bytes_f"] < 2 * 126e6 else ""}
+            except Exception as ex:
+                others[oc["name"]] = {"error": str(ex)[:200]}
+        line["configs"] = others
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r = time_oracle(cfg, steps=1000, warmup=1, budget_s=15.0)
+        r = time_oracle(cfg, steps=1000, warmup=1, budget_s=12.0)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "ms_per_step")}
+        r1 = time_oracle(cfg, steps=1000, warmup=0, budget_s=8.0, threads=1)
+        line["cpu_baseline"]["single_thread"] = {k: r1[k] for k in ("value", "unit", "cores", "ms_per_step", "sample")}
     return line if rank == 0 else None
 
 
@@ -339,7 +433,10 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: cfg5, the largest "
+                    "single-GPU configuration, 56.6 GB + as much workspace)")
+    ap.add_argument("--no-all-configs", dest="all_configs", action="store_false", help="skip the brief runs of the other "
+                    "BASELINE.json configs that the default run attaches under `configs`")
     ap.add_argument("--workload", type=str, default=None, help="a workload by name, incl. the NEXT-row cases "
                     "(bot_5d_k3_16, bot_6d_k3_9: the paper's bump-on-tail case, 4th order)")
     ap.add_argument("--cfl", type=float, default=None, help="choose dt so that the largest x shift is CFL cells (PAPER.md:351)")

@@ -110,6 +110,9 @@ int sldg_poisson(sldg_ctx* ctx, const double* rho, double* E);
 /* a7, Strang splitting: advect_x(dt/2); density; poisson; advect_v(dt);
  * advect_x(dt/2).  rho and E of the step stay in the workspace (sldg_last_rho / sldg_last_E). */
 int sldg_step(sldg_ctx* ctx, double* f, double dt);
+/* Small problems (|f| <= 256 MB; option graph) replay a CUDA graph of the step, captured at the first call with a
+ * given (f, dt).  1 if such a graph is instantiated right now (the next sldg_step with the same f, dt replays it). */
+int sldg_graph_active(const sldg_ctx* ctx);
 
 /* ---- CGdG Poisson solver (NEXT row, Appendix) --------------------------------
  * Alternative to sldg_poisson: symmetric interior penalty (SIPG) dG discretisation of

@@ -30,6 +30,7 @@ EXPORTS = {
     "sldg_density": (C.c_int, [_vp, _vp, _vp]),
     "sldg_poisson": (C.c_int, [_vp, _vp, _vp]),
     "sldg_step": (C.c_int, [_vp, _vp, C.c_double]),
+    "sldg_graph_active": (C.c_int, [_vp]),
     "sldg_steps": (C.c_int, [_vp, _vp, C.c_double, C.c_int]),
     "sldg_step_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int]),
     "sldg_field_elems": (_ll, [_vp]),
@@ -248,6 +249,9 @@ class Sldg:
 
     def step(self, f, dt):
         _check(lib().sldg_step(self._h, self._fp(f), float(dt)), self._h)
+
+    def graph_active(self):
+        return bool(lib().sldg_graph_active(self._h))
 
     def steps(self, f, dt, nsteps):
         _check(lib().sldg_steps(self._h, self._fp(f), float(dt), int(nsteps)), self._h)

@@ -6,6 +6,7 @@ library loads (and exports its symbols) on a box without a CUDA driver.
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
@@ -26,20 +27,25 @@ def _stale(target, deps):
 
 
 def build(force=False, verbose=False):
-    objs = []
+    objs, jobs = [], []
     extra = ["-Xptxas", "-v"] if verbose else []
-    extra += os.environ.get("SLDG_NVCC_EXTRA", "").split()      # experiments only (e.g. -DSLDG_WALK_U2=6)
     for s in SOURCES:
         src = os.path.join(CSRC, s)
         obj = os.path.join(CSRC, os.path.splitext(s)[0] + ".o")
         if force or _stale(obj, [src] + HEADERS):
-            subprocess.check_call([NVCC] + FLAGS + extra + ["-c", src, "-o", obj])
+            jobs.append([NVCC] + FLAGS + extra + ["-c", src, "-o", obj])
         objs.append(obj)
         if s in DUAL:          # second compilation: real = float (single precision mode, sldg_real.h)
             obj32 = os.path.join(CSRC, os.path.splitext(s)[0] + "_f32.o")
             if force or _stale(obj32, [src] + HEADERS):
-                subprocess.check_call([NVCC] + FLAGS + extra + ["-DSLDG_REAL_FLOAT", "-c", src, "-o", obj32])
+                jobs.append([NVCC] + FLAGS + extra + ["-DSLDG_REAL_FLOAT", "-c", src, "-o", obj32])
             objs.append(obj32)
+    # the translation units are independent: compile them side by side
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as pool:
+        for rc in pool.map(lambda cmd: subprocess.run(cmd, capture_output=not verbose, text=True), jobs):
+            if rc.returncode != 0:
+                sys.stderr.write((rc.stdout or "") + (rc.stderr or ""))
+                raise subprocess.CalledProcessError(rc.returncode, rc.args)
     if force or _stale(LIB, objs):
         subprocess.check_call([NVCC, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
     return LIB

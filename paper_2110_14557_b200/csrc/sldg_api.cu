@@ -124,7 +124,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     c->stream = 0; c->last_cuda = 0; c->sm_count = 148;
     c->ws = nullptr; c->ws_bytes = 0; c->ws_ready = false;
     c->timing = false; c->launches = 0;
-    c->graph_exec = nullptr; c->graph_f = nullptr; c->graph_dt = 0.0; c->graph_launches = 0; c->opt_graph = 1;
+    c->cap_stream = nullptr; c->graph_exec = nullptr; c->graph_f = nullptr; c->graph_dt = 0.0; c->graph_launches = 0; c->opt_graph = 1;
     c->phi = nullptr; c->cg_info = nullptr; c->poisson_solver = 0; c->cg_tol = 1e-3; c->cg_sigma = sldg_sipg_sigma_default(degree);
     c->cg_maxiter = 0;
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
@@ -135,7 +135,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
-    c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
+    c->dPoly = nullptr; c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
 
     if (host_only) { *out = c; return SLDG_OK; }                            // sldg_plan_query
 
@@ -145,7 +145,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     if (e == cudaSuccess) {
         int sm = 0;
         if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sm > 0) c->sm_count = sm;
-        e = sldg_upload_poly(&c->poly);
+        e = sldg_upload_poly(c);
     }
     const size_t NN2 = 2 * (size_t)c->K1 * c->K1;
     long long maxD = 0;
@@ -206,6 +206,7 @@ extern "C" int sldg_destroy(sldg_ctx* c)
 {
     if (!c) return SLDG_EINVAL;
     sldg_graph_drop(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     for (int a = 0; a < SLDG_MAX_DIM; a++) {
         if (c->dS[a]) cudaFree(c->dS[a]);
         if (c->dAB[a]) cudaFree(c->dAB[a]);
@@ -218,6 +219,7 @@ extern "C" int sldg_destroy(sldg_ctx* c)
     }
     if (c->dS_hook) cudaFree(c->dS_hook);
     if (c->dAB_hook) cudaFree(c->dAB_hook);
+    if (c->dPoly) cudaFree(c->dPoly);
     if (c->dScalar) cudaFree(c->dScalar);
     if (c->dCounter) cudaFree(c->dCounter);
     if (c->hS) cudaFreeHost(c->hS);
@@ -853,13 +855,28 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
     ShiftTable tabs[3];
     if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;       // host tables + upload (synchronises): before the capture
     const long long l0 = c->launches;
-    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    // A capture cannot be started on the legacy default stream (or the per-thread one): the step is then recorded on a
+    // stream of the context's own.  Nothing executes during a capture, so no ordering between the two streams is needed;
+    // the instantiated graph is launched on the caller's stream.
+    cudaStream_t const user = c->stream;
+    cudaStream_t cap = user;
+    if (user == 0 || user == cudaStreamLegacy || user == cudaStreamPerThread) {
+        if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            c->cap_stream = nullptr;
+            cudaGetLastError();
+            return step_enqueue(c, f, dt);
+        }
+        cap = c->cap_stream;
+    }
+    if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
         cudaGetLastError();
         return step_enqueue(c, f, dt);
     }
+    c->stream = cap;
     r = step_enqueue(c, f, dt);
+    c->stream = user;
     cudaGraph_t g = nullptr;
-    cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    cudaError_t e = cudaStreamEndCapture(cap, &g);
     if (r || e != cudaSuccess || !g) {
         if (g) cudaGraphDestroy(g);
         cudaGetLastError();
@@ -874,6 +891,8 @@ extern "C" int sldg_step(sldg_ctx* c, double* f, double dt)
     CK(cudaGraphLaunch(c->graph_exec, c->stream));
     return SLDG_OK;
 }
+
+extern "C" int sldg_graph_active(const sldg_ctx* c) { return (c && c->graph_exec) ? 1 : 0; }
 
 // nsteps Strang steps.  Consecutive steps may leave their result in alternate buffers when that saves passes (for
 // dim_x = 3 both x half steps of a step can then be the one-pass fused x_1+x_2+x_3 sweep); the last step restores

@@ -5,13 +5,16 @@
 //  per-x-node shift tables of the v-sweeps
 #include "sldg_internal.h"
 
-__constant__ ABPoly c_poly;
+// The polynomial coefficients of A(alpha), B(alpha) depend on the degree: each context owns its device copy (c->dPoly),
+// so contexts of different degree can live side by side.
+cudaError_t sldg_upload_poly(sldg_ctx* c)
+{
+    cudaError_t e = cudaMalloc((void**)&c->dPoly, sizeof(ABPoly));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(c->dPoly, &c->poly, sizeof(ABPoly), cudaMemcpyHostToDevice);
+}
 
-cudaError_t sldg_upload_poly(const ABPoly* p) { return cudaMemcpyToSymbol(c_poly, p, sizeof(ABPoly)); }
-
-#ifndef SLDG_RHO_U
-#define SLDG_RHO_U 8
-#endif
+#define SLDG_RHO_U 8          // loads in flight per thread of the rho kernel
 
 namespace {
 
@@ -19,8 +22,8 @@ namespace {
 // delta = ((-E) * tau) / h_v in exactly this operation order (reading O3); s = floor(delta), alpha = delta - s.
 // A(alpha), B(alpha) by Horner on the polynomial coefficients.  Output SoA: AB[m][X].
 template <int K1, class TAB>
-__global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double hv, int N, long long X,
-                              int* __restrict__ S, TAB* __restrict__ AB)
+__global__ void vtable_kernel(const ABPoly* __restrict__ poly, const double* __restrict__ Ed, double tau, double hv, int N,
+                              long long X, int* __restrict__ S, TAB* __restrict__ AB)
 {
     long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (x >= X) return;
@@ -36,7 +39,7 @@ __global__ void vtable_kernel(const double* __restrict__ Ed, double tau, double 
     const double xc = alpha - 0.5;              // coefficients are in powers of (alpha - 1/2)
 #pragma unroll
     for (int m = 0; m < NN; m++) {
-        double a = sldg_horner<K1>(c_poly, 0, m, xc), b = sldg_horner<K1>(c_poly, 1, m, xc);
+        double a = sldg_horner<K1>(*poly, 0, m, xc), b = sldg_horner<K1>(*poly, 1, m, xc);
         if (cp) { a = (m % (K1 + 1) == 0) ? 1.0 : 0.0; b = 0.0; }
         AB[(long long)m * X + x] = (TAB)a;
         AB[(long long)(NN + m) * X + x] = (TAB)b;
@@ -317,11 +320,11 @@ static void vtable_dispatch(sldg_ctx* c, const double* Ed, double tau, double hv
     int block = 128;
     unsigned grid = (unsigned)((c->X + block - 1) / block);
     switch (c->K1) {
-    case 1: vtable_kernel<1, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 2: vtable_kernel<2, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 3: vtable_kernel<3, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 4: vtable_kernel<4, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
-    case 5: vtable_kernel<5, TAB><<<grid, block, 0, c->stream>>>(Ed, tau, hv, N, c->X, S, AB); break;
+    case 1: vtable_kernel<1, TAB><<<grid, block, 0, c->stream>>>(c->dPoly, Ed, tau, hv, N, c->X, S, AB); break;
+    case 2: vtable_kernel<2, TAB><<<grid, block, 0, c->stream>>>(c->dPoly, Ed, tau, hv, N, c->X, S, AB); break;
+    case 3: vtable_kernel<3, TAB><<<grid, block, 0, c->stream>>>(c->dPoly, Ed, tau, hv, N, c->X, S, AB); break;
+    case 4: vtable_kernel<4, TAB><<<grid, block, 0, c->stream>>>(c->dPoly, Ed, tau, hv, N, c->X, S, AB); break;
+    case 5: vtable_kernel<5, TAB><<<grid, block, 0, c->stream>>>(c->dPoly, Ed, tau, hv, N, c->X, S, AB); break;
     }
 }
 

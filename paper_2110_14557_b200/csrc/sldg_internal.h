@@ -21,7 +21,7 @@
 enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5, KIND_FUSED = 6, KIND_FUSEDV = 7, KIND_FUSEDX2 = 8 };
 
 // Polynomial coefficients of A_jl(alpha), B_jl(alpha) in powers of (alpha - 1/2), ascending, row-major
-// [2][K1*K1][SLDG_MAXPOLY]; the fp64 copy sits in __constant__ memory for the device-side table kernel.
+// [2][K1*K1][SLDG_MAXPOLY]; the fp64 copy is uploaded per context (dPoly) for the device-side table kernel.
 struct ABPoly {
     double c[2][SLDG_MAXNN][SLDG_MAXPOLY];
 };
@@ -92,6 +92,7 @@ struct sldg_ctx {
     double* dInvT[3];               // inverse DFT+transfer matrices, transposed
     double* dKap[3];                // signed wave numbers per x axis [D_a], Nyquist kept (zeroed in-kernel)
     double* dWx[SLDG_MAX_DIM];      // per-axis quadrature weights h_a w_j  [D_a]
+    ABPoly* dPoly;                  // device copy of `poly` (v-sweep table kernel); per context: the layout depends on k
     double* dScalar;                // 1 double result of mass / energy
     unsigned long long* dCounter;   // [2] work counter of the persistent axis-0 kernel (self-resetting)
     int* hS; double* hAB;           // pinned host staging for table uploads
@@ -126,6 +127,7 @@ struct sldg_ctx {
     long long a_launch[SLDG_MAX_DIM]; double a_ms[SLDG_MAX_DIM];
 
     // CUDA graph of one Strang step (small problems)
+    cudaStream_t cap_stream;        // capture stream of the context (used when the caller's stream is a default stream)
     cudaGraphExec_t graph_exec; const double* graph_f; double graph_dt; long long graph_launches;
     int opt_graph;                  // 0 = never, 1 = problems up to 256 MB (default), 2 = always
 
@@ -197,7 +199,7 @@ cudaError_t sldg_launch_sweep_fused(sldg_ctx* c, const double* fin, double* fout
                                     const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1);
 cudaError_t sldg_launch_sweep_fused_cell(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g0,
                                          const SweepGeom& g1, const ShiftTable& t0, const ShiftTable& t1, int any_copy);
-cudaError_t sldg_upload_poly(const ABPoly* p);
+cudaError_t sldg_upload_poly(sldg_ctx* c);         // device copy of c->poly, owned by the context (c->dPoly)
 cudaError_t sldg_launch_vtable(sldg_ctx* c, const double* Ed, double tau, double hv, int N, int* S, double* AB);
 cudaError_t sldg_launch_wv(sldg_ctx* c);
 cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho);

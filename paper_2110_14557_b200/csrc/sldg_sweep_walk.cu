@@ -41,24 +41,12 @@ template <> struct Vec<2> {
     }
 };
 
-#ifndef SLDG_WALK_U1
-#define SLDG_WALK_U1 8
-#endif
-#ifndef SLDG_WALK_U2
-#define SLDG_WALK_U2 4
-#endif
-#ifndef SLDG_WALK_U3
-#define SLDG_WALK_U3 4
-#endif
-#ifndef SLDG_WALK_U4
-#define SLDG_WALK_U4 4
-#endif
 // cells loaded ahead of the one being computed (loads in flight per thread = U * K1 * VEC values)
 template <int K1> struct Unroll {
 #ifdef SLDG_REAL_FLOAT
     static constexpr int U = (K1 == 3) ? 8 : 4;            // measured: cfg2 (k=2) prefers 8 cells in flight, cfg4 (k=1) 4
 #else
-    static constexpr int U = (K1 == 1) ? SLDG_WALK_U1 : (K1 == 2) ? SLDG_WALK_U2 : (K1 == 3) ? SLDG_WALK_U3 : (K1 == 4) ? SLDG_WALK_U4 : 2;
+    static constexpr int U = (K1 == 1) ? 8 : (K1 <= 4) ? 4 : 2;             // measured on B200 (cfg2-5)
 #endif
 };
 

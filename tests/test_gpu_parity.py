@@ -361,8 +361,12 @@ def test_graph_replay_of_the_step_is_bitwise_the_plain_step(P, cfg):
         n0 = g.launch_count()
         for i, h in enumerate(seq):
             g.step(fg, h)
+            # the replay path is really taken (the binding hands over torch's default stream, on which a capture cannot
+            # start: the library then records on a stream of its own), and never with graph = 0
+            assert g.graph_active() == (graph != 0), (graph, i)
             if i == 1:
                 g.advect_x(fg, 0.3 * dt)            # rewrites the cached x tables: the graph must not survive
+                assert not g.graph_active()
         outs.append((fg.cpu().numpy(), g.launch_count() - n0))
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][0], outs[2][0])
     assert outs[0][1] == outs[1][1] == outs[2][1]                 # replays count the launches they contain
@@ -372,6 +376,25 @@ def test_graph_replay_of_the_step_is_bitwise_the_plain_step(P, cfg):
         if i == 1:
             fo = o.advect_x(fo, 0.3 * dt)
     assert rel_inf(outs[0][0], fo) <= TOL_STEPS
+
+
+def test_contexts_of_different_degree_live_side_by_side(P):
+    """The A/B polynomial coefficients of the device-side v-table kernel are per context: a k=1 context keeps working
+    after a k=2 (and a k=3) context was created on the same device (they used to share one __constant__ copy)."""
+    dom = [0.0, 4 * np.pi, 0.0, 4 * np.pi, -6.0, 6.0, -6.0, 6.0]
+    cells = [4, 4, 6, 6]
+    ctxs = {}
+    for k in (1, 2, 3, 1):                               # the second k=1 context is created last
+        ctxs.setdefault(k, []).append((P.Sldg(2, 2, cells, k, dom), O.Oracle(2, 2, cells, k, dom)))
+    for k in (1, 2, 3):
+        for g, o in ctxs[k]:
+            rng = np.random.default_rng(W.SEED + k)
+            f0 = rng.random(tuple(reversed(o.D)))
+            E = rng.uniform(-3.0, 3.0, size=(2,) + tuple(reversed(o.D[:2])))
+            fg = torch.from_numpy(f0).to(g.device).contiguous()
+            g.advect_v(fg, torch.from_numpy(E).to(g.device).contiguous(), 0.37)
+            want = o.advect_v(f0, E, 0.37)
+            assert rel_inf(fg.cpu().numpy(), want) <= 1e-12, k
 
 
 # --------------------------------------------------------------- fused x1+x2+x3 pass (dim_x = 3, degree <= 1)
