@@ -96,8 +96,8 @@ int sldg_advect_x(sldg_ctx* ctx, double* f, double dt);
 /* a5+a6, steps 3a-3c: for d = 1..dim_x, f(x, v_d + E_d(x) dt), i.e. the same update
  * along v_d with delta = ((-E_d(x)) * dt) / h_{v_d} per x node (sign from eq. (1), reading H).
  * Velocity axes beyond dim_x are not advected (reading D).  E is [dim_x][X].  Result in f.
- * E is the same for all sweeps, so the v_1 and v_2 sweeps may run as one pass over f (same
- * arithmetic in the same order: bit-identical to separate sweeps; option fuse_v). */
+ * E is the same for all sweeps, so the v_1 and v_2 sweeps (option fuse_v), or for dim_x = 3 all three
+ * (option fuse_v3), may run as one pass over f: same arithmetic in the same order, bit-identical to separate sweeps. */
 int sldg_advect_v(sldg_ctx* ctx, double* f, const double* E, double dt);
 
 /* a3: rho[x] = sum_v (prod_d h_{v_d} w_{j_d}) f[x,v]. */
@@ -187,11 +187,12 @@ int sldg_advect_axis(sldg_ctx* ctx, double* f, int axis, const double* delta_hos
  * Kinds: 0 = sweep along axis 0 (TMA/SMEM kernel), 1 = sweep along a slow axis, 2 = rho,
  * 3 = Poisson/E, 4 = shift tables, 5 = copies, 6 = fused x pass (x_1+x_2, or x_1+x_2+x_3 for dim_x = 3, in one
  * launch), 7 = fused v_1+v_2 pass (one launch), 8 = double x half step (x_1+x_2 applied twice in one launch, inside
- * sldg_steps); the per-axis figures of sldg_timing_axis book an equal share of a
+ * sldg_steps), 9 = fused v_1+v_2+v_3 pass (one launch, dim_x = 3), 10 = double x half step for dim_x = 3
+ * (x_1+x_2+x_3 applied twice in one launch, inside sldg_steps); the per-axis figures of sldg_timing_axis book an equal share of a
  * fused launch's time on each of its axes.  sldg_timing_read synchronises, adds the elapsed
  * times of all events recorded since the last read, and returns per kind the number of launches
  * and the total milliseconds (arrays of SLDG_NKINDS entries, host). */
-#define SLDG_NKINDS 9
+#define SLDG_NKINDS 11
 int sldg_timing_enable(sldg_ctx* ctx, int on);
 int sldg_timing_read(sldg_ctx* ctx, long long* launches, double* ms);
 /* total kernel launches enqueued by this context since creation */
@@ -203,11 +204,11 @@ int sldg_timing_axis(const sldg_ctx* ctx, long long* launches, double* ms);
 /* Host-only (no CUDA device needed): the plan of one sldg_step (nsteps == 0) or of sldg_steps(nsteps) for a problem
  * of this shape, obtained by running the library's planning code with every launch replaced by a counter.
  * shifts_below_one: 1 = every x shift is 0 or -1 cell (|v| dt/2 < h_x: slow-axis x sweeps may then run in place),
- * fuse_v / x_double: the options of the same names (sldg_set_option).  counts (host, 6 entries) = passes over f of
+ * fuse_v / fuse_v3 / x_double: the options of the same names (sldg_set_option).  counts (host, 6 entries) = passes over f of
  * the x sweeps, passes of the v sweeps, rho passes, field solves, whole-array device copies, kernel launches counted
  * by sldg_launch_count.  A fused or merged launch is ONE pass.  Returns 0 or a negative code. */
 int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
-                    int shifts_below_one, int fuse_v, int x_double, long long* counts);
+                    int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts);
 
 /* Tuning knob (affects speed only, never results): see DESIGN.md section 5. */
 int sldg_set_option(sldg_ctx* ctx, const char* name, long long value);

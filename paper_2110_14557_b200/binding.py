@@ -9,9 +9,9 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = "libsldg_b200.so"
 
-NKINDS = 9
+NKINDS = 11
 MAX_DIM = 6
-KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x", "sweep_fused_v", "sweep_fused_x_double"]
+KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x", "sweep_fused_v", "sweep_fused_x_double", "sweep_fused_v3", "sweep_fused_x3_double"]
 
 _vp, _dp, _ip, _ll = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_longlong
 _llp = C.POINTER(C.c_longlong)
@@ -57,7 +57,7 @@ EXPORTS = {
     "sldg_cg_info": (C.c_int, [_vp, _ip, _dp]),
     "sldg_last_phi": (_vp, [_vp]),
     "sldg_sipg_matrices": (C.c_int, [C.c_int, C.c_double, _dp, _dp]),
-    "sldg_plan_query": (C.c_int, [C.c_int, C.c_int, _ip, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+    "sldg_plan_query": (C.c_int, [C.c_int, C.c_int, _ip, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                   C.POINTER(C.c_longlong)]),
 }
 
@@ -120,13 +120,13 @@ def sipg_matrices(degree, sigma=0.0):
     return M, B
 
 
-def plan_query(dim_x, dim_v, cells, degree, nsteps, precision="f64", shifts_below_one=True, fuse_v=1, x_double=1):
+def plan_query(dim_x, dim_v, cells, degree, nsteps, precision="f64", shifts_below_one=True, fuse_v=1, x_double=1, fuse_v3=1):
     """sldg_plan_query (host-only call): passes over f that sldg_step (nsteps == 0) / sldg_steps(nsteps) would launch.
     -> dict(x_passes, v_passes, rho_passes, field_solves, copies, launches)"""
     cells_c = (C.c_int * len(cells))(*[int(c) for c in cells])
     out = (C.c_longlong * 6)()
     _check(lib().sldg_plan_query(int(dim_x), int(dim_v), cells_c, int(degree), 1 if precision == "f32" else 0, int(nsteps),
-                                 1 if shifts_below_one else 0, int(fuse_v), int(x_double), out))
+                                 1 if shifts_below_one else 0, int(fuse_v), int(fuse_v3), int(x_double), out))
     return dict(zip(("x_passes", "v_passes", "rho_passes", "field_solves", "copies", "launches"), [int(v) for v in out]))
 
 

@@ -36,7 +36,7 @@ void sldg_ev_end(sldg_ctx* c)
 }
 
 // ------------------------------------------------------------------ layout of the workspace
-struct WsLayout { size_t f2, vS, vAB, vS2, vAB2, Wv, rho, E, part, cplx[6], red, phi, cg_info, total; long long part_cap; };
+struct WsLayout { size_t f2, vS, vAB, vS2, vAB2, vS3, vAB3, Wv, rho, E, part, cplx[6], red, phi, cg_info, total; long long part_cap; };
 
 static WsLayout ws_layout(const sldg_ctx* c)
 {
@@ -49,6 +49,8 @@ static WsLayout ws_layout(const sldg_ctx* c)
     L.vAB = take(X * NN2 * 8);
     L.vS2 = take(X * 4);
     L.vAB2 = take(X * NN2 * 8);
+    L.vS3 = take(c->dx == 3 ? X * 4 : 0);
+    L.vAB3 = take(c->dx == 3 ? X * NN2 * 8 : 0);
     L.Wv = take((size_t)c->V * 8);
     L.rho = take(X * 8);
     L.E = take(X * 8 * c->dx);
@@ -132,6 +134,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     c->opt_poisson_small = 1; c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
+    c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
@@ -251,6 +254,7 @@ extern "C" int sldg_set_workspace(sldg_ctx* c, void* dev, size_t bytes)
     c->ws = b; c->ws_bytes = bytes;
     c->f2 = (double*)(b + L.f2); c->vS = (int*)(b + L.vS); c->vAB = (double*)(b + L.vAB);
     c->vS2 = (int*)(b + L.vS2); c->vAB2 = (double*)(b + L.vAB2);
+    c->vS3 = (int*)(b + L.vS3); c->vAB3 = (double*)(b + L.vAB3);
     c->Wv = (double*)(b + L.Wv); c->rho = (double*)(b + L.rho); c->E = (double*)(b + L.E);
     c->part = (double*)(b + L.part); c->part_cap = L.part_cap;
     for (int i = 0; i < 6; i++) c->cplx[i] = (double*)(b + L.cplx[i]);
@@ -605,14 +609,57 @@ static bool fusedv_possible(const sldg_ctx* c)
     const long long walks = ((c->X + wx - 1) / wx) * (c->V / (c->D[c->dx] * c->D[c->dx + 1]));
     return walks >= 2LL * c->sm_count;
 }
-// buffer flips of one v advection
-static int v_flips(const sldg_ctx* c, bool fuse) { return fuse ? c->dx - 1 : c->dx; }
-static int v_flips(const sldg_ctx* c) { return v_flips(c, fusedv_possible(c)); }
+// the fused v_1+v_2+v_3 pass (sldg_sweep_fusedv3.cu): dim_x = dim_v = 3, degree <= 1
+static bool fusedv3_possible(const sldg_ctx* c)
+{
+    if (!c->opt_fuse_v3 || c->dx != 3) return false;
+    if (!(c->prec == SLDG_F32 ? sldg_fusedv3_shape_f32(c) : sldg_fusedv3_shape_f64(c))) return false;
+    if (c->opt_fuse_v3 == 2) return true;
+    // auto: a block walks all of v_3 serially; the pass pays only when its walks (x tiles times v_2 strips) fill the GPU
+    const long long walks = ((c->X + 15) / 16) * ((c->cells[4] + 3) / 4);
+    return walks >= 2LL * c->sm_count;
+}
 
-// v-sweeps on (*cur, *oth): v_1 and v_2 in one fused out-of-place pass when the shape allows, every other sweep a
-// slow-axis walk; each pass flips the pair.
-// fuse: 1 = the fused pass when the shape allows, 0 = separate walks (a plan may veto the fused pass: step_best)
-static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt, bool fuse = true)
+// How a v advection runs: every sweep a walk (VM_WALKS), v_1+v_2 in one pass and v_3 a walk (VM_FUSED2), or all of
+// v_1..v_3 in one pass (VM_FUSED3).  Buffer flips and cost in tenths of a walk pass (measured on B200: the fused
+// v_1+v_2 pass 1.3, the fused v_1+v_2+v_3 pass 1.5 walk passes).
+enum { VM_WALKS = 0, VM_FUSED2 = 1, VM_FUSED3 = 2 };
+static bool v_mode_possible(const sldg_ctx* c, int mode)
+{
+    return mode == VM_WALKS || (mode == VM_FUSED2 && fusedv_possible(c)) || (mode == VM_FUSED3 && fusedv3_possible(c));
+}
+static int v_flips(const sldg_ctx* c, int mode) { return mode == VM_FUSED3 ? 1 : mode == VM_FUSED2 ? c->dx - 1 : c->dx; }
+static int v_cost(const sldg_ctx* c, int mode) { return mode == VM_FUSED3 ? 15 : mode == VM_FUSED2 ? 13 + 10 * (c->dx - 2) : 10 * c->dx; }
+static bool v_mode_forced(const sldg_ctx* c, int mode)       // tests: option value 2 takes the pass whenever the shape allows
+{
+    return (mode == VM_FUSED3 && c->opt_fuse_v3 == 2) || (mode == VM_FUSED2 && c->opt_fuse_v == 2 && !(c->opt_fuse_v3 == 2 && fusedv3_possible(c)));
+}
+// the cheapest mode of a v advection inside a run of steps (any buffer parity)
+static int v_mode_best(const sldg_ctx* c)
+{
+    int best = VM_WALKS, cost = 1 << 30;
+    for (int m = VM_WALKS; m <= VM_FUSED3; m++) {
+        if (!v_mode_possible(c, m)) continue;
+        if (v_mode_forced(c, m)) return m;
+        if (v_cost(c, m) < cost) { cost = v_cost(c, m); best = m; }
+    }
+    return best;
+}
+// the cheapest mode of a v advection on its own whose result must end in the buffer it started in (a copy = 10)
+static int v_mode_standalone(const sldg_ctx* c)
+{
+    int best = VM_WALKS, cost = 1 << 30;
+    for (int m = VM_WALKS; m <= VM_FUSED3; m++) {
+        if (!v_mode_possible(c, m)) continue;
+        if (v_mode_forced(c, m)) return m;
+        const int k = v_cost(c, m) + ((v_flips(c, m) & 1) ? 10 : 0);
+        if (k < cost) { cost = k; best = m; }
+    }
+    return best;
+}
+
+// v-sweeps on (*cur, *oth) in the given mode; every pass is out of place and flips the pair.
+static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt, int mode)
 {
     int axes[3];
     ShiftTable tabs[3];
@@ -621,25 +668,39 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         tabs[i].S = c->vS; tabs[i].AB = c->vAB; tabs[i].strideIdx = 1; tabs[i].strideM = c->X;
     }
     VPrep p = {E, dt};
-    if (fuse && fusedv_possible(c)) {
+    if (!v_mode_possible(c, mode)) mode = VM_WALKS;
+    if (mode == VM_FUSED3) {
+        int r;
+        if ((r = vtable_into(c, &p, 0, c->vS, c->vAB))) return r;
+        if ((r = vtable_into(c, &p, 1, c->vS2, c->vAB2))) return r;
+        if ((r = vtable_into(c, &p, 2, c->vS3, c->vAB3))) return r;
+        ShiftTable t2 = tabs[1], t3 = tabs[2];
+        t2.S = c->vS2; t2.AB = c->vAB2; t3.S = c->vS3; t3.AB = c->vAB3;
+        if (!c->dry) {
+            sldg_ev_begin(c, KIND_FUSEDV3, c->dx);
+            cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv3_f32(c, *cur, *oth, tabs[0], t2, t3)
+                                                : sldg_launch_sweep_fusedv3_f64(c, *cur, *oth, tabs[0], t2, t3);
+            sldg_ev_end(c);
+            if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+        } else c->dry_v++;
+        c->launches++;
+        double* t = *cur; *cur = *oth; *oth = t;
+        return SLDG_OK;
+    }
+    if (mode == VM_FUSED2) {
         int r;
         if ((r = vtable_into(c, &p, 0, c->vS, c->vAB))) return r;
         if ((r = vtable_into(c, &p, 1, c->vS2, c->vAB2))) return r;
         ShiftTable t2 = tabs[1];
         t2.S = c->vS2; t2.AB = c->vAB2;
-        if (c->dry) {
-            c->dry_v++; c->launches++;
-            double* t = *cur; *cur = *oth; *oth = t;
-            if (c->dx == 2) return SLDG_OK;
-            VPrepOff o = {p, 2};
-            return run_sweeps(c, cur, oth, axes + 2, tabs + 2, c->dx - 2, false, vprep_off, &o);
-        }
-        sldg_ev_begin(c, KIND_FUSEDV, c->dx);                  // axis field: first of the two fused axes
-        cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
-                                            : sldg_launch_sweep_fusedv_f64(c, *cur, *oth, tabs[0], t2);
-        sldg_ev_end(c);
+        if (!c->dry) {
+            sldg_ev_begin(c, KIND_FUSEDV, c->dx);                  // axis field: first of the two fused axes
+            cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
+                                                : sldg_launch_sweep_fusedv_f64(c, *cur, *oth, tabs[0], t2);
+            sldg_ev_end(c);
+            if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
+        } else c->dry_v++;
         c->launches++;
-        if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
         double* t = *cur; *cur = *oth; *oth = t;
         if (c->dx == 2) return SLDG_OK;
         VPrepOff o = {p, 2};
@@ -654,8 +715,8 @@ extern "C" int sldg_advect_v(sldg_ctx* c, double* f, const double* E, double dt)
     if (r) return r;
     if (!E) return SLDG_EINVAL;
     double *cur = f, *oth = c->f2;
-    if ((r = advect_v_impl(c, &cur, &oth, E, dt))) return r;
-    // an odd number of v-sweeps (dim_x = 1 or 3) leaves the result in the workspace: one device copy.
+    if ((r = advect_v_impl(c, &cur, &oth, E, dt, v_mode_standalone(c)))) return r;
+    // an odd number of v passes (dim_x = 1 or 3) leaves the result in the workspace: one device copy.
     // sldg_step avoids it by fixing the parity in its second x half step.
     if (cur != f) return copy_back(c, f, cur);
     return SLDG_OK;
@@ -773,31 +834,36 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
     return SLDG_OK;
 }
 
-// passes over f of one Strang step whose total number of buffer flips has parity `flip_total`; *p1 = flip parity of
-// the first x half step that achieves it
-static int step_cost(const sldg_ctx* c, bool flip_total, int* p1, bool fuse_v)
+// passes over f of the two x half steps of one Strang step whose total number of buffer flips has parity `flip_total`,
+// given the flips of its v advection; *p1 = flip parity of the first x half step that achieves it
+static int step_cost(const sldg_ctx* c, bool flip_total, int* p1, int vflips)
 {
     int best = 1 << 30;
     for (int q1 = 0; q1 < 2; q1++) {
-        const int q2 = (q1 + v_flips(c, fuse_v) + (flip_total ? 1 : 0)) & 1;
+        const int q2 = (q1 + vflips + (flip_total ? 1 : 0)) & 1;
         XPlan a = x_plan(c, q1 != 0), b = x_plan(c, q2 != 0);
         if (a.ok && b.ok && a.passes + b.passes < best) { best = a.passes + b.passes; if (p1) *p1 = q1; }
     }
     return best;
 }
-// The cheapest plan of one Strang step in tenths of a pass over f: x passes as above, v_1+v_2 as two walks (20) or as
-// the fused pass (13: measured 1.3 walk passes).  For dim_x = 2 a single step that must end in its own buffer is
-// cheaper WITHOUT the fused v pass (its odd flip would cost a two-pass in-place x half step: 43 against 40).
-static int step_best(const sldg_ctx* c, bool flip_total, int* p1, bool* fuse_v)
+// The cheapest plan of one Strang step in tenths of a pass over f: x passes as above plus the v advection in one of its
+// modes (v_cost).  For dim_x = 2 a single step that must end in its own buffer is cheaper WITHOUT the fused v pass (its
+// odd flip would cost a two-pass in-place x half step: 43 against 40); for dim_x = 3 such a step takes the fused
+// v_1+v_2 pass + the v_3 walk (two flips: both x half steps stay one-pass), while steps that may end in the other buffer
+// (sldg_steps) take the one-pass v advection.
+static int step_best(const sldg_ctx* c, bool flip_total, int* p1, int* vmode)
 {
-    int p_off = 0, p_on = 0;
-    const int off = 10 * step_cost(c, flip_total, &p_off, false) + 10 * c->dx;
-    int on = 1 << 30;
-    if (fusedv_possible(c)) on = 10 * step_cost(c, flip_total, &p_on, true) + 13 + 10 * (c->dx - 2);
-    const bool use = on < off || (c->opt_fuse_v == 2 && on < (1 << 30));       // forced: tests
-    if (p1) *p1 = use ? p_on : p_off;
-    if (fuse_v) *fuse_v = use;
-    return use ? on : off;
+    int best = 1 << 30, bm = VM_WALKS, bp = 0;
+    for (int m = VM_WALKS; m <= VM_FUSED3; m++) {
+        if (!v_mode_possible(c, m)) continue;
+        int q = 0;
+        const int k = 10 * step_cost(c, flip_total, &q, v_flips(c, m)) + v_cost(c, m);
+        if (v_mode_forced(c, m)) { best = k; bm = m; bp = q; break; }
+        if (k < best) { best = k; bm = m; bp = q; }
+    }
+    if (p1) *p1 = bp;
+    if (vmode) *vmode = bm;
+    return best;
 }
 
 // One Strang step on the pair (*cur, *oth).  The dx v-sweeps flip the pair dx times; the two x half steps choose
@@ -810,12 +876,12 @@ static int step_core(sldg_ctx* c, double** cur, double** oth, double dt, bool fl
     ShiftTable tabs[3];
     if ((r = build_x_tables(c, dt / 2.0, tabs))) return r;
     int p1 = 0;
-    bool fuse_v = false;
-    step_best(c, flip_total, &p1, &fuse_v);
+    int vmode = VM_WALKS;
+    step_best(c, flip_total, &p1, &vmode);
     if ((r = advect_x_impl(c, cur, oth, dt / 2.0, p1 != 0))) return r;
     if ((r = sldg_density(c, *cur, c->rho))) return r;
     if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
-    if ((r = advect_v_impl(c, cur, oth, c->E, dt, fuse_v))) return r;
+    if ((r = advect_v_impl(c, cur, oth, c->E, dt, vmode))) return r;
     const bool want_other = flip_total;                       // where the step has to end, relative to `start`
     const bool now_other = (*cur != start);
     return advect_x_impl(c, cur, oth, dt / 2.0, now_other != want_other);
@@ -913,19 +979,28 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
     double *cur = f, *oth = c->f2;
     // n - 1 merged passes save n - 1 passes over f; restoring the buffer parity at the end costs one of them back when
     // the number of flips is odd (2 steps with an even number of v flips: nothing gained, the plain plan runs)
-    if (x_double_possible(c) && (nsteps >= 3 || (nsteps == 2 && (v_flips(c) & 1)))) {
+    const int vm = v_mode_best(c);
+    if (x_double_possible(c) && (nsteps >= 3 || (nsteps == 2 && (v_flips(c, vm) & 1)))) {
         // x(dt/2) | rho, E, v(dt) | x(dt/2) x(dt/2) as one pass | rho, E, v(dt) | ... | x(dt/2): the same sweeps in the
         // same order as nsteps single steps.  The last half step restores the buffer parity.
         if ((r = advect_x_impl(c, &cur, &oth, dt / 2.0, true))) return r;
         // The closing half step is one pass only if it may flip the buffers, i.e. if the flips before it are odd in
-        // number: 1 + nsteps * v_flips + (nsteps - 1).  With the fused v pass (one flip) that count is even: the LAST v
-        // advection then runs as two walks (one flip and 0.7 pass more) and the closing half step saves a whole pass.
-        const bool fused_v = fusedv_possible(c);
-        const bool last_v_walks = fused_v && ((1 + nsteps * v_flips(c, true) + (nsteps - 1)) % 2 == 0);
+        // number: 1 + nsteps * v_flips + (nsteps - 1).  With a one-flip v pass that count is even: the LAST v advection
+        // then runs in the cheapest mode of the other flip parity (dim_x = 2: two walks, 0.7 pass more; dim_x = 3: the
+        // fused v_1+v_2 pass + the v_3 walk, 0.8 pass more) when that costs less than the x pass it saves.
+        int vm_last = vm;
+        if ((1 + nsteps * v_flips(c, vm) + (nsteps - 1)) % 2 == 0) {
+            const int gain = 10 * (x_plan(c, false).passes - x_plan(c, true).passes);
+            int extra = gain;
+            for (int m = VM_WALKS; m <= VM_FUSED3; m++)
+                if (v_mode_possible(c, m) && ((v_flips(c, m) ^ v_flips(c, vm)) & 1) && v_cost(c, m) - v_cost(c, vm) < extra) {
+                    extra = v_cost(c, m) - v_cost(c, vm); vm_last = m;
+                }
+        }
         for (int s = 0; s < nsteps; s++) {
             if ((r = sldg_density(c, cur, c->rho))) return r;
             if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
-            if ((r = advect_v_impl(c, &cur, &oth, c->E, dt, !(last_v_walks && s == nsteps - 1)))) return r;
+            if ((r = advect_v_impl(c, &cur, &oth, c->E, dt, s == nsteps - 1 ? vm_last : vm))) return r;
             if (s < nsteps - 1) r = advect_x_double(c, &cur, &oth, dt / 2.0);
             else r = advect_x_impl(c, &cur, &oth, dt / 2.0, cur != f);
             if (r) return r;
@@ -947,9 +1022,9 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
 // count what it would launch.  The same functions plan and launch (c->dry only replaces the launches), so the counts
 // are those of the real calls.
 extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
-                               int shifts_below_one, int fuse_v, int x_double, long long* counts)
+                               int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts)
 {
-    if (!counts || nsteps < 0 || fuse_v < 0 || fuse_v > 2 || x_double < 0 || x_double > 1) return SLDG_EINVAL;
+    if (!counts || nsteps < 0 || fuse_v < 0 || fuse_v > 2 || fuse_v3 < 0 || fuse_v3 > 2 || x_double < 0 || x_double > 1) return SLDG_EINVAL;
     if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
     if (dim_x < 1 || dim_x > 3) return SLDG_EINVAL;
     double dom[2 * SLDG_MAX_DIM];
@@ -957,7 +1032,7 @@ extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degre
     sldg_ctx* c = nullptr;
     int r = create_impl(&c, dim_x, dim_v, cells, degree, dom, precision, true);
     if (r) return r;
-    c->dry = true; c->dry_safe = shifts_below_one; c->opt_graph = 0; c->opt_fuse_v = fuse_v; c->opt_x_double = x_double;
+    c->dry = true; c->dry_safe = shifts_below_one; c->opt_graph = 0; c->opt_fuse_v = fuse_v; c->opt_fuse_v3 = fuse_v3; c->opt_x_double = x_double;
     c->ws_ready = true;
     // distinct, aligned, never dereferenced: the planner only compares and swaps them
     double* f = reinterpret_cast<double*>((uintptr_t)0x10000);
@@ -1130,6 +1205,8 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
             if ((r.kind == KIND_SWEEP0 || r.kind == KIND_SWEEP) && r.axis >= 0) { c->a_launch[r.axis]++; c->a_ms[r.axis] += t; }
             if (r.kind == KIND_FUSED) { const int nf = r.axis == 3 ? 3 : 2; for (int a = 0; a < nf; a++) { c->a_launch[a]++; c->a_ms[a] += t / nf; } }
             if (r.kind == KIND_FUSEDX2) { for (int a = 0; a < 2; a++) { c->a_launch[a] += 2; c->a_ms[a] += t / 2; } }   // four sweeps
+            if (r.kind == KIND_FUSEDV3) { for (int a = r.axis; a < r.axis + 3; a++) { c->a_launch[a]++; c->a_ms[a] += t / 3; } }
+            if (r.kind == KIND_FUSEDX3D) { for (int a = 0; a < 3; a++) { c->a_launch[a] += 2; c->a_ms[a] += t / 3; } }    // six sweeps
             if (r.kind == KIND_FUSEDV) { for (int a = r.axis; a < r.axis + 2; a++) { c->a_launch[a]++; c->a_ms[a] += t / 2; } }
         }
         c->ev_free.push_back(r);
@@ -1170,6 +1247,10 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "poisson_small")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_poisson_small = (int)value; return SLDG_OK; }
     if (!strcmp(name, "x_double")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_double = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fuse_v3")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v3 = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv3_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv3_wx = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv3_strip")) { if (value < 0 || value > 5) return SLDG_EINVAL; c->opt_fv3_strip = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv3_slots")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv3_slots = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv_wx = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_stages")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_inflight")) { if (value < 1024 || value > 220 * 1024) return SLDG_EINVAL; c->opt_fv_inflight = (int)value; return SLDG_OK; }

@@ -18,7 +18,7 @@
 #define SLDG_COPY_BIT (1 << 30)
 #define SLDG_S_MASK (SLDG_COPY_BIT - 1)
 
-enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5, KIND_FUSED = 6, KIND_FUSEDV = 7, KIND_FUSEDX2 = 8 };
+enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5, KIND_FUSED = 6, KIND_FUSEDV = 7, KIND_FUSEDX2 = 8, KIND_FUSEDV3 = 9, KIND_FUSEDX3D = 10 };
 
 // Polynomial coefficients of A_jl(alpha), B_jl(alpha) in powers of (alpha - 1/2), ascending, row-major
 // [2][K1*K1][SLDG_MAXPOLY]; the fp64 copy is uploaded per context (dPoly) for the device-side table kernel.
@@ -103,6 +103,7 @@ struct sldg_ctx {
     double* f2;                     // second f buffer
     int* vS; double* vAB;           // v-sweep tables [X], [2 K1^2][X]
     int* vS2; double* vAB2;         // second v-sweep table (the fused v_1+v_2 pass needs both at once)
+    int* vS3; double* vAB3;         // third one (fused v_1+v_2+v_3 pass, dim_x = 3)
     double* Wv;                     // [V]
     double* rho; double* E;         // [X], [dx][X]
     double* part; long long part_cap;   // rho partial sums
@@ -157,6 +158,10 @@ struct sldg_ctx {
     int opt_fv_ppb;                 // fused v kernel: planes per block (0 = auto)
     int opt_fv_cps;                 // fused v kernel, degree <= 1: v_2 cells per tensor copy
     int opt_fv_l2;                  // fused v kernel: L2 promotion of the tensor map (0 none, 1 64 B, 2 128 B, 3 256 B)
+    int opt_fuse_v3;                // v_1, v_2 and v_3 sweeps in one pass (sldg_sweep_fusedv3.cu; dim_x = 3, degree <= 1): 0 never, 1 auto, 2 whenever the shape allows
+    int opt_fv3_wx;                 // fused v_1v_2v_3 kernel: x nodes per tile (0 = auto)
+    int opt_fv3_strip;              // fused v_1v_2v_3 kernel: v_2 donor pairs per strip (0 = auto: 4)
+    int opt_fv3_slots;              // fused v_1v_2v_3 kernel: ring slots (0 = as many as shared memory holds)
     int opt_poisson_small;          // 1: x grids of up to 1024 nodes are solved by one single-block launch (FFT route)
     int opt_rho_vec;                // 0 = auto (2 when aligned), 1
     int opt_rho_blocks;             // rho kernel: 128-thread blocks per SM to aim for
@@ -187,6 +192,10 @@ bool sldg_fusedv_shape_f64(const sldg_ctx* c, int* wx_out, int* threads_out);
 bool sldg_fusedv_shape_f32(const sldg_ctx* c, int* wx_out, int* threads_out);
 cudaError_t sldg_launch_sweep_fusedv_f64(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2);
 cudaError_t sldg_launch_sweep_fusedv_f32(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2);
+bool sldg_fusedv3_shape_f64(const sldg_ctx* c);
+bool sldg_fusedv3_shape_f32(const sldg_ctx* c);
+cudaError_t sldg_launch_sweep_fusedv3_f64(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2, const ShiftTable& t3);
+cudaError_t sldg_launch_sweep_fusedv3_f32(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2, const ShiftTable& t3);
 SLDG_DECL_SWEEPS(_f64)
 SLDG_DECL_SWEEPS(_f32)
 cudaError_t sldg_launch_sweep_walk(sldg_ctx* c, const double* fin, double* fout, const SweepGeom& g,

@@ -23,13 +23,12 @@
 // Arithmetic per value is identical (same operands, same order) to sweep_walk_kernel on v_1 then on v_2, so the
 // fused and the unfused plans agree bit for bit.  Out of place only; degree <= 3; D_1 <= 256 (one TMA box);
 // X * sizeof(real) a multiple of 16.
-#include <cuda.h>
-
 #include <type_traits>
 
 #include "sldg_async.h"
 #include "sldg_internal.h"
 #include "sldg_real.h"
+#include "sldg_tmap.h"
 
 namespace {
 
@@ -42,17 +41,6 @@ struct FVParams {
     uint32_t stage_bytes;         // ring slot stride (>= D_1 * WX * sizeof(real), multiple of 128)
     ShiftTable t1, t2;
 };
-
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-        ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
 
 template <int K1> struct FVTraits {
     static constexpr bool KEEP = (K1 <= 2);        // first v_2 block kept in registers (else streamed in again)
@@ -293,27 +281,6 @@ __global__ void __launch_bounds__(FVTraits<K1>::MAXT)
     else body(std::false_type{});
 }
 
-typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiled encode_fn()
-{
-    static EncodeTiled fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult qr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
-            qr == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiled>(p);
-        else
-            cudaGetLastError();
-    }
-    return fn;
-}
-
 template <int K1>
 cudaError_t launch(sldg_ctx* c, const CUtensorMap& tm, const FVParams& P, int threads, size_t smem)
 {
@@ -338,7 +305,7 @@ bool SLDG_SFX(sldg_fusedv_shape)(const sldg_ctx* c, int* wx_out, int* threads_ou
     if (D1 > 256 || c->cells[c->dx] < 1) return false;
     if ((c->X * (long long)sizeof(real)) & 15) return false;
     // 32-bit tensor coordinates, and the driver's tensor-map encoder must be reachable (no libcuda link)
-    if (c->X >= (1LL << 31) || c->V / D1 >= (1LL << 31) || (!c->dry && !encode_fn())) return false;
+    if (c->X >= (1LL << 31) || c->V / D1 >= (1LL << 31) || (!c->dry && !sldg_encode_tiled())) return false;
     const int cap = (K1 <= 2) ? FVTraits<1>::MAXT : (K1 == 3) ? FVTraits<3>::MAXT : FVTraits<4>::MAXT;  // threads allowed
     // x nodes per tile: rows of 128 B when the thread budget allows, else 64 B; never below 32 B
     int wx = c->opt_fv_wx > 0 ? c->opt_fv_wx : (int)(128 / sizeof(real));
@@ -365,7 +332,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     int wx = 0, threads = 0;
     if (fin == fout || !SLDG_SFX(sldg_fusedv_shape)(c, &wx, &threads)) return cudaErrorNotSupported;
     if ((((uintptr_t)fin) | ((uintptr_t)fout)) & 15) return cudaErrorNotSupported;
-    EncodeTiled enc = encode_fn();
+    SldgEncodeTiled enc = sldg_encode_tiled();
     if (!enc) return cudaErrorNotSupported;
     const int K1 = c->K1, a1 = c->dx, a2 = c->dx + 1;
     const long long D1 = c->D[a1], D2 = c->D[a2];
@@ -409,10 +376,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv)(sldg_ctx* c, const void* fin, voi
     const cuuint32_t box[3] = {(cuuint32_t)wx, (cuuint32_t)D1, (cuuint32_t)rps};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUtensorMapDataType dt = sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    const CUtensorMapL2promotion l2 = c->opt_fv_l2 == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
-                                    : c->opt_fv_l2 == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
-                                    : c->opt_fv_l2 == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
-                                                        : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
+    const CUtensorMapL2promotion l2 = sldg_l2_promotion(c->opt_fv_l2);
     if (enc(&tm, dt, 3, const_cast<void*>(fin), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, l2, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorNotSupported;

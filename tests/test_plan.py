@@ -29,11 +29,11 @@ def test_single_step_budget(name):
     assert (r["x_passes"], r["v_passes"], r["rho_passes"], r["field_solves"], r["copies"]) == (2, 2, 1, 1, 0)
 
 
-@pytest.mark.parametrize("name,x,v", [("cfg2", 11, 11), ("cfg3", 11, 11), ("cfg4", 20, 20), ("cfg5", 20, 20)])
+@pytest.mark.parametrize("name,x,v", [("cfg2", 11, 11), ("cfg3", 11, 11), ("cfg4", 20, 10), ("cfg5", 20, 10)])
 def test_ten_steps_budget(name, x, v):
     """sldg_steps(10).  dim_x = 2: first half step 1 pass, 9 merged double half steps, 9 fused v passes and the last v
     advection as two walks (so that the flips before the closing half step are odd and it is ONE pass).  dim_x = 3: 2 x
-    passes and 2 v passes per step."""
+    passes and ONE v pass (v_1+v_2+v_3 fused) per step."""
     r = q(CFG[name], 10)
     assert (r["x_passes"], r["v_passes"], r["rho_passes"], r["field_solves"], r["copies"]) == (x, v, 10, 10, 0)
 
@@ -43,10 +43,14 @@ def test_options_change_the_budget_as_documented():
     assert q(c2, 10, x_double=0)["x_passes"] == 20 and q(c2, 10, x_double=0)["v_passes"] == 10     # alternating buffers
     r = q(c2, 10, x_double=0, fuse_v=0)
     assert (r["x_passes"], r["v_passes"]) == (20, 20)
-    r = q(c4, 10, fuse_v=0)                      # three v walks: odd flips, sldg_steps alternates buffers
+    r = q(c4, 10, fuse_v=0, fuse_v3=0)           # three v walks: odd flips, sldg_steps alternates buffers
     assert (r["x_passes"], r["v_passes"]) == (20, 30)
-    r = q(c4, 0, fuse_v=0)                       # a single step: one x half step needs two passes
+    r = q(c4, 10, fuse_v3=0)                     # fused v_1+v_2 + the v_3 walk
+    assert (r["x_passes"], r["v_passes"]) == (20, 20)
+    r = q(c4, 0, fuse_v=0, fuse_v3=0)            # a single step: one x half step needs two passes
     assert (r["x_passes"], r["v_passes"]) == (3, 3)
+    r = q(c4, 0, fuse_v=0)                       # a single step with the one-pass v advection only: the odd flip costs an x pass
+    assert (r["x_passes"], r["v_passes"]) == (3, 1)
     r = q(c2, 0, fuse_v=2)                       # forced fused v in a single dim_x = 2 step: the odd flip costs an x pass
     assert (r["x_passes"], r["v_passes"]) == (3, 1)
     r = q(c2, 10, precision="f32")               # single precision: no automatic fused v for dim_x = 2
@@ -70,11 +74,11 @@ def test_degree_three_fuses_v_but_not_the_x_half_steps():
 def test_every_plan_ends_in_the_callers_buffer_without_a_copy(dx, dv, k):
     cells = [6, 5, 4, 6, 5, 4][:dx + dv]
     big = [64, 48, 40, 24, 20, 16][:dx + dv]
-    for cc, n, safe, fv, xd, prec in itertools.product((cells, big), (0, 1, 2, 3, 4, 7), (True, False), (0, 1, 2), (0, 1),
-                                                       ("f64", "f32")):
-        r = P.plan_query(dx, dv, cc, k, n, precision=prec, shifts_below_one=safe, fuse_v=fv, x_double=xd)
+    for cc, n, safe, fv, xd, prec, fv3 in itertools.product((cells, big), (0, 1, 2, 3, 4, 7), (True, False), (0, 1, 2), (0, 1),
+                                                            ("f64", "f32"), (0, 1, 2) if dx == 3 else (1,)):
+        r = P.plan_query(dx, dv, cc, k, n, precision=prec, shifts_below_one=safe, fuse_v=fv, x_double=xd, fuse_v3=fv3)
         steps = max(1, n)
-        assert r["copies"] == 0, (cc, n, safe, fv, xd, prec, r)
+        assert r["copies"] == 0, (cc, n, safe, fv, xd, prec, fv3, r)
         assert r["rho_passes"] == steps and r["field_solves"] == steps
         # never more passes than one per 1-D sweep, never fewer than the merged minimum
         assert r["x_passes"] <= 2 * dx * steps and r["v_passes"] <= dx * steps
