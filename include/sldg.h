@@ -143,7 +143,7 @@ int sldg_sipg_matrices(int degree, double sigma, double* hostM, double* hostB);
  * sweeps in the same order).  What changes is the number of passes over f: consecutive steps may keep their
  * intermediate result in the workspace buffer, and for dim_x = 2 the second x half step of a step and the
  * first x half step of the next one (same time increment, nothing in between) run as ONE pass
- * (option x_double).  f at the intermediate integer times is then not written out: call sldg_step when a
+ * (option x_double; for dim_x = 3 only when forced with x_double = 2: that pass is slower than two on B200).  f at the intermediate integer times is then not written out: call sldg_step when a
  * per-step diagnostic needs it.  sldg_plan_query reports the pass budget of either call. */
 int sldg_steps(sldg_ctx* ctx, double* f, double dt, int nsteps);
 
@@ -209,6 +209,15 @@ int sldg_timing_axis(const sldg_ctx* ctx, long long* launches, double* ms);
  * by sldg_launch_count.  A fused or merged launch is ONE pass.  Returns 0 or a negative code. */
 int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
                     int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts);
+
+/* Diagnostic (no part of the hot path): the rate at which the SMs can pull the strided row tiles the fused v passes
+ * gather -- pieces [rows][wx] of a row-major [R][X] fp64 device array `src` -- with no arithmetic and no stores.
+ * mode 0: 2-d TMA tensor copies into a ring of `depth` shared-memory slots; mode 1: 1-d TMA bulk copies, one per
+ * row piece; mode 2: plain 128-bit global loads by all threads (depth 2 or 4 boxes in flight per thread).
+ * `threads` per block (multiple of 32, <= 256), every block handles `chunks_per_block` consecutive boxes of one x tile.
+ * Runs one untimed and `reps` timed launches; *ms_out (host) = elapsed ms of the timed ones.  Synchronises. */
+int sldg_probe_load_rate(sldg_ctx* ctx, const double* src, long long X, long long R, int mode, int wx, int rows,
+                         int depth, int threads, int chunks_per_block, int reps, double* ms_out);
 
 /* Tuning knob (affects speed only, never results): see DESIGN.md section 5. */
 int sldg_set_option(sldg_ctx* ctx, const char* name, long long value);

@@ -51,6 +51,7 @@ EXPORTS = {
     "sldg_launch_count": (_ll, [_vp]),
     "sldg_timing_axis": (C.c_int, [_vp, _llp, _dp]),
     "sldg_set_option": (C.c_int, [_vp, C.c_char_p, _ll]),
+    "sldg_probe_load_rate": (C.c_int, [_vp, _vp, _ll, _ll, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _dp]),
     "sldg_poisson_cg": (C.c_int, [_vp, _vp, _vp, C.c_double, C.c_int]),
     "sldg_set_poisson_solver": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, C.c_double]),
     "sldg_cg_reset": (C.c_int, [_vp]),
@@ -311,6 +312,14 @@ class Sldg:
 
     def launch_count(self):
         return int(lib().sldg_launch_count(self._h))
+
+    def probe_load_rate(self, src, X, R, mode, wx, rows, depth, threads, chunks_per_block, reps=3):
+        """sldg_probe_load_rate -> GB/s of the timed launches (bytes = the boxes' bytes)"""
+        ms = C.c_double()
+        _check(lib().sldg_probe_load_rate(self._h, _ptr(src), int(X), int(R), int(mode), int(wx), int(rows), int(depth),
+                                          int(threads), int(chunks_per_block), int(reps), C.byref(ms)), self._h)
+        nbytes = (X // wx) * wx * (R // rows) * rows * 8
+        return reps * nbytes / (ms.value * 1e-3) / 1e9
 
     def set_option(self, name, value):
         _check(lib().sldg_set_option(self._h, name.encode(), int(value)))

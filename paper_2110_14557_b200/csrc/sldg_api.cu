@@ -132,7 +132,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
-    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
+    c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_f3d_threads = 128; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     c->opt_poisson_small = 1; c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
     c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
@@ -813,6 +813,13 @@ extern "C" int sldg_sipg_matrices(int degree, double sigma, double* hostM, doubl
 // one) as ONE pass of the fused cell kernel applying the sweep pair twice (sldg_sweep_fused_cell.cu, DBL).
 static bool x_double_possible(const sldg_ctx* c)
 {
+    // dim_x = 3 (sldg_sweep_fused3d.cu): built, bit-identical, and measured SLOWER than two one-pass half steps on B200 (the
+    // pass is bound by fp64 issue, not by HBM: cfg4 22.1 against 2 x 11.9 ms at the best tiling, cfg5 43.8 against 2 x 17.5
+    // ms), so it is planned only when forced (option x_double = 2)
+    if (c->dx == 3) {
+        if (c->opt_x_double != 2 || !c->opt_fuse_x || !c->opt_fuse3) return false;
+        return c->prec == SLDG_F32 ? sldg_fused3d_shape_f32(c) : sldg_fused3d_shape_f64(c);
+    }
     if (!c->opt_x_double || !c->opt_fuse_x || c->dx != 2 || c->K1 > 3 || c->opt_fused_impl == 2) return false;
     if (c->cells[0] > 128 || ((c->K1 * c->D[0] * (long long)c->esize) & 15)) return false;
     return (size_t)(2 + 1) * c->K1 * c->D[0] * c->esize + (size_t)2 * 2 * c->K1 * c->D[0] * c->esize + 64 <= 227 * 1024;
@@ -823,6 +830,18 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
     int r = build_x_tables(c, tau, tabs);
     if (r) return r;
     if (c->dry) { c->dry_x++; c->launches++; double* t = *cur; *cur = *oth; *oth = t; return SLDG_OK; }
+    if (c->dx == 3) {
+        SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
+        const int anycp3 = (c->tab_anycp[0] || c->tab_anycp[1] || c->tab_anycp[2]) ? 1 : 0;
+        sldg_ev_begin(c, KIND_FUSEDX3D, 0);
+        cudaError_t e3 = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3d_f32(c, *cur, *oth, g3, tabs, anycp3)
+                                             : sldg_launch_sweep_fused3d_f64(c, *cur, *oth, g3, tabs, anycp3);
+        sldg_ev_end(c);
+        c->launches++;
+        if (e3 != cudaSuccess) { c->last_cuda = (int)e3; return SLDG_ECUDA; }
+        double* t3 = *cur; *cur = *oth; *oth = t3;
+        return SLDG_OK;
+    }
     const int anycp = (c->tab_anycp[0] || c->tab_anycp[1]) ? 1 : 0;
     sldg_ev_begin(c, KIND_FUSEDX2, 0);
     cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], anycp)
@@ -1024,7 +1043,7 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
 extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
                                int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts)
 {
-    if (!counts || nsteps < 0 || fuse_v < 0 || fuse_v > 2 || fuse_v3 < 0 || fuse_v3 > 2 || x_double < 0 || x_double > 1) return SLDG_EINVAL;
+    if (!counts || nsteps < 0 || fuse_v < 0 || fuse_v > 2 || fuse_v3 < 0 || fuse_v3 > 2 || x_double < 0 || x_double > 2) return SLDG_EINVAL;
     if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
     if (dim_x < 1 || dim_x > 3) return SLDG_EINVAL;
     double dom[2 * SLDG_MAX_DIM];
@@ -1237,6 +1256,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "fused_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_fused_threads = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse3")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fuse3 = (int)value; return SLDG_OK; }
     if (!strcmp(name, "f3_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_f3_threads = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "f3d_threads")) { if (value < 1 || value > 256) return SLDG_EINVAL; c->opt_f3d_threads = (int)value; return SLDG_OK; }
     if (!strcmp(name, "f3_stages")) { if (value < 2 || value > 4) return SLDG_EINVAL; c->opt_f3_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "x_copy")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_copy = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fused_impl")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fused_impl = (int)value; return SLDG_OK; }
@@ -1245,7 +1265,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "cell_bytes")) { if (value < 256 || value > 96 * 1024) return SLDG_EINVAL; c->opt_cell_bytes = (int)value; return SLDG_OK; }
     if (!strcmp(name, "cell_stages")) { if (value < 2 || value > 6) return SLDG_EINVAL; c->opt_cell_stages = (int)value; return SLDG_OK; }
     if (!strcmp(name, "poisson_small")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_poisson_small = (int)value; return SLDG_OK; }
-    if (!strcmp(name, "x_double")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_x_double = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "x_double")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_x_double = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v3")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v3 = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv3_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv3_wx = (int)value; return SLDG_OK; }

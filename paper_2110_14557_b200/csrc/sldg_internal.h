@@ -145,12 +145,13 @@ struct sldg_ctx {
     int opt_fuse3;                  // 1: x_1, x_2 and x_3 sweeps in one pass (dim_x = 3, degree <= 1)
     int opt_f3_threads;             // fused3 kernel: threads per block (<= 256) = N_0 * strip cells
     int opt_f3_stages;              // fused3 kernel: input stages (2..4)
+    int opt_f3d_threads;            // double x_1x_2x_3 pass: compute threads per block (<= 256) = N_0 * (strip cells + 1)
     int opt_x_copy;                 // 1: sldg_advect_x runs the plan that ends in the workspace, then copies back (tests)
     int opt_cell_threads;           // fused cell kernel: threads per block (<= 128) = planes per block * N_0
     int opt_cell_rows;              // fused cell kernel: x_2 cells per chunk (0 = from opt_cell_bytes)
     int opt_cell_bytes;             // fused cell kernel: target bytes of one input stage (all planes of the block)
     int opt_cell_stages;            // fused cell kernel: input stages (2..6)
-    int opt_x_double;               // 1: sldg_steps merges the x half steps of consecutive Strang steps into one pass (dim_x = 2, degree <= 2)
+    int opt_x_double;               // 1: sldg_steps merges the x half steps of consecutive Strang steps into one pass (dim_x = 2: degree <= 2; dim_x = 3: degree <= 1)
     int opt_fuse_v;                 // v_1 and v_2 sweeps in one pass (sldg_sweep_fusedv.cu): 0 never, 1 when the shape allows and the walks fill the GPU, 2 whenever the shape allows
     int opt_fv_wx;                  // fused v kernel: x nodes per tile (0 = auto: 128-byte rows if the threads allow)
     int opt_fv_stages;              // fused v kernel: ring depth (0 = from opt_fv_inflight)
@@ -192,6 +193,10 @@ bool sldg_fusedv_shape_f64(const sldg_ctx* c, int* wx_out, int* threads_out);
 bool sldg_fusedv_shape_f32(const sldg_ctx* c, int* wx_out, int* threads_out);
 cudaError_t sldg_launch_sweep_fusedv_f64(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2);
 cudaError_t sldg_launch_sweep_fusedv_f32(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2);
+bool sldg_fused3d_shape_f64(const sldg_ctx* c);
+bool sldg_fused3d_shape_f32(const sldg_ctx* c);
+cudaError_t sldg_launch_sweep_fused3d_f64(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
+cudaError_t sldg_launch_sweep_fused3d_f32(sldg_ctx* c, const void* fin, void* fout, const SweepGeom* g, const ShiftTable* t, int any_copy);
 bool sldg_fusedv3_shape_f64(const sldg_ctx* c);
 bool sldg_fusedv3_shape_f32(const sldg_ctx* c);
 cudaError_t sldg_launch_sweep_fusedv3_f64(sldg_ctx* c, const void* fin, void* fout, const ShiftTable& t1, const ShiftTable& t2, const ShiftTable& t3);

@@ -60,13 +60,14 @@ __device__ __forceinline__ void fv3_table(const ShiftTable& t, long long idx, re
     }
 }
 
-template <int K1, int S>
+// WXT: x nodes per tile as a compile-time constant (shared-memory offsets become immediates), 0 = P.WX at run time
+template <int K1, int S, int WXT>
 __global__ void __launch_bounds__(FV3_MAXT)
     sweep_fusedv3_kernel(const __grid_constant__ CUtensorMap tmap, const FV3Params P)
 {
     constexpr int NN = K1 * K1, N3V = K1 * K1 * K1;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    const int ST = P.slots, WX = P.WX, N1 = P.N1, N2 = P.N2, N3 = P.N3;
+    const int ST = P.slots, WX = WXT ? WXT : P.WX, N1 = P.N1, N2 = P.N2, N3 = P.N3;
     const int D1 = N1 * K1, D2 = N2 * K1;
     const uint32_t ring_s = smem_u32(smem_raw);
     const uint32_t full_s = ring_s + (uint32_t)ST * P.slot_bytes;       // ST full barriers, then ST empty barriers
@@ -170,12 +171,19 @@ __global__ void __launch_bounds__(FV3_MAXT)
             if (t == 0) produce();
             mbar_wait(fbar, ph);
             real a[NN][K1], b[NN][K1];
+            const real* pa = pa0 + soff;
+            const real* pb = pb0 + soff;
 #pragma unroll
-            for (int r = 0; r < NN; r++)
+            for (int r = 0; r < NN; r++) {
 #pragma unroll
-                for (int m = 0; m < K1; m++) { a[r][m] = pa0[soff + r * rowvals + m * WX]; b[r][m] = pb0[soff + r * rowvals + m * WX]; }
-            // the slot is read: hand it back.  It is refilled by the ASYNC proxy (TMA) once every warp has arrived, so the
-            // generic-proxy reads above are ordered before that write by a proxy fence (see sldg_sweep_fusedv.cu)
+                for (int m = 0; m < K1; m++) { a[r][m] = pa[m * WX]; b[r][m] = pb[m * WX]; }
+                pa += rowvals; pb += rowvals;
+            }
+            // The slot is read: hand it back.  It is refilled by the ASYNC proxy (TMA) once every warp has arrived, so the
+            // generic-proxy reads above are ordered before that write by a proxy fence.  (Tried instead: an arrive placed
+            // after the arithmetic that consumes the loads, with the results as unused operands of the asm statement.  The
+            // dependency exists only in the compiler's IR, not in the PTX that ptxas schedules: the drift test failed, 256
+            // wrong values, and the time did not change: 13.9 against 13.7 ms on cfg4.)
             fence_async_smem();
             __syncwarp();
             if (warp_lead) mbar_arrive(fbar + 8u * (uint32_t)ST);
@@ -281,10 +289,10 @@ __global__ void __launch_bounds__(FV3_MAXT)
     else body(std::false_type{});
 }
 
-template <int K1, int S>
+template <int K1, int S, int WXT>
 cudaError_t launch(sldg_ctx* c, const CUtensorMap& tm, const FV3Params& P, int threads, size_t smem)
 {
-    auto kern = sweep_fusedv3_kernel<K1, S>;
+    auto kern = sweep_fusedv3_kernel<K1, S, WXT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long grid = (long long)P.ntiles * P.nstrips;
@@ -297,11 +305,11 @@ template <int K1>
 cudaError_t dispatch(sldg_ctx* c, const CUtensorMap& tm, const FV3Params& P, int threads, size_t smem)
 {
     switch (P.S) {
-    case 1: return launch<K1, 1>(c, tm, P, threads, smem);
-    case 2: return launch<K1, 2>(c, tm, P, threads, smem);
-    case 3: return launch<K1, 3>(c, tm, P, threads, smem);
-    case 4: return launch<K1, 4>(c, tm, P, threads, smem);
-    case 5: return launch<K1, 5>(c, tm, P, threads, smem);
+    case 1: return P.WX == 16 ? launch<K1, 1, 16>(c, tm, P, threads, smem) : launch<K1, 1, 0>(c, tm, P, threads, smem);
+    case 2: return P.WX == 16 ? launch<K1, 2, 16>(c, tm, P, threads, smem) : launch<K1, 2, 0>(c, tm, P, threads, smem);
+    case 3: return P.WX == 16 ? launch<K1, 3, 16>(c, tm, P, threads, smem) : launch<K1, 3, 0>(c, tm, P, threads, smem);
+    case 4: return P.WX == 16 ? launch<K1, 4, 16>(c, tm, P, threads, smem) : launch<K1, 4, 0>(c, tm, P, threads, smem);
+    case 5: return P.WX == 16 ? launch<K1, 5, 16>(c, tm, P, threads, smem) : launch<K1, 5, 0>(c, tm, P, threads, smem);
     }
     return cudaErrorNotSupported;
 }

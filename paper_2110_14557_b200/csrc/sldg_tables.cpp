@@ -151,23 +151,17 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
     int n = k + 1;
     long D = (long)ncell * n;
     // P[mm][l] = l_l(eta_mm), eta_mm = (mm + 1/2)/(k+1)  (equidistant points of one cell)
-    ld P[SLDG_MAXK1][SLDG_MAXK1], Pi[SLDG_MAXK1][2 * SLDG_MAXK1];
+    // and its inverse in closed form: the map back from the equidistant points to the GL nodes evaluates the
+    // interpolation polynomial through the equidistant values, Pinv[l][mm] = (Lagrange basis of eta_mm)(xi_l)
+    ld P[SLDG_MAXK1][SLDG_MAXK1], Pinv[SLDG_MAXK1][SLDG_MAXK1];
     for (int mm = 0; mm < n; mm++)
-        for (int l = 0; l < n; l++) P[mm][l] = lagrange_at(n, xi, l, ((ld)mm + 0.5L) / (ld)n);
-    for (int i = 0; i < n; i++)
-        for (int j = 0; j < n; j++) { Pi[i][j] = P[i][j]; Pi[i][n + j] = (i == j) ? 1.0L : 0.0L; }
-    for (int col = 0; col < n; col++) {
-        int piv = col;
-        for (int r = col + 1; r < n; r++) if (fabsl(Pi[r][col]) > fabsl(Pi[piv][col])) piv = r;
-        for (int j = 0; j < 2 * n; j++) { ld t = Pi[col][j]; Pi[col][j] = Pi[piv][j]; Pi[piv][j] = t; }
-        ld dd = Pi[col][col];
-        for (int j = 0; j < 2 * n; j++) Pi[col][j] /= dd;
-        for (int r = 0; r < n; r++) {
-            if (r == col) continue;
-            ld fct = Pi[r][col];
-            for (int j = 0; j < 2 * n; j++) Pi[r][j] -= fct * Pi[col][j];
+        for (int l = 0; l < n; l++) {
+            P[mm][l] = lagrange_at(n, xi, l, ((ld)mm + 0.5L) / (ld)n);
+            ld r = 1;                                         // exact rational nodes: (mm + 1/2)/n
+            for (int m2 = 0; m2 < n; m2++)
+                if (m2 != mm) r *= ((ld)xi[l] - ((ld)m2 + 0.5L) / (ld)n) / ((ld)(mm - m2) / (ld)n);
+            Pinv[l][mm] = r;
         }
-    }
     std::vector<ld> cs(D), sn(D);
     for (long r = 0; r < D; r++) {
         cs[r] = cosl(twopi * (ld)r / (ld)D);
@@ -182,7 +176,7 @@ void sldg_build_dft(int k, const double* xi, int ncell, double* fwdT, double* in
                 for (int mm = 0; mm < n; mm++) {
                     long r = (m * (i * n + mm)) % D;
                     gr += cs[r] * P[mm][l];  gi += -sn[r] * P[mm][l];          // e^{-2 pi i m e / D}
-                    hr += cs[r] * Pi[l][n + mm]; hi += sn[r] * Pi[l][n + mm];  // e^{+2 pi i m e / D}
+                    hr += cs[r] * Pinv[l][mm]; hi += sn[r] * Pinv[l][mm];  // e^{+2 pi i m e / D}
                 }
                 long node = i * n + l;
                 // forward G[m][node] stored transposed at [node][m]

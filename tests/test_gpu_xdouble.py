@@ -81,6 +81,74 @@ def test_steps_with_double_x_pass_are_bitwise_the_plain_plan(P, geom, dt, prec):
         assert rel_inf(outs[0][0], want) <= 1e-10
 
 
+# dim_x = 3: the double x_1x_2x_3 pass (sldg_sweep_fused3d.cu)
+X3D_GEOMS = [
+    ([4, 5, 3, 2, 2, 2], 1),          # 5 x_2 cells: strips of 1..5 cells, ragged last strip
+    ([20, 7, 3, 2, 2, 2], 1),         # D_0 = 40 as in BASELINE cfg4; 7 x_2 cells
+    ([6, 5, 1, 2, 3, 2], 1),          # a single x_3 cell: the wrap cells are the only donor pairs
+    ([6, 5, 2, 2, 3, 2], 1),          # two x_3 cells
+    ([4, 1, 3, 2, 2, 3], 1),          # a single x_2 cell: every halo cell is the cell itself
+    ([4, 2, 3, 2, 2, 3], 1),          # two x_2 cells: the input range wraps around the axis
+    ([8, 6, 4, 2, 3, 2], 0),          # degree 0 (D_0 = 8: bulk-copy rule holds)
+    ([5, 4, 3, 2, 2, 2], 0),          # degree 0, D_0 = 5: rows not a multiple of 16 B -> plain plan
+    ([3, 2, 2, 3, 2, 2], 2),          # degree 2: no fused x_1x_2x_3 passes at all -> plain plan
+]
+
+
+@pytest.mark.parametrize("geom", X3D_GEOMS, ids=lambda g: f"{'x'.join(map(str, g[0]))}-k{g[1]}")
+@pytest.mark.parametrize("dt", [0.03, 0.9])                     # |x shift| < 1 cell / up to ~10 cells (wraps)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_steps_with_double_x3_pass_are_bitwise_the_plain_plan(P, geom, dt, prec):
+    cells, k = geom
+    dom = dom_of(3, 3)
+    o = O.Oracle(3, 3, cells, k, dom, threads=O.lib().orc_max_threads())
+    f0 = W.random_field(o.shape, seed=43 + k)
+    if prec == "f32":
+        f0 = f0.to(torch.float32)
+    outs = []
+    # (x_double, fuse_v3, f3d_threads, f3_stages, nsteps)
+    # x_double = 2: the dim_x = 3 double pass is planned only when forced (measured slower than two passes on B200)
+    for xd, fv3, thr, st, n in ((0, 0, 128, 3, 4), (2, 0, 128, 3, 4), (2, 2, 2 * cells[0], 2, 4), (2, 2, 3 * cells[0], 4, 4),
+                                (2, 0, 256, 3, 4), (2, 2, 128, 3, 3), (1, 2, 128, 3, 3)):
+        g = P.Sldg(3, 3, cells, k, dom, precision=prec)
+        g.set_option("graph", 0); g.set_option("x_double", xd); g.set_option("fuse_v3", fv3)
+        g.set_option("f3d_threads", min(256, thr)); g.set_option("f3_stages", st)
+        fg = f0.to(g.device).contiguous()
+        n0 = g.launch_count()
+        g.steps(fg, dt, n)
+        outs.append((fg.cpu().numpy(), g.launch_count() - n0, n))
+    for x, _, n in outs[1:5]:
+        assert np.array_equal(outs[0][0], x)
+    assert np.array_equal(outs[5][0], outs[6][0])                   # three steps, one-pass v advection on both sides
+    doubled = k <= 1 and (cells[0] * (k + 1) * (k + 1) * (8 if prec == "f64" else 4)) % 16 == 0
+    if doubled:
+        assert outs[1][1] < outs[0][1] and outs[5][1] < outs[6][1]  # the merged passes really ran
+    else:
+        assert outs[1][1] == outs[0][1]
+    if prec == "f64":
+        want = f0.numpy()
+        for _ in range(4):
+            want, _, _ = o.step(want, dt)
+        assert rel_inf(outs[0][0], want) <= 1e-10
+
+
+@pytest.mark.parametrize("n", [2, 3, 5])
+def test_steps_equal_repeated_single_steps_with_the_double_x3_pass(P, n):
+    cfg = W.scaled(W.CONFIGS[3], [6, 5, 4, 6, 4, 4])
+    o = O.Oracle(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], threads=1)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    g.set_option("graph", 0); g.set_option("fuse_v3", 2); g.set_option("x_double", 2)
+    fa, fb = f0.to(g.device).contiguous(), f0.to(g.device).contiguous()
+    for _ in range(n):
+        g.step(fa, cfg["dt"])
+    g.timing_enable(True); g.timing_read()
+    g.steps(fb, cfg["dt"], n)
+    kinds, _ = g.timing_read()
+    assert torch.equal(fa, fb)
+    assert kinds["sweep_fused_x3_double"][0] == n - 1
+
+
 @pytest.mark.parametrize("n", [2, 3, 5])
 def test_steps_equal_repeated_single_steps_with_the_double_pass(P, n):
     cfg = W.scaled(W.CONFIGS[1], [12, 10, 8, 8])
@@ -98,7 +166,7 @@ def test_steps_equal_repeated_single_steps_with_the_double_pass(P, n):
 @pytest.mark.parametrize("geom", [(2, 2, [12, 10, 8, 8], 2), (2, 3, [8, 8, 6, 6, 4], 1), (3, 3, [6, 4, 4, 6, 4, 4], 1)],
                          ids=lambda g: f"{g[0]}x{g[1]}v-k{g[3]}")
 @pytest.mark.parametrize("n", [0, 2, 5])
-@pytest.mark.parametrize("fuse_v,x_double", [(0, 0), (2, 0), (2, 1), (0, 1)])
+@pytest.mark.parametrize("fuse_v,x_double", [(0, 0), (2, 0), (2, 1), (0, 1), (2, 2)])
 def test_plan_query_counts_are_those_of_the_real_calls(P, geom, n, fuse_v, x_double):
     """The host-only sldg_plan_query (tests/test_plan.py checks its budgets on the CPU) must report exactly the sweep
     launches the real sldg_step / sldg_steps make: per-kind launch counts from the library's event instrumentation."""
