@@ -21,7 +21,13 @@
  * alias each other.  The library never allocates O(|f|) memory itself.
  *
  * STREAM / SYNC.  All device work is enqueued on the stream given to sldg_set_stream (default:
- * the legacy default stream).  No call synchronises, except those marked "synchronises".
+ * the legacy default stream).  No call synchronises, except those marked "synchronises".  One conditional case:
+ * the x-sweep shift tables are built on the host per time increment and cached (two increments per axis, least
+ * recently used evicted: a Strang run with its dt/2 plus one more increment never rebuilds).  A call that needs
+ * a table that is not cached -- sldg_advect_x, sldg_step, sldg_steps, sldg_step_host with a new dt -- rebuilds
+ * it, which SYNCHRONISES the stream once (the pinned staging buffer is reused) and therefore must not happen
+ * inside a caller's stream capture; sldg_advect_axis (test hook) always uploads its table and synchronises.
+ * Non-finite dt or shift-table entries are rejected with SLDG_EINVAL before anything is enqueued.
  *
  * ERRORS.  Every int-returning call returns SLDG_OK (0) or a negative code; nothing throws,
  * aborts or prints.  A context is not thread-safe.  There is NO CPU fallback: without a CUDA
@@ -194,6 +200,7 @@ int sldg_advect_axis(sldg_ctx* ctx, double* f, int axis, const double* delta_hos
  * and the total milliseconds (arrays of SLDG_NKINDS entries, host). */
 #define SLDG_NKINDS 11
 int sldg_timing_enable(sldg_ctx* ctx, int on);
+/* SLDG_ECUDA (and no figures) if an event could not be created since the last read: launches went unrecorded. */
 int sldg_timing_read(sldg_ctx* ctx, long long* launches, double* ms);
 /* total kernel launches enqueued by this context since creation */
 long long sldg_launch_count(const sldg_ctx* ctx);
@@ -219,7 +226,9 @@ int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int prec
 int sldg_probe_load_rate(sldg_ctx* ctx, const double* src, long long X, long long R, int mode, int wx, int rows,
                          int depth, int threads, int chunks_per_block, int reps, double* ms_out);
 
-/* Tuning knob (affects speed only, never results): see DESIGN.md section 5. */
+/* Tuning knob (affects speed only, never results): see DESIGN.md section 5.  A fused pass whose launcher declines
+ * a shape that the planner accepted is replaced by the separate sweeps (plus one device copy when the buffer
+ * parity differs): same bits, never an error. */
 int sldg_set_option(sldg_ctx* ctx, const char* name, long long value);
 
 #ifdef __cplusplus

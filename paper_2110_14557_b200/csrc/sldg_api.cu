@@ -23,15 +23,23 @@ void sldg_ev_begin(sldg_ctx* c, int kind, int axis)
     EventRec r;
     if (!c->ev_free.empty()) { r = c->ev_free.back(); c->ev_free.pop_back(); }
     else {
-        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+        if (cudaEventCreate(&r.a) != cudaSuccess) { c->ev_failed = true; c->last_cuda = (int)cudaGetLastError(); return; }
+        if (cudaEventCreate(&r.b) != cudaSuccess) { cudaEventDestroy(r.a); c->ev_failed = true; c->last_cuda = (int)cudaGetLastError(); return; }
     }
     r.kind = kind; r.axis = axis;
     cudaEventRecord(r.a, c->stream);
     c->ev.push_back(r);
 }
+// a launcher declined (cudaErrorNotSupported): forget the event opened for it
+static void ev_cancel(sldg_ctx* c)
+{
+    if (!c->timing || c->ev.empty() || c->ev_failed) return;
+    c->ev_free.push_back(c->ev.back());
+    c->ev.pop_back();
+}
 void sldg_ev_end(sldg_ctx* c)
 {
-    if (!c->timing || c->ev.empty()) return;
+    if (!c->timing || c->ev.empty() || c->ev_failed) return;
     cudaEventRecord(c->ev.back().b, c->stream);
 }
 
@@ -56,7 +64,7 @@ static WsLayout ws_layout(const sldg_ctx* c)
     L.E = take(X * 8 * c->dx);
     // rho partial sums: enough chunks to fill the GPU (see sldg_launch_density), at least 1
     long long xtiles = (c->X + 255) / 256;
-    long long nchunk = ((long long)148 * 64 + xtiles - 1) / xtiles;
+    long long nchunk = ((long long)c->sm_count * 64 + xtiles - 1) / xtiles;
     if (nchunk > c->V / 16) nchunk = c->V / 16;
     if (nchunk < 1) nchunk = 1;
     nchunk += 1;
@@ -134,8 +142,10 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_f3d_threads = 128; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     c->opt_poisson_small = 1; c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
-    c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0;
-    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->dS[a] = nullptr; c->dAB[a] = nullptr; c->tab_valid[a] = false; c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
+    c->opt_decline = 0; c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0;
+    for (int a = 0; a < SLDG_MAX_DIM; a++) { c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
+    for (int a = 0; a < 3; a++) for (int i = 0; i < SLDG_XTAB_SLOTS; i++) { XTab& x = c->xtab[a][i]; x.dS = nullptr; x.dAB = nullptr; x.tau = 0.0; x.valid = x.anycp = x.safe = false; x.used = 0; }
+    c->xtab_clock = 0; c->ev_failed = false;
     for (int a = 0; a < 3; a++) { c->dFwdT[a] = c->dInvT[a] = c->dKap[a] = nullptr; }
     c->dS_hook = nullptr; c->dAB_hook = nullptr; c->hook_cap = 0;
     c->dPoly = nullptr; c->dScalar = nullptr; c->dCounter = nullptr; c->hS = nullptr; c->hAB = nullptr; c->hcap = 0;
@@ -161,8 +171,10 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     if (e == cudaSuccess) e = cudaMemset(c->dCounter, 0, 16);
     for (int a = 0; a < dim_x && e == cudaSuccess; a++) {
         long long Ds = c->D[dim_x + a];
-        e = cudaMalloc((void**)&c->dS[a], (size_t)Ds * 4);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&c->dAB[a], (size_t)Ds * NN2 * 8);
+        for (int i = 0; i < SLDG_XTAB_SLOTS && e == cudaSuccess; i++) {
+            e = cudaMalloc((void**)&c->xtab[a][i].dS, (size_t)Ds * 4);
+            if (e == cudaSuccess) e = cudaMalloc((void**)&c->xtab[a][i].dAB, (size_t)Ds * NN2 * 8);
+        }
     }
     if (e == cudaSuccess) { e = cudaMalloc((void**)&c->dS_hook, (size_t)maxD * 4); }
     if (e == cudaSuccess) { e = cudaMalloc((void**)&c->dAB_hook, (size_t)maxD * NN2 * 8); c->hook_cap = maxD; }
@@ -211,11 +223,13 @@ extern "C" int sldg_destroy(sldg_ctx* c)
     sldg_graph_drop(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     for (int a = 0; a < SLDG_MAX_DIM; a++) {
-        if (c->dS[a]) cudaFree(c->dS[a]);
-        if (c->dAB[a]) cudaFree(c->dAB[a]);
         if (c->dWx[a]) cudaFree(c->dWx[a]);
     }
     for (int a = 0; a < 3; a++) {
+        for (int i = 0; i < SLDG_XTAB_SLOTS; i++) {
+            if (c->xtab[a][i].dS) cudaFree(c->xtab[a][i].dS);
+            if (c->xtab[a][i].dAB) cudaFree(c->xtab[a][i].dAB);
+        }
         if (c->dFwdT[a]) cudaFree(c->dFwdT[a]);
         if (c->dInvT[a]) cudaFree(c->dInvT[a]);
         if (c->dKap[a]) cudaFree(c->dKap[a]);
@@ -312,7 +326,10 @@ static int upload_table(sldg_ctx* c, const double* delta, long long n, int N, in
 {
     const size_t NN2 = 2 * (size_t)c->K1 * c->K1;
     if (n > c->hcap) return SLDG_EINVAL;
-    // the pinned staging buffers may still be in flight from a previous upload on this stream
+    for (long long i = 0; i < n; i++)
+        if (!isfinite(delta[i])) return SLDG_EINVAL;       // a NaN / Inf shift has no floor(): nothing is enqueued
+    // the pinned staging buffers may still be in flight from a previous upload on this stream: SYNCHRONISES
+    // (include/sldg.h marks the calls that can get here)
     CK(cudaStreamSynchronize(c->stream));
     for (long long i = 0; i < n; i++) host_entry(c, delta[i], N, c->hS + i, c->hAB + (size_t)i * NN2);
     if (c->prec == SLDG_F32) {          // A, B were evaluated in long double; the sweep takes them rounded to fp32
@@ -422,9 +439,16 @@ static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
         for (int a = 0; a < c->dx; a++) { c->tab_safe[a] = c->dry_safe != 0; c->tab_anycp[a] = false; tabs[a] = ShiftTable(); }
         return SLDG_OK;
     }
+    if (!isfinite(dt)) return SLDG_EINVAL;
     for (int a = 0; a < c->dx; a++) {
         const int b = c->dx + a;
-        if (!c->tab_valid[a] || c->tab_tau[a] != dt) {
+        XTab* x = nullptr;
+        for (int i = 0; i < SLDG_XTAB_SLOTS; i++)
+            if (c->xtab[a][i].valid && c->xtab[a][i].tau == dt) x = &c->xtab[a][i];
+        if (!x) {
+            x = &c->xtab[a][0];                             // a free slot, else the least recently used one
+            for (int i = 1; i < SLDG_XTAB_SLOTS; i++)
+                if (x->valid && (!c->xtab[a][i].valid || c->xtab[a][i].used < x->used)) x = &c->xtab[a][i];
             std::vector<double> delta((size_t)c->D[b]);
             for (long long n = 0; n < c->D[b]; n++) {
                 // node coordinate lo + (i + xi_j) h, then delta = (v * dt) / h_x   (reading O3)
@@ -435,7 +459,8 @@ static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
                 delta[(size_t)n] = vt / c->h[a];
             }
             sldg_graph_drop(c);                 // a captured step reads these device tables
-            int r = upload_table(c, delta.data(), c->D[b], c->cells[a], c->dS[a], c->dAB[a]);
+            x->valid = false;
+            int r = upload_table(c, delta.data(), c->D[b], c->cells[a], x->dS, x->dAB);
             if (r) return r;
             bool safe = true, anycp = false;
             for (long long n = 0; n < c->D[b]; n++) {
@@ -443,10 +468,11 @@ static int build_x_tables(sldg_ctx* c, double dt, ShiftTable* tabs)
                 const int sv = c->hS[n] & SLDG_S_MASK;
                 if (sv != 0 && sv != c->cells[a] - 1) safe = false;
             }
-            c->tab_safe[a] = safe; c->tab_anycp[a] = anycp;
-            c->tab_valid[a] = true; c->tab_tau[a] = dt;
+            x->safe = safe; x->anycp = anycp; x->valid = true; x->tau = dt;
         }
-        tabs[a].S = c->dS[a]; tabs[a].AB = c->dAB[a]; tabs[a].strideIdx = NN2; tabs[a].strideM = 1;
+        x->used = ++c->xtab_clock;
+        c->tab_safe[a] = x->safe; c->tab_anycp[a] = x->anycp;
+        tabs[a].S = x->dS; tabs[a].AB = x->dAB; tabs[a].strideIdx = NN2; tabs[a].strideM = 1;
     }
     return SLDG_OK;
 }
@@ -532,8 +558,17 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
         SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
         sldg_ev_begin(c, KIND_FUSED, 3);                       // axis field of a fused event = number of fused axes
         const int anycp = (c->tab_anycp[0] || c->tab_anycp[1] || c->tab_anycp[2]) ? 1 : 0;
-        cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3_f32(c, *cur, *oth, g3, tabs, anycp)
+        cudaError_t e = (c->opt_decline & 4) ? cudaErrorNotSupported
+                      : c->prec == SLDG_F32 ? sldg_launch_sweep_fused3_f32(c, *cur, *oth, g3, tabs, anycp)
                                             : sldg_launch_sweep_fused3_f64(c, *cur, *oth, g3, tabs, anycp);
+        if (e == cudaErrorNotSupported) {                  // the launcher declined a shape the planner accepted: the
+            ev_cancel(c);                                   // same flip parity without the three-sweep pass
+            const int keep = c->opt_fuse3;
+            c->opt_fuse3 = 0;
+            r = advect_x_impl(c, cur, oth, dt, flip);
+            c->opt_fuse3 = keep;
+            return r;
+        }
         sldg_ev_end(c);
         c->launches++;
         if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
@@ -543,8 +578,16 @@ static int advect_x_impl(sldg_ctx* c, double** cur, double** oth, double dt, boo
     if (p.fused && !c->dry) {
         sldg_ev_begin(c, KIND_FUSED, 0);
         cudaError_t e = cudaErrorNotSupported;
-        if (c->opt_fused_impl != 2) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], (c->tab_anycp[0] || c->tab_anycp[1]) ? 1 : 0);
-        if (e == cudaErrorNotSupported && c->prec == SLDG_F64) e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        if (c->opt_fused_impl != 2 && !(c->opt_decline & 8)) e = sldg_launch_sweep_fused_cell(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], (c->tab_anycp[0] || c->tab_anycp[1]) ? 1 : 0);
+        if (e == cudaErrorNotSupported && c->prec == SLDG_F64 && !(c->opt_decline & 8)) e = sldg_launch_sweep_fused(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1]);
+        if (e == cudaErrorNotSupported) {                  // both fused kernels declined: the same flip parity from separate sweeps
+            ev_cancel(c);
+            const int keep = c->opt_fuse_x;
+            c->opt_fuse_x = 0;
+            r = advect_x_impl(c, cur, oth, dt, flip);
+            c->opt_fuse_x = keep;
+            return r;
+        }
         sldg_ev_end(c);
         c->launches++;
         if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
@@ -658,6 +701,22 @@ static int v_mode_standalone(const sldg_ctx* c)
     return best;
 }
 
+static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt, int mode);
+// A fused v pass declined by its launcher (cudaErrorNotSupported for a shape the planner accepted): the separate walks run
+// instead, and one device copy restores the buffer parity the plan counted on when theirs differs.  Results are the same
+// bits either way (include/sldg.h: the options change speed only).
+static int v_fallback(sldg_ctx* c, double** cur, double** oth, const double* E, double dt, int flips_planned)
+{
+    double* const want = (flips_planned & 1) ? *oth : *cur;
+    int r = advect_v_impl(c, cur, oth, E, dt, VM_WALKS);
+    if (r) return r;
+    if (*cur != want) {
+        if ((r = copy_back(c, want, *cur))) return r;
+        double* t = *cur; *cur = *oth; *oth = t;
+    }
+    return SLDG_OK;
+}
+
 // v-sweeps on (*cur, *oth) in the given mode; every pass is out of place and flips the pair.
 static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* E, double dt, int mode)
 {
@@ -678,8 +737,10 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         t2.S = c->vS2; t2.AB = c->vAB2; t3.S = c->vS3; t3.AB = c->vAB3;
         if (!c->dry) {
             sldg_ev_begin(c, KIND_FUSEDV3, c->dx);
-            cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv3_f32(c, *cur, *oth, tabs[0], t2, t3)
+            cudaError_t e = (c->opt_decline & 2) ? cudaErrorNotSupported
+                          : c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv3_f32(c, *cur, *oth, tabs[0], t2, t3)
                                                 : sldg_launch_sweep_fusedv3_f64(c, *cur, *oth, tabs[0], t2, t3);
+            if (e == cudaErrorNotSupported) { ev_cancel(c); return v_fallback(c, cur, oth, E, dt, v_flips(c, VM_FUSED3)); }
             sldg_ev_end(c);
             if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
         } else c->dry_v++;
@@ -695,8 +756,10 @@ static int advect_v_impl(sldg_ctx* c, double** cur, double** oth, const double* 
         t2.S = c->vS2; t2.AB = c->vAB2;
         if (!c->dry) {
             sldg_ev_begin(c, KIND_FUSEDV, c->dx);                  // axis field: first of the two fused axes
-            cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
+            cudaError_t e = (c->opt_decline & 1) ? cudaErrorNotSupported
+                          : c->prec == SLDG_F32 ? sldg_launch_sweep_fusedv_f32(c, *cur, *oth, tabs[0], t2)
                                                 : sldg_launch_sweep_fusedv_f64(c, *cur, *oth, tabs[0], t2);
+            if (e == cudaErrorNotSupported) { ev_cancel(c); return v_fallback(c, cur, oth, E, dt, v_flips(c, VM_FUSED2)); }
             sldg_ev_end(c);
             if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
         } else c->dry_v++;
@@ -834,8 +897,14 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
         SweepGeom g3[3] = {geom_of(c, 0), geom_of(c, 1), geom_of(c, 2)};
         const int anycp3 = (c->tab_anycp[0] || c->tab_anycp[1] || c->tab_anycp[2]) ? 1 : 0;
         sldg_ev_begin(c, KIND_FUSEDX3D, 0);
-        cudaError_t e3 = c->prec == SLDG_F32 ? sldg_launch_sweep_fused3d_f32(c, *cur, *oth, g3, tabs, anycp3)
+        cudaError_t e3 = (c->opt_decline & 16) ? cudaErrorNotSupported
+                       : c->prec == SLDG_F32 ? sldg_launch_sweep_fused3d_f32(c, *cur, *oth, g3, tabs, anycp3)
                                              : sldg_launch_sweep_fused3d_f64(c, *cur, *oth, g3, tabs, anycp3);
+        if (e3 == cudaErrorNotSupported) {                 // declined: the two half steps one after the other (one flip in all)
+            ev_cancel(c);
+            if ((r = advect_x_impl(c, cur, oth, tau, true))) return r;
+            return advect_x_impl(c, cur, oth, tau, false);
+        }
         sldg_ev_end(c);
         c->launches++;
         if (e3 != cudaSuccess) { c->last_cuda = (int)e3; return SLDG_ECUDA; }
@@ -844,8 +913,14 @@ static int advect_x_double(sldg_ctx* c, double** cur, double** oth, double tau)
     }
     const int anycp = (c->tab_anycp[0] || c->tab_anycp[1]) ? 1 : 0;
     sldg_ev_begin(c, KIND_FUSEDX2, 0);
-    cudaError_t e = c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], anycp)
+    cudaError_t e = (c->opt_decline & 16) ? cudaErrorNotSupported
+                  : c->prec == SLDG_F32 ? sldg_launch_sweep_fused_cell2_f32(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], anycp)
                                         : sldg_launch_sweep_fused_cell2_f64(c, *cur, *oth, geom_of(c, 0), geom_of(c, 1), tabs[0], tabs[1], anycp);
+    if (e == cudaErrorNotSupported) {                      // declined: the two half steps one after the other (one flip in all)
+        ev_cancel(c);
+        if ((r = advect_x_impl(c, cur, oth, tau, true))) return r;
+        return advect_x_impl(c, cur, oth, tau, false);
+    }
     sldg_ev_end(c);
     c->launches++;
     if (e != cudaSuccess) { c->last_cuda = (int)e; return SLDG_ECUDA; }
@@ -1095,6 +1170,8 @@ extern "C" int sldg_advect_axis(sldg_ctx* c, double* f, int axis, const double* 
         const int NN = c->K1 * c->K1;
         std::vector<int> S((size_t)X);
         std::vector<double> AB((size_t)(X * NN2)), ent((size_t)NN2);
+        for (long long x = 0; x < X; x++)
+            if (!isfinite(delta_host[x])) return SLDG_EINVAL;
         for (long long x = 0; x < X; x++) {
             host_entry(c, delta_host[x], c->cells[axis], &S[(size_t)x], ent.data());
             for (int m = 0; m < 2 * NN; m++) AB[(size_t)((long long)m * X + x)] = ent[(size_t)m];
@@ -1215,6 +1292,11 @@ extern "C" int sldg_timing_read(sldg_ctx* c, long long* launches, double* ms)
 {
     if (!c || !launches || !ms) return SLDG_EINVAL;
     CK(cudaStreamSynchronize(c->stream));
+    if (c->ev_failed) {                                     // some launches went unrecorded: no partial figures
+        for (auto& r : c->ev) c->ev_free.push_back(r);
+        c->ev.clear(); c->ev_failed = false;
+        return SLDG_ECUDA;
+    }
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
     for (auto& r : c->ev) {
@@ -1267,6 +1349,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "poisson_small")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_poisson_small = (int)value; return SLDG_OK; }
     if (!strcmp(name, "x_double")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_x_double = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "decline")) { if (value < 0 || value > 31) return SLDG_EINVAL; c->opt_decline = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fuse_v3")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v3 = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv3_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv3_wx = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv3_strip")) { if (value < 0 || value > 5) return SLDG_EINVAL; c->opt_fv3_strip = (int)value; return SLDG_OK; }

@@ -64,6 +64,14 @@ struct SweepGeom {
 
 struct EventRec { cudaEvent_t a, b; int kind, axis; };
 
+#define SLDG_XTAB_SLOTS 2
+struct XTab {                   // one cached x-sweep shift table (device): [D_{dx+a}] and [D_{dx+a}][2 K1^2]
+    int* dS; double* dAB;
+    double tau;                 // time increment it was built for
+    bool valid, anycp, safe;
+    unsigned long long used;    // last use (context clock)
+};
+
 struct sldg_ctx {
     int dx, dv, d, k, K1;
     int prec;                       // SLDG_F64 / SLDG_F32: storage and sweep arithmetic type of f (reading W)
@@ -81,12 +89,13 @@ struct sldg_ctx {
     int sm_count;
 
     // ctx-owned small device tables
-    int* dS[SLDG_MAX_DIM];          // x-sweep shift tables, one per x axis: [D_{dx+a}]
-    double* dAB[SLDG_MAX_DIM];      //                                       [D_{dx+a}][2 K1^2]
-    double tab_tau[SLDG_MAX_DIM];   // dt the cached table of x axis a was built for
-    bool tab_valid[SLDG_MAX_DIM];
-    bool tab_anycp[SLDG_MAX_DIM];   // some entry of the cached table has alpha == 0 (copy bit)
-    bool tab_safe[SLDG_MAX_DIM];    // every shift of the cached table is 0 or -1: a walk may run in place
+    // x-sweep shift tables: per x axis a cache of SLDG_XTAB_SLOTS tables (a Strang run alternates between dt/2 and, through
+    // sldg_advect_x, other increments: two slots keep both resident, least recently used evicted)
+    XTab xtab[3][SLDG_XTAB_SLOTS];
+    unsigned long long xtab_clock;
+    bool tab_anycp[SLDG_MAX_DIM];   // of the table selected by the last build_x_tables: some entry has alpha == 0 (copy bit)
+    bool tab_safe[SLDG_MAX_DIM];    //   "   : every shift is 0 or -1: a walk may run in place
+    bool ev_failed;                 // an instrumentation event could not be created: sldg_timing_read reports it
     int* dS_hook; double* dAB_hook; long long hook_cap;   // test-hook tables (x axes)
     double* dFwdT[3];               // forward transfer+DFT matrices, transposed [n][m], re then im
     double* dInvT[3];               // inverse DFT+transfer matrices, transposed
@@ -159,6 +168,7 @@ struct sldg_ctx {
     int opt_fv_ppb;                 // fused v kernel: planes per block (0 = auto)
     int opt_fv_cps;                 // fused v kernel, degree <= 1: v_2 cells per tensor copy
     int opt_fv_l2;                  // fused v kernel: L2 promotion of the tensor map (0 none, 1 64 B, 2 128 B, 3 256 B)
+    int opt_decline;                // test knob, bit mask: the launcher of a fused pass answers cudaErrorNotSupported (1 fused v_1v_2, 2 fused v_1v_2v_3, 4 fused x_1x_2x_3, 8 fused x_1x_2, 16 double x pass): the planned pass then falls back to separate sweeps
     int opt_fuse_v3;                // v_1, v_2 and v_3 sweeps in one pass (sldg_sweep_fusedv3.cu; dim_x = 3, degree <= 1): 0 never, 1 auto, 2 whenever the shape allows
     int opt_fv3_wx;                 // fused v_1v_2v_3 kernel: x nodes per tile (0 = auto)
     int opt_fv3_strip;              // fused v_1v_2v_3 kernel: v_2 donor pairs per strip (0 = auto: 4)

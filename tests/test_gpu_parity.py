@@ -534,3 +534,69 @@ def test_small_grid_poisson_in_one_launch_is_bitwise_the_multi_launch_route(P, g
     assert np.array_equal(outs[0][0], outs[1][0])
     assert outs[0][1] == 1 and outs[1][1] == dx + dx * (1 + dx)
     assert rel_inf(outs[0][0], o.poisson(rho.numpy())) <= 1e-12
+
+
+# --------------------------------------------------------------- boundary behaviour (include/sldg.h)
+
+def test_x_table_cache_holds_two_time_increments(P):
+    """include/sldg.h STREAM / SYNC: the x-sweep tables of two time increments stay cached per axis, so a caller that
+    alternates advect_x(dt) and advect_x(dt/2) uploads (and synchronises) only in the first two calls; a third
+    increment evicts the least recently used one."""
+    g, o = make_pair(P, 2, 2, [6, 5, 4, 3], 1)
+    f = W.random_field(o.shape, seed=5).to(g.device).contiguous()
+    g.timing_enable(True); g.timing_read()
+    g.advect_x(f, 0.1); g.advect_x(f, 0.05)
+    kinds, _ = g.timing_read()
+    assert kinds["copies"][0] == 2 * 2                       # two increments x two axes, one upload event each
+    for _ in range(3):
+        g.advect_x(f, 0.1); g.advect_x(f, 0.05)
+    kinds, _ = g.timing_read()
+    assert kinds["copies"][0] == 0                           # cached: no upload, no synchronisation
+    g.advect_x(f, 0.2); g.advect_x(f, 0.05); g.advect_x(f, 0.2)
+    kinds, _ = g.timing_read()
+    assert kinds["copies"][0] == 2                           # 0.2 evicted 0.1 (least recently used); 0.05 stayed
+    g.advect_x(f, 0.1)
+    kinds, _ = g.timing_read()
+    assert kinds["copies"][0] == 2
+    g.timing_enable(False)
+
+
+def test_non_finite_time_increment_and_shifts_are_rejected(P):
+    g, o = make_pair(P, 2, 2, [6, 5, 4, 3], 1)
+    f0 = W.random_field(o.shape, seed=5)
+    f = f0.to(g.device).contiguous()
+    for bad in (float("nan"), float("inf"), -float("inf")):
+        with pytest.raises(P.SldgError, match="invalid argument"):
+            g.advect_x(f, bad)
+        with pytest.raises(P.SldgError, match="invalid argument"):
+            g.step(f, bad)
+        d = np.zeros(o.D[2]); d[3] = bad
+        with pytest.raises(P.SldgError, match="invalid argument"):
+            g.advect_axis(f, 0, d)
+        d = np.zeros(o.X); d[7] = bad
+        with pytest.raises(P.SldgError, match="invalid argument"):
+            g.advect_axis(f, 2, d)
+    assert torch.equal(f.cpu(), f0)                          # nothing was enqueued
+
+
+@pytest.mark.parametrize("geom", [(2, 2, [8, 6, 6, 5], 1), (3, 3, [4, 3, 2, 4, 3, 2], 1), (2, 3, [6, 4, 5, 4, 3], 2)],
+                         ids=lambda g: f"{g[0]}x{g[1]}v-k{g[3]}")
+def test_declined_fused_passes_fall_back_to_the_same_bits(P, geom):
+    """include/sldg.h: a fused pass whose launcher declines (cudaErrorNotSupported) is replaced by the separate sweeps,
+    plus one device copy where the buffer parity differs -- same bits, never an error (test knob `decline`)."""
+    dx, dv, cells, k = geom
+    g, o = make_pair(P, dx, dv, cells, k)
+    f0 = W.random_field(o.shape, seed=8)
+    outs = []
+    for decline in (0, 1, 2, 4, 8, 16, 31):
+        g.set_option("graph", 0); g.set_option("fuse_v", 2); g.set_option("fuse_v3", 2); g.set_option("x_double", 2)
+        g.set_option("decline", decline)
+        fg = f0.to(g.device).contiguous()
+        g.steps(fg, 0.07, 3)
+        g.step(fg, 0.07)
+        E = g.last_E()
+        g.advect_v(fg, E, 0.07)
+        g.advect_x(fg, 0.07)
+        outs.append(fg.cpu().numpy())
+    for x in outs[1:]:
+        assert np.array_equal(outs[0], x)
