@@ -6,7 +6,10 @@ full-size device array, the complete x-space of a few velocity CELLS and the com
 runs the full-size GPU call, and compares those slabs with the oracle applied to the same slabs as a small problem
 (one cell per frozen axis).  Poisson runs on the full-size rho directly.  Single sweeps with random shift tables
 (CFL > 1 and integer) are checked on sampled lines with the oracle's line routine.
-Bars as in test_gpu_parity.py: 1e-12 per sweep, bit-exact for integer shifts.
+Bars as in test_gpu_parity.py: 1e-12 per sweep, bit-exact for integer shifts.  The same slab / line tests run in single
+precision mode (reading W) against the fp32 oracle (2e-6 per sweep, bit-exact integer shifts) on configs
+2-5, and in fp64 on the paper's fourth-order bump-on-tail workloads (k = 3).  Every comparison appends
+its measured error (max|g-o|/max|o| and the element-wise figure of reading L) to the parity report (conftest.py).
 """
 import numpy as np
 import pytest
@@ -18,6 +21,7 @@ from oracle import oracle as O
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-12
+TOL32 = 2e-6          # (2(k+1)+1) ulp32 of sum|A||u|, FMA chains against separately rounded products (reading W)
 
 
 def rel_inf(g, o):
@@ -56,28 +60,64 @@ def cell_domain(cfg, axis, i):
     return [lo + i * h, lo + (i + 1) * h]
 
 
-@pytest.fixture(scope="module", params=[1, 2, 3, 4], ids=lambda i: W.CONFIGS[i]["name"])
+ALL = {c["name"]: c for c in W.CONFIGS + W.NEXT_CONFIGS}
+FULL_CASES = ([(W.CONFIGS[i]["name"], "f64") for i in (1, 2, 3, 4)] + [(W.CONFIGS[i]["name"], "f32") for i in (1, 2, 3, 4)] +
+              [("bot_5d_k3_16", "f64"), ("bot_6d_k3_9", "f64")])
+
+
+class Full:
+    """One full-size problem on the device plus the oracle's functions of its precision."""
+
+    def __init__(self, cfg, g, f, prec):
+        self.cfg, self.g, self.f, self.prec = cfg, g, f, prec
+        self.tol = TOL if prec == "f64" else TOL32
+        self.np_dtype = np.float64 if prec == "f64" else np.float32
+
+    def o_advect_x(self, o, b, tau):
+        return o.advect_x(b, tau) if self.prec == "f64" else o.advect_x_f32(b, tau)
+
+    def o_advect_v(self, o, b, E, tau):
+        return o.advect_v(b, E, tau) if self.prec == "f64" else o.advect_v_f32(b, E, tau)
+
+    def o_density(self, o, b):
+        return o.density(b) if self.prec == "f64" else o.density_f32(b)
+
+    def mass_tol(self):
+        return 1e-12 if self.prec == "f64" else 2e-6
+
+
+@pytest.fixture(scope="module", params=FULL_CASES, ids=lambda c: f"{c[0]}-{c[1]}")
 def full(request, P):
-    cfg = W.CONFIGS[request.param]
-    need = 2 * W.field_elems(cfg) * 8 + (6 << 30)
+    name, prec = request.param
+    cfg = ALL[name]
+    es = 8 if prec == "f64" else 4
+    need = 2 * W.field_elems(cfg) * es + (6 << 30)
     free, _ = torch.cuda.mem_get_info()
     if free < need:
         pytest.fail(f"{cfg['name']}: needs {need >> 30} GiB of device memory, {free >> 30} GiB free")
-    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    g = P.Sldg(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"], precision=prec)
     f = g.empty_field()
-    W.initial_data(cfg, [g.node_coords(a) for a in range(g.d)], device=g.device, out=f)
-    W.perturb_inplace(f, seed=W.SEED + request.param)
-    yield cfg, g, f
+    coords = [g.node_coords(a) for a in range(g.d)]
+    if prec == "f32":                     # the generator works in fp64: fill slab by slab along the slowest axis
+        D = f.shape[0]
+        step = max(1, D // 8)
+        for a in range(0, D, step):
+            b = min(D, a + step)
+            f[a:b].copy_(W.initial_data(cfg, coords[:-1] + [coords[-1][a:b]], device=g.device))
+    else:
+        W.initial_data(cfg, coords, device=g.device, out=f)
+    W.perturb_inplace(f, seed=W.SEED + len(name))
+    yield Full(cfg, g, f, prec)
     g.close()
     del f
     torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("xcopy", [0, 1], ids=["even-parity plan", "odd-parity plan (the one-pass fused sweeps)"])
-def test_advect_x_on_full_x_space_of_sampled_velocity_cells(full, xcopy):
+def test_advect_x_on_full_x_space_of_sampled_velocity_cells(full, xcopy, parity_report):
     """x_copy = 1 runs the plan sldg_step / sldg_steps use for their flipping x half steps: the fused x1+x2 pass
     (dim_x = 2) or the fused x1+x2+x3 pass (dim_x = 3), in the launch configuration bench.py times."""
-    cfg, g, f = full
+    cfg, g, f = full.cfg, full.g, full.f
     g.set_option("x_copy", xcopy)
     dx, dv = cfg["dim_x"], cfg["dim_v"]
     vaxes = list(range(dx, dx + dv))
@@ -86,20 +126,22 @@ def test_advect_x_on_full_x_space_of_sampled_velocity_cells(full, xcopy):
     tau = cfg["dt"] / 2
     m0 = g.mass(f)
     g.advect_x(f, tau)
-    assert abs(g.mass(f) - m0) <= 1e-12 * abs(m0)
+    assert abs(g.mass(f) - m0) <= full.mass_tol() * abs(m0)
     for c, b in zip(cells, before):
         dom = list(cfg["domain"][:2 * dx])
         for a, i in zip(vaxes, c):
             dom += cell_domain(cfg, a, i)
         o = O.Oracle(dx, dv, cfg["cells"][:dx] + [1] * dv, cfg["degree"], dom, threads=O.lib().orc_max_threads())
-        want = o.advect_x(b, tau)
+        want = full.o_advect_x(o, b, tau)
         got = f[slab_index(g, vaxes, c)].cpu().numpy()
-        assert rel_inf(got, want) <= TOL * dx, (c, rel_inf(got, want))
+        err = parity_report.add("advect_x full x-space of a v cell", cfg["name"], f"x_copy={xcopy} v-cell {c}", got, want,
+                                full.tol * dx, full.prec)
+        assert err <= full.tol * dx, (c, err)
     g.set_option("x_copy", 0)
 
 
-def test_density_poisson_advect_v_on_full_v_space_of_sampled_x_cells(full):
-    cfg, g, f = full
+def test_density_poisson_advect_v_on_full_v_space_of_sampled_x_cells(full, parity_report):
+    cfg, g, f = full.cfg, full.g, full.f
     dx, dv = cfg["dim_x"], cfg["dim_v"]
     xaxes = list(range(dx))
     cells = cell_samples(cfg["cells"][:dx], 5, seed=2)
@@ -118,37 +160,49 @@ def test_density_poisson_advect_v_on_full_v_space_of_sampled_x_cells(full):
     k1 = cfg["degree"] + 1
     xsl = [tuple(slice(i * k1, (i + 1) * k1) for i in reversed(c)) for c in cells]
     scale = np.abs(rho_h).max()
-    for o, b, sl in zip(smalls, before, xsl):
-        assert np.abs(rho_h[sl] - o.density(b)).max() <= TOL * scale
+    for o, b, sl, c in zip(smalls, before, xsl, cells):
+        want = full.o_density(o, b)
+        parity_report.add("density of an x cell (scaled by max rho)", cfg["name"], f"x-cell {c}", rho_h[sl] / scale, want / scale,
+                          TOL, full.prec)
+        assert np.abs(rho_h[sl] - want).max() <= TOL * scale
     # Poisson on the full-size rho (the oracle's naive DFT handles X <= 110592)
     ofull = O.Oracle(dx, dv, cfg["cells"][:dx] + [1] * dv, cfg["degree"],
                      list(cfg["domain"][:2 * dx]) + [0.0, 1.0] * dv, threads=O.lib().orc_max_threads())
     E = g.poisson(rho)
     E_h = E.cpu().numpy()
     E_o = ofull.poisson(rho_h)
-    assert rel_inf(E_h, E_o) <= 1e-11, rel_inf(E_h, E_o)
+    # the stated per-operation bar, also on the largest x grids (measured: at most 5.2e-13, profiles/r2_parity.md)
+    err = parity_report.add("poisson on the full-size rho", cfg["name"], f"X={g.X}", E_h, E_o, TOL, full.prec)
+    assert err <= TOL, err
     # advect_v with the physical field and with a strong seeded field (|delta| up to ~3 cells)
     hv = (cfg["domain"][2 * dx + 1] - cfg["domain"][2 * dx]) / cfg["cells"][dx]
     dt = cfg["dt"]
     strong = W.random_E(dx, g.xshape, amplitude=3.0 * hv / dt, device=g.device)
-    for Efield in (E, strong):
+    # second run: every fused v pass the shape allows, forced (dim_x = 3: the one-pass v_1+v_2+v_3 sweep that sldg_steps plans)
+    for Efield, force in ((E, 1), (strong, 2)):
         Eh = Efield.cpu().numpy()
         m0 = g.mass(f)
+        g.set_option("fuse_v", force); g.set_option("fuse_v3", force)
         g.advect_v(f, Efield, dt)
-        assert abs(g.mass(f) - m0) <= 1e-12 * abs(m0)
+        g.set_option("fuse_v", 1); g.set_option("fuse_v3", 1)
+        assert abs(g.mass(f) - m0) <= full.mass_tol() * abs(m0)
         after = []
         for o, b, c, sl in zip(smalls, before, cells, xsl):
-            want = o.advect_v(b, np.ascontiguousarray(Eh[(slice(None),) + sl]), dt)
+            want = full.o_advect_v(o, b, np.ascontiguousarray(Eh[(slice(None),) + sl]), dt)
             got = f[slab_index(g, xaxes, c)].cpu().numpy()
-            assert rel_inf(got, want) <= TOL * dx, (c, rel_inf(got, want))
+            err = parity_report.add("advect_v full v-space of an x cell", cfg["name"],
+                                    f"{'physical E' if force == 1 else 'strong seeded E, fused passes forced'} x-cell {c}", got, want,
+                                    full.tol * dx, full.prec)
+            assert err <= full.tol * dx, (c, err)
             after.append(got)
         before = after
 
 
 @pytest.mark.parametrize("kind", ["cfl", "intmix"])
-def test_single_sweeps_on_sampled_lines(full, kind):
-    """Every swept axis through the test hook at full size; 4096 seeded lines per axis against orc_sweep_line."""
-    cfg, g, f = full
+def test_single_sweeps_on_sampled_lines(full, kind, parity_report):
+    """Every swept axis through the test hook at full size; 4092 seeded lines per axis against orc_sweep_line (fp32: the
+    lines as a 1x1v problem through orc_sweep_axis_f32, one shift per line)."""
+    cfg, g, f = full.cfg, full.g, full.f
     dx = cfg["dim_x"]
     k = cfg["degree"]
     rng = np.random.default_rng(7)
@@ -158,7 +212,7 @@ def test_single_sweeps_on_sampled_lines(full, kind):
         outer = g.nf // (inner * Da)
         n = g.D[dx + axis] if axis < dx else g.X
         delta = W.delta_table(n, kind, seed=W.SEED + axis, ncells=cfg["cells"][axis]).numpy()
-        ns = 4096
+        ns = 4092                      # divisible by k+1 = 1..4
         q = np.concatenate([[0, outer - 1], rng.integers(0, outer, ns - 2)])
         p = np.concatenate([[0, inner - 1], rng.integers(0, inner, ns - 2)])
         qt, pt = torch.from_numpy(q).to(g.device), torch.from_numpy(p).to(g.device)
@@ -171,19 +225,26 @@ def test_single_sweeps_on_sampled_lines(full, kind):
             sidx = (q // sdiv) % g.D[dx + axis]
         else:                  # shift index = flat x node
             sidx = p % g.X
-        want = np.stack([O.sweep_line(k, lines_in[i], delta[sidx[i]]) for i in range(ns)])
+        if full.prec == "f64":
+            want = np.stack([O.sweep_line(k, lines_in[i], delta[sidx[i]]) for i in range(ns)])
+        else:
+            ol = O.Oracle(1, 1, [cfg["cells"][axis], ns // (k + 1)], k, [0.0, 1.0, 0.0, 1.0], threads=O.lib().orc_max_threads())
+            want = ol.sweep_axis_f32(lines_in, 0, delta[sidx])
         if kind == "intmix":
             assert np.array_equal(lines_out, want), axis
         else:
-            assert rel_inf(lines_out, want) <= TOL, (axis, rel_inf(lines_out, want))
+            err = parity_report.add("single sweep on 4092 sampled lines", cfg["name"], f"axis {axis}, CFL > 1 shifts", lines_out, want,
+                                    full.tol, full.prec)
+            assert err <= full.tol, (axis, err)
 
 
 def test_constants_are_preserved_by_two_steps_at_full_size(full):
     """rows of A + B sum to 1 (invariant p4), so a constant f stays constant to round-off through
     every sweep of sldg_steps at full size (fused passes, in-place walks, v sweeps with E = 0 up to round-off).
     Runs last: it overwrites the module's f."""
-    cfg, g, f = full
+    cfg, g, f = full.cfg, full.g, full.f
     f.fill_(0.375)
     g.steps(f, cfg["dt"], 2)
     lo, hi = float(f.min()), float(f.max())
-    assert abs(lo - 0.375) <= 1e-13 and abs(hi - 0.375) <= 1e-13, (lo, hi)
+    bar = 1e-13 if full.prec == "f64" else 2e-6
+    assert abs(lo - 0.375) <= bar and abs(hi - 0.375) <= bar, (lo, hi)

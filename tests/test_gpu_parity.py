@@ -189,7 +189,7 @@ def test_advect_v_constant_dyadic_field_is_exact_integer_shift(P):
 
 
 @pytest.mark.parametrize("cfg", small_cfgs(), ids=lambda c: c["name"])
-def test_ten_strang_steps(P, cfg):
+def test_ten_strang_steps(P, cfg, parity_report):
     g, o = pair_of_cfg(P, cfg)
     coords = [o.node_coords(a) for a in range(o.d)]
     f0 = W.initial_data(cfg, coords)
@@ -199,10 +199,11 @@ def test_ten_strang_steps(P, cfg):
     for _ in range(10):
         g.step(fg, cfg["dt"])
         fo, rho_o, E_o = o.step(fo, cfg["dt"])
-    assert rel_inf(fg.cpu().numpy(), fo) <= TOL_STEPS
-    assert rel_inf(g.last_rho().cpu().numpy(), rho_o) <= TOL_STEPS
-    # E is a difference quantity (rho - 1 ~ 1e-2..1e-3): relative to max|E| it inherits rho's absolute error
-    assert np.abs(g.last_E().cpu().numpy() - E_o).max() <= TOL_STEPS * max(1.0, np.abs(E_o).max())
+    assert parity_report.add("10 Strang steps", cfg["name"], "f", fg.cpu().numpy(), fo, TOL_STEPS) <= TOL_STEPS
+    assert parity_report.add("10 Strang steps", cfg["name"], "rho of step 10", g.last_rho().cpu().numpy(), rho_o, TOL_STEPS) <= TOL_STEPS
+    # E comes from rho - 1 (1e-2..1e-3 of rho), so relative to max|E| it carries rho's error times max|rho| / max|rho - 1|;
+    # the stated relative bar still holds with two orders to spare (profiles/r2_parity.md)
+    assert parity_report.add("10 Strang steps", cfg["name"], "E of step 10", g.last_E().cpu().numpy(), E_o, TOL_STEPS) <= TOL_STEPS
     assert abs(g.mass(fg) - m0) <= 1e-12 * abs(m0)
     assert abs(g.mass(fg) - o.mass(fo)) <= 1e-12 * abs(m0)
     Eg = g.last_E()
@@ -219,7 +220,7 @@ def next_cfgs():
 
 
 @pytest.mark.parametrize("cfg", next_cfgs(), ids=lambda c: c["name"])
-def test_bump_on_tail_and_cfl_above_one_ten_strang_steps(P, cfg):
+def test_bump_on_tail_and_cfl_above_one_ten_strang_steps(P, cfg, parity_report):
     g, o = pair_of_cfg(P, cfg)
     f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
     fg, fo = f0.to(g.device).contiguous(), f0.numpy()
@@ -227,8 +228,9 @@ def test_bump_on_tail_and_cfl_above_one_ten_strang_steps(P, cfg):
     for _ in range(10):
         g.step(fg, cfg["dt"])
         fo, rho_o, E_o = o.step(fo, cfg["dt"])
-    assert rel_inf(fg.cpu().numpy(), fo) <= TOL_STEPS
-    assert np.abs(g.last_E().cpu().numpy() - E_o).max() <= TOL_STEPS * max(1.0, np.abs(E_o).max())
+    assert parity_report.add("10 Strang steps (k = 3, CFL up to 5)", cfg["name"], "f", fg.cpu().numpy(), fo, TOL_STEPS) <= TOL_STEPS
+    assert parity_report.add("10 Strang steps (k = 3, CFL up to 5)", cfg["name"], "E of step 10", g.last_E().cpu().numpy(), E_o,
+                             TOL_STEPS) <= TOL_STEPS
     assert abs(g.mass(fg) - m0) <= 1e-12 * abs(m0)
 
 
