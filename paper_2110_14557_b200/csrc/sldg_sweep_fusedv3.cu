@@ -211,8 +211,10 @@ __global__ void __launch_bounds__(FV3_MAXT)
         const long long stepX = X, stepRow = rowX - (long long)(K1 - 1) * X;
         real* o3 = P.fout + (long long)(c * K1) * X + x0 + x + (long long)io3 * cell3X + (long long)ov2_0 * cell2X;
 
-#pragma unroll 1
-        for (int j = 0; j <= N3; j++) {
+        // one v_3 cell: FIRST = the cell that only initialises the walk (no output); peeled so that the walk's loop carries no
+        // `first cell?` branches
+        auto cell = [&](auto first_t) {
+            constexpr bool FIRST = decltype(first_t)::value;
             real g[2][N3V];
             real* o2 = o3;
             int ov2 = ov2_0;
@@ -258,7 +260,7 @@ __global__ void __launch_bounds__(FV3_MAXT)
                                     for (int l = 0; l < K1; l++) acc += t2[j2 * 2 * K1 + K1 + l] * prv[(j3 * K1 + l) * K1 + j1];
                                     h[j3] = (CP && cp2) ? nxt[(j3 * K1 + j2) * K1 + j1] : acc;
                                 }
-                                if (j > 0) {
+                                if constexpr (!FIRST) {
 #pragma unroll
                                     for (int j3 = 0; j3 < K1; j3++) {
                                         real acc = 0;
@@ -279,11 +281,14 @@ __global__ void __launch_bounds__(FV3_MAXT)
                     }
                 }
             }
-            if (j > 0) {
+            if constexpr (!FIRST) {
                 o3 += cell3X;
                 if (++io3 == N3) { io3 = 0; o3 -= wrap3; }
             }
-        }
+        };
+        cell(std::true_type{});
+#pragma unroll 1
+        for (int j = 1; j <= N3; j++) cell(std::false_type{});
     };
     if (anycp) body(std::true_type{});
     else body(std::false_type{});
