@@ -602,3 +602,26 @@ def test_declined_fused_passes_fall_back_to_the_same_bits(P, geom):
         outs.append(fg.cpu().numpy())
     for x in outs[1:]:
         assert np.array_equal(outs[0], x)
+
+
+def test_v_shard_plumbing_drives_the_cuda_context(P):
+    """paper_2110_14557_b200/shard.py with the CUDA context as its engine (single rank: the halo exchange is the periodic
+    wrap of the rank's own slab): a context on the widened sub-domain for the sweeps, one on the interior for rho.  The
+    interior must equal the plain single-domain steps (same sweeps; rho summed over the same values in another order)."""
+    from paper_2110_14557_b200 import shard as S
+    cfg = W.scaled(W.CONFIGS[0], [6, 4, 6, 8])
+    g, o = pair_of_cfg(P, cfg)
+    f0 = W.initial_data(cfg, [o.node_coords(a) for a in range(o.d)])
+    ref = f0.to(g.device).contiguous()
+    for _ in range(3):
+        g.step(ref, cfg["dt"])
+    geom = S.Geometry(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
+    H = 2
+    sh = S.VShard(geom, 0, 1, H, lambda gm: P.Sldg(gm.dim_x, gm.dim_v, gm.cells, gm.degree, gm.domain))
+    k1 = cfg["degree"] + 1
+    f_ext = torch.zeros(tuple(reversed([c * k1 for c in sh.extended.cells])), dtype=torch.float64, device=g.device)
+    sh.interior_of(f_ext).copy_(f0)
+    for _ in range(3):
+        sh.step(f_ext, cfg["dt"])
+    got, want = sh.interior_of(f_ext).cpu().numpy(), ref.cpu().numpy()
+    assert rel_inf(got, want) <= 1e-13
