@@ -149,21 +149,27 @@ __global__ void __launch_bounds__(F3D_MAXT + 32) sweep_fused3d_kernel(const F3DP
     for (int j = 0; j < ST; j++) issue_load(j);
 
     // x_1- then x_2-swept (k+1)^3 block [j3][j2][j1] of this thread's (x_1 cell, x_2 slot mu) from a stage whose planes
-    // are `tp` values apart: donors are the stage's slots mu + 1 (A) and mu (B)
+    // are `tp` values apart: donors are the stage's slots mu + 1 (A) and mu (B).  Addresses: four per-thread bases (A / B
+    // donor slot x the two x_1 donor cells), computed once, plus block-uniform offsets j3 * tp + j2 * D0 -- nothing is
+    // recomputed per load (the first version of this kernel spent a quarter of its issue slots on index arithmetic).
+    const int pAa = ((mu + 1) * K1) * D0 + oa, pAb = ((mu + 1) * K1) * D0 + ob;
+    const int pBa = (mu * K1) * D0 + oa, pBb = (mu * K1) * D0 + ob;
     auto swept12 = [&](const real* stage, int tp, real (&N)[N3]) {
+        const real* const qAa = stage + pAa;
+        const real* const qAb = stage + pAb;
+        const real* const qBa = stage + pBa;
+        const real* const qBb = stage + pBb;
 #pragma unroll
         for (int j3 = 0; j3 < K1; j3++) {
-            const real* plane = stage + j3 * tp;
             real sw[2][NN];                                // [A-donor | B-donor][j2'][j1]
 #pragma unroll
             for (int dn = 0; dn < 2; dn++) {
-                const int slot = mu + 1 - dn;
 #pragma unroll
                 for (int j2 = 0; j2 < K1; j2++) {
-                    const real* row = plane + (slot * K1 + j2) * D0;
+                    const int uo = j3 * tp + j2 * D0;      // block-uniform
                     V3D<K1> a, b;
-                    a.load(row + oa);
-                    b.load(row + ob);
+                    a.load((dn ? qBa : qAa) + uo);
+                    b.load((dn ? qBb : qAb) + uo);
 #pragma unroll
                     for (int j1 = 0; j1 < K1; j1++) {
                         real acc = 0;
@@ -204,7 +210,7 @@ __global__ void __launch_bounds__(F3D_MAXT + 32) sweep_fused3d_kernel(const F3DP
                     for (int l = 0; l < K1; l++) acc += B3[j3 * K1 + l] * prv[(l * K1 + j2) * K1 + j1];
                     r.v[j1] = (CP && cp3) ? nxt[(j3 * K1 + j2) * K1 + j1] : acc;
                 }
-                r.store(obase + j3 * op + j2 * D0);
+                r.store(obase + (j3 * op + j2 * D0));      // block-uniform offset
             }
     };
     const int cofs = (mu * K1) * D0 + i0 * K1;             // this thread's cell inside a mid / output plane
