@@ -263,7 +263,7 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
     ms_single_calls = s0.elapsed_time(s1) / steps
     # ---- the same K steps again with CUDA events around every launch (on the library's stream): per-kernel figures
     g.timing_enable(True)
-    g.steps(f, dt, 2)                         # untimed: with events on, small problems leave the graph path (kernels load here)
+    g.steps(f, dt, steps)                     # untimed, same plan: with events on, small problems leave the graph path (kernels load here)
     g.timing_read()
     g.steps(f, dt, steps)
     kinds, axes = g.timing_read()
