@@ -120,9 +120,11 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     const int run1 = min(nS + 1, N1 - d0);                 // cells before the periodic wrap
     const uint32_t cellb = (uint32_t)CELL * ES;
 
+    int lst = 0;                                           // producer: stage of the next load (loads are issued in order)
     auto issue_load = [&](int j) {                         // x_3 cell j -> stage j % ST
         if (lead && j < N2) {
-            const int st = j % ST;
+            const int st = lst;
+            if (++lst == ST) lst = 0;
             const uint32_t bar = bars_s + (uint32_t)st * 8u;
             mbar_expect_tx(bar, (uint32_t)(K1 * (nS + 1)) * cellb);
 #pragma unroll
@@ -142,21 +144,27 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     __syncthreads();
     for (int j = 0; j < ST; j++) issue_load(j);
 
-    // x_1- then x_2-swept (k+1)^3 block [j3][j2][j1] of this thread's (x_1 cell, x_2 cell) from one input stage
+    // x_1- then x_2-swept (k+1)^3 block [j3][j2][j1] of this thread's (x_1 cell, x_2 cell) from one input stage.
+    // Addresses: four per-thread bases (A / B donor slot x the two x_1 donor cells), computed once, plus block-uniform
+    // offsets j3 * TP + j2 * D0: no index arithmetic per load.
+    const int pAa = ((e1 + 1) * K1) * D0 + oa, pAb = ((e1 + 1) * K1) * D0 + ob;
+    const int pBa = (e1 * K1) * D0 + oa, pBb = (e1 * K1) * D0 + ob;
     auto swept12 = [&](const real* stage, real (&N)[N3]) {
+        const real* const qAa = stage + pAa;
+        const real* const qAb = stage + pAb;
+        const real* const qBa = stage + pBa;
+        const real* const qBb = stage + pBb;
 #pragma unroll
         for (int j3 = 0; j3 < K1; j3++) {
-            const real* plane = stage + j3 * TP;
             real sw[2][NN];                                // [A-donor cell c-s_2 | B-donor cell c-s_2-1][j2'][j1]
 #pragma unroll
             for (int dn = 0; dn < 2; dn++) {
-                const int slot = e1 + 1 - dn;
 #pragma unroll
                 for (int j2 = 0; j2 < K1; j2++) {
-                    const real* row = plane + (slot * K1 + j2) * D0;
+                    const int uo = j3 * TP + j2 * D0;      // block-uniform
                     V3<K1> a, b;
-                    a.load(row + oa);
-                    b.load(row + ob);
+                    a.load((dn ? qBa : qAa) + uo);
+                    b.load((dn ? qBb : qAb) + uo);
 #pragma unroll
                     for (int j1 = 0; j1 < K1; j1++) {
                         real acc = 0;
@@ -194,23 +202,26 @@ __global__ void __launch_bounds__(288) sweep_fused3_kernel(const F3Params P)
     issue_load(ST);
 
     int io3 = s3 + 1; if (io3 >= N2) io3 -= N2;            // output x_3 cell of the current donor pair
+    int cst = (ST > 1) ? 1 : 0;                            // consumers: stage and phase of the next input cell (cell 1)
+    uint32_t cph = (ST > 1) ? 0u : 1u;
+    const int cofs = (e1 * K1) * D0 + i0 * K1;             // this thread's cell inside an output plane
     // one step of the x_3 walk: nxt <- swept block of input cell h+1 (or the first one), output cell from (nxt, prv).
     // The walk alternates between `prev` and `alt` (two steps per trip): no register moves between steps.
     real alt[N3];
     auto step3 = [&](int h, real (&nxt)[N3], const real (&prv)[N3]) {
         const int j = h + 1;
-        const int st = j % ST;
         if (j < N2) {
             if (active) {
-                mbar_wait(bars_s + (uint32_t)st * 8u, (uint32_t)((j / ST) & 1));
-                swept12(sin_ + st * SS, nxt);
+                mbar_wait(bars_s + (uint32_t)cst * 8u, cph);
+                swept12(sin_ + cst * SS, nxt);
             }
+            if (++cst == ST) { cst = 0; cph ^= 1u; }
         } else {
 #pragma unroll
             for (int m = 0; m < N3; m++) nxt[m] = first[m];
         }
         if (active) {
-            real* obase = sout + (h & 1) * OS + (e1 * K1) * D0 + i0 * K1;
+            real* obase = sout + (h & 1) * OS + cofs;
 #pragma unroll
             for (int j3 = 0; j3 < K1; j3++)
 #pragma unroll
