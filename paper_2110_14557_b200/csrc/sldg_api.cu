@@ -139,7 +139,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     c->cg_maxiter = 0;
     memset(c->t_launch, 0, sizeof(c->t_launch)); memset(c->t_ms, 0, sizeof(c->t_ms));
     memset(c->a_launch, 0, sizeof(c->a_launch)); memset(c->a_ms, 0, sizeof(c->a_ms));
-    c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
+    c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_rho_tma = 1; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_f3d_threads = 128; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     c->opt_poisson_small = 1; c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
     c->opt_decline = 0; c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0;
@@ -1360,6 +1360,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "fv_ppb")) { if (value < 0 || value > (1 << 20)) return SLDG_EINVAL; c->opt_fv_ppb = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_cps")) { if (value < 1 || value > 8) return SLDG_EINVAL; c->opt_fv_cps = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_l2")) { if (value < 0 || value > 3) return SLDG_EINVAL; c->opt_fv_l2 = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "rho_tma")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_rho_tma = (int)value; return SLDG_OK; }
     if (!strcmp(name, "rho_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_rho_vec = (int)value; return SLDG_OK; }
     if (!strcmp(name, "rho_blocks")) { if (value < 1 || value > 64) return SLDG_EINVAL; c->opt_rho_blocks = (int)value; return SLDG_OK; }
     if (!strcmp(name, "walk_vec")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_walk_vec = (int)value; return SLDG_OK; }

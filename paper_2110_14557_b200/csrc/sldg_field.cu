@@ -3,7 +3,9 @@
 //  rho[x] = sum_v W_v f[x,v]   HBM-bound: one read of f
 //  -Laplace phi = 1 - rho, E = -grad phi  (reading P1)     tiny, latency-bound
 //  per-x-node shift tables of the v-sweeps
+#include "sldg_async.h"
 #include "sldg_internal.h"
+#include "sldg_tmap.h"
 
 // The polynomial coefficients of A(alpha), B(alpha) depend on the degree: each context owns its device copy (c->dPoly),
 // so contexts of different degree can live side by side.
@@ -102,6 +104,87 @@ __global__ void __launch_bounds__(128) rho_partial_kernel(const T* __restrict__ 
     }
 #pragma unroll
     for (int e = 0; e < VEC; e++) part[(long long)blockIdx.y * X + x + e] = acc[e];
+}
+
+// rho by TMA (large problems): f seen as [V][X]; a block owns a tile of 32 x values and a chunk of v rows and streams boxes
+// of 32 x RHO_ROWS values (2-d tensor copies into a full/empty mbarrier ring; tests/test_gpu_probe.py: this path streams at
+// 1.05-1.1 of the device-copy rate, the plain-load kernel above at 0.95).  Lane = two x values, warp w sums rows w, w + 8, ... of
+// every box in ascending v with fma(W_v, f, acc); the eight warps' sums are added in warp order: deterministic.
+constexpr int RHO_WX = 64, RHO_ROWS = 32, RHO_WARPS = 8;     // lane = TWO x values (one 16-byte / 8-byte load per row)
+struct RhoTmaParams { const double* Wv; double* part; long long X, V, vchunk; int ntiles, slots; uint32_t slot_bytes; };
+
+template <class T>
+__global__ void __launch_bounds__(RHO_WARPS * 32) rho_tma_kernel(const __grid_constant__ CUtensorMap tmap, const RhoTmaParams P)
+{
+    using namespace sldg_async;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    const int ST = P.slots;
+    const uint32_t ring_s = smem_u32(smem_raw);
+    const uint32_t full_s = ring_s + (uint32_t)ST * P.slot_bytes, empty_s = full_s + 8u * ST;
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const int tile = (int)(blockIdx.x % (unsigned)P.ntiles);
+    const long long chunk = blockIdx.x / (unsigned)P.ntiles;
+    const long long v0 = chunk * P.vchunk;
+    const long long v1 = min(P.V, v0 + P.vchunk);
+    const int total = (int)((v1 - v0 + RHO_ROWS - 1) / RHO_ROWS);
+    if (t == 0) {
+        for (int s = 0; s < ST; s++) { mbar_init(full_s + 8u * s, 1); mbar_init(empty_s + 8u * s, RHO_WARPS); }
+        mbar_init_fence();
+    }
+    __syncthreads();
+    const uint32_t box_bytes = (uint32_t)(RHO_ROWS * RHO_WX * sizeof(T));
+    int pst = 0, pn = 0, pi = 0;
+    auto produce = [&]() {
+        if (pi >= total) return;
+        if (pn > 0) mbar_wait(empty_s + 8u * pst, (uint32_t)((pn - 1) & 1));
+        mbar_expect_tx(full_s + 8u * pst, box_bytes);
+        asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                     ::"r"(ring_s + (uint32_t)pst * P.slot_bytes), "l"(&tmap), "r"(tile * RHO_WX), "r"((int)(v0 + (long long)pi * RHO_ROWS)),
+                       "r"(full_s + 8u * pst) : "memory");
+        if (++pst == ST) { pst = 0; pn++; }
+        pi++;
+    };
+    if (t == 0) for (int i = 0; i < ST - 1; i++) produce();
+    int st = 0; uint32_t ph = 0;
+    double acc0[2] = {0.0, 0.0}, acc1[2] = {0.0, 0.0};              // [x value of the lane], even / odd rows of this warp
+    for (int i = 0; i < total; i++) {
+        if (t == 0) produce();
+        const long long vb = v0 + (long long)i * RHO_ROWS;
+        double wv[RHO_ROWS / RHO_WARPS];                            // the weights do not depend on the box: loaded before the wait
+#pragma unroll
+        for (int r = 0; r < RHO_ROWS / RHO_WARPS; r++) {
+            const long long v = vb + w + r * RHO_WARPS;
+            wv[r] = (v < v1) ? __ldg(P.Wv + v) : 0.0;               // rows past the chunk (zero-filled, or the next chunk's) count 0
+        }
+        mbar_wait(full_s + 8u * st, ph);
+        typedef typename Pair<T>::type T2;
+        const T2* box = reinterpret_cast<const T2*>(smem_raw + (size_t)st * P.slot_bytes) + lane;
+        T2 val[RHO_ROWS / RHO_WARPS];
+#pragma unroll
+        for (int r = 0; r < RHO_ROWS / RHO_WARPS; r++) val[r] = box[(w + r * RHO_WARPS) * (RHO_WX / 2)];
+        fence_async_smem();                                         // generic-proxy reads -> the slot's refill by the async proxy
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty_s + 8u * st);
+#pragma unroll
+        for (int r = 0; r < RHO_ROWS / RHO_WARPS; r += 2) {
+            acc0[0] = fma(wv[r], (double)val[r].x, acc0[0]);         acc0[1] = fma(wv[r], (double)val[r].y, acc0[1]);
+            acc1[0] = fma(wv[r + 1], (double)val[r + 1].x, acc1[0]); acc1[1] = fma(wv[r + 1], (double)val[r + 1].y, acc1[1]);
+        }
+        if (++st == ST) { st = 0; ph ^= 1u; }
+    }
+    __syncthreads();                                                // the ring is drained: reuse it for the warps' sums
+    double* red = reinterpret_cast<double*>(smem_raw);
+    red[w * RHO_WX + 2 * lane] = acc0[0] + acc1[0];
+    red[w * RHO_WX + 2 * lane + 1] = acc0[1] + acc1[1];
+    __syncthreads();
+    if (w < 2) {                                                    // warp 0: x values 0..31 of the tile, warp 1: 32..63
+        const int xi = w * 32 + lane;
+        double s = 0.0;
+#pragma unroll
+        for (int u = 0; u < RHO_WARPS; u++) s += red[u * RHO_WX + xi];
+        const long long x = (long long)tile * RHO_WX + xi;
+        if (x < P.X) P.part[chunk * P.X + x] = s;
+    }
 }
 
 __global__ void rho_final_kernel(const double* __restrict__ part, long long X, int nchunk, double* __restrict__ rho)
@@ -346,8 +429,64 @@ cudaError_t sldg_launch_wv(sldg_ctx* c)
     return cudaGetLastError();
 }
 
+// rho through the TMA kernel when the problem is large enough to fill the GPU with x tiles x v chunks; cudaErrorNotSupported otherwise
+static cudaError_t density_tma(sldg_ctx* c, const double* f, double* rho)
+{
+    const long long X = c->X, V = c->V;
+    const size_t es = c->esize;
+    if (!c->opt_rho_tma || ((X * (long long)es) & 15) || (((uintptr_t)f) & 15) || X < RHO_WX || V < 4 * RHO_ROWS) return cudaErrorNotSupported;
+    if (X >= (1LL << 31) || V >= (1LL << 31)) return cudaErrorNotSupported;
+    SldgEncodeTiled enc = sldg_encode_tiled();
+    if (!enc) return cudaErrorNotSupported;
+    RhoTmaParams P;
+    P.Wv = c->Wv; P.part = c->part; P.X = X; P.V = V;
+    P.ntiles = (int)((X + RHO_WX - 1) / RHO_WX);
+    // chunks of whole boxes: about 20 waves of blocks (two are resident per SM), so that the last, partial wave does not show
+    // (measured on cfg4: 1000 blocks = 3.4 waves ran 8 % slower than the plain-load kernel); no more than the partial-sum buffer holds
+    long long nchunk = ((long long)c->sm_count * 40 + P.ntiles - 1) / P.ntiles;
+    const long long nbox = (V + RHO_ROWS - 1) / RHO_ROWS;
+    if (nchunk > nbox / 4) nchunk = nbox / 4;
+    if (nchunk > c->part_cap / X) nchunk = c->part_cap / X;
+    if (nchunk < 1) nchunk = 1;
+    long long bpc = (nbox + nchunk - 1) / nchunk;                       // boxes per chunk
+    P.vchunk = bpc * RHO_ROWS;
+    nchunk = (V + P.vchunk - 1) / P.vchunk;
+    if ((long long)P.ntiles * nchunk < 2LL * c->sm_count) return cudaErrorNotSupported;
+    P.slot_bytes = (uint32_t)(RHO_ROWS * RHO_WX * es);
+    P.slots = 6;
+    const size_t smem = (size_t)P.slots * P.slot_bytes + 16 * (size_t)P.slots + 64;
+    CUtensorMap tm;
+    const cuuint64_t gdim[2] = {(cuuint64_t)X, (cuuint64_t)V};
+    const cuuint64_t gstr[1] = {(cuuint64_t)X * es};
+    const cuuint32_t box[2] = {(cuuint32_t)RHO_WX, (cuuint32_t)RHO_ROWS};
+    const cuuint32_t estr[2] = {1u, 1u};
+    if (enc(&tm, es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<double*>(f), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorNotSupported;
+    const unsigned grid = (unsigned)((long long)P.ntiles * nchunk);
+    cudaError_t e;
+    if (es == 8) {
+        e = cudaFuncSetAttribute(rho_tma_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        rho_tma_kernel<double><<<grid, RHO_WARPS * 32, smem, c->stream>>>(tm, P);
+    } else {
+        e = cudaFuncSetAttribute(rho_tma_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        rho_tma_kernel<float><<<grid, RHO_WARPS * 32, smem, c->stream>>>(tm, P);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    rho_final_kernel<<<(unsigned)((X + 255) / 256), 256, 0, c->stream>>>(c->part, X, (int)nchunk, rho);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+
 cudaError_t sldg_launch_density(sldg_ctx* c, const double* f, double* rho)
 {
+    {
+        const cudaError_t et = density_tma(c, f, rho);
+        if (et != cudaErrorNotSupported) return et;
+    }
     const long long X = c->X, V = c->V;
     const bool f32 = c->prec == SLDG_F32;
     int vec = ((X & 1) == 0 && (((uintptr_t)f) & (f32 ? 7 : 15)) == 0) ? 2 : 1;

@@ -174,6 +174,7 @@ struct sldg_ctx {
     int opt_fv3_strip;              // fused v_1v_2v_3 kernel: v_2 donor pairs per strip (0 = auto: 4)
     int opt_fv3_slots;              // fused v_1v_2v_3 kernel: ring slots (0 = as many as shared memory holds)
     int opt_poisson_small;          // 1: x grids of up to 1024 nodes are solved by one single-block launch (FFT route)
+    int opt_rho_tma;                // 1: large problems read f through TMA tensor copies (rho_tma_kernel), 0: plain loads only
     int opt_rho_vec;                // 0 = auto (2 when aligned), 1
     int opt_rho_blocks;             // rho kernel: 128-thread blocks per SM to aim for
 };

