@@ -1,0 +1,35 @@
+"""The measurement contract on a GPU: `bench.py` on the small config prints ONE JSON line that carries the keys the driver reads
+(metric / value / ms_per_step / dtype / config.workload / clocks / e2e / gpu_launches) plus the roofline block, the physical
+traffic figures and the per-launch-kind table; the figures must be consistent with each other."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_bench_line_on_the_small_config():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "0", "--steps", "5", "--warmup", "3",
+                          "--no-all-configs", "--no-cpu-baseline"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "dtype", "data",
+                "config", "clocks", "e2e", "gpu_launches", "roofline", "physical_bytes_per_step", "physical_frac", "kernels", "parts"):
+        assert key in d, key
+    assert d["config"]["workload"] == "cfg1_4d_landau_8x16_k1" and d["dtype"] == "f64" and d["n_gpus"] == 1 and d["steps"] == 5
+    assert d["gpu_launches"] > 0 and d["ms_per_step"] > 0 and d["value"] > 0
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    # physical traffic = sweep launches x 2|f|8 B + rho launches x |f|8 B, per step
+    nf8 = d["config"]["bytes_f"]
+    n_pass = sum(v["launches"] for k, v in d["kernels"].items() if k.startswith("sweep"))
+    n_rho = d["kernels"]["rho"]["launches"]
+    assert abs(d["physical_bytes_per_step"] - (2 * nf8 * n_pass + nf8 * n_rho) / d["steps"]) < 1.0
+    e = d["e2e"]
+    assert e["h2d_bytes_per_step"] == nf8 and e["d2h_bytes_per_step"] == nf8 and e["value"] > 0
