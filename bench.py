@@ -224,6 +224,9 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
     fill_initial(W, g, cfg, f, args.dtype, dev)
     if args.poisson == "cg":
         g.set_poisson_solver(1, tol=1e-3)
+    for kv in args.option or []:              # tuning knobs of sldg_set_option (speed only, never results): name=value
+        name, val = kv.split("=")
+        g.set_option(name, int(val))
     dt = cfg["dt"]
     nf = W.field_elems(cfg)
     nsweeps = sweeps_per_step(cfg)
@@ -445,6 +448,8 @@ def main():
                     "route (default) or the CGdG solver with the paper's tolerance 1e-3 and warm start (PAPER.md:496-567)")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="f32: single precision mode (PAPER.md:191); "
                     "the metric then counts 2*|f|*4 B per sweep")
+    ap.add_argument("--option", action="append", default=None, help="a tuning knob of sldg_set_option as name=value (repeatable), "
+                    "e.g. --option x_double=2 (profiles/ uses this to capture kernels the default plan does not launch)")
     ap.add_argument("--cells", type=str, default=None, help="override cells, e.g. 16,16,16,16 (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
