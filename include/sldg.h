@@ -47,6 +47,7 @@ extern "C" {
 #define SLDG_ENOMEM (-2)        /* host or small device allocation failed                  */
 #define SLDG_ECUDA (-3)         /* a CUDA runtime call failed; see sldg_last_cuda_error    */
 #define SLDG_ENOWORKSPACE (-4)  /* sldg_set_workspace not called or too small              */
+#define SLDG_ETOOLARGE (-5)     /* sldg_density_static: x grid larger than its fixed scratch */
 
 #define SLDG_MAX_DIM 6
 #define SLDG_MAX_DEGREE 4
@@ -225,6 +226,47 @@ int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int prec
  * Runs one untimed and `reps` timed launches; *ms_out (host) = elapsed ms of the timed ones.  Synchronises. */
 int sldg_probe_load_rate(sldg_ctx* ctx, const double* src, long long X, long long R, int mode, int wx, int rows,
                          int depth, int threads, int chunks_per_block, int reps, double* ms_out);
+
+/* ---- rho for callers that cannot allocate device memory -----------------------------------
+ * Same operation as sldg_density (a3): rho[x] = sum_v Wv[v] f[v][x], f seen as a row-major [V][X]
+ * array (x contiguous: exactly the layout above with X = prod of the x extents, V = prod of the v extents).
+ *
+ * Why it exists.  sldg_density needs a context (sldg_create calls cudaMalloc for its small tables) and a workspace
+ * for the partial sums of its two-stage reduction.  Not every caller can provide those where rho is needed: a host
+ * application that has already given all of HBM to its own memory pool (a new cudaMalloc fails, or makes the pool
+ * shrink); a loop that shares the GPU with other streams and cannot afford the device-wide synchronisation that
+ * cudaMalloc/cudaFree imply; a plug-in that receives pointers and a stream from its host and is not allowed to own
+ * device memory.  This call needs NO context and NO workspace and never calls cudaMalloc, cudaFree or any allocating
+ * routine: its partial sums live in a fixed 8 MiB array inside the library image.  That array occupies 8 MiB on every
+ * GPU onto which the library's device code is loaded, until the process exits.
+ *
+ *   f          device, [V][X] values, double (precision SLDG_F64) or float (SLDG_F32); 16-byte alignment (8 for
+ *              float) and even X select the 2-wide loads, anything else still works
+ *   Wv         device, [V] doubles: the velocity quadrature weight of row v, prod_d h_{v_d} w_{j_d} with v_1 fastest
+ *              (w from sldg_gauss_legendre; the caller builds and uploads it once, at a time when it may allocate)
+ *   rho        device, [X] doubles, written completely; must not alias f or Wv
+ *   stream     a cudaStream_t as void*, NULL = legacy default stream; the call enqueues two kernels and returns
+ *   cuda_error_host  host, may be NULL: receives the cudaError_t when SLDG_ECUDA is returned, 0 otherwise
+ * All pointers must belong to the device that is current in the calling thread.
+ *
+ * LIMIT.  X <= SLDG_DENSITY_STATIC_MAX_X (= sldg_density_static_max_x(), 1 048 576 x nodes; the largest BASELINE config
+ * has 110 592).  A larger X returns SLDG_ETOOLARGE before anything is enqueued; V is not limited by the scratch.
+ * Other errors: SLDG_EINVAL (NULL pointer, X or V < 1, unknown precision), SLDG_ECUDA.
+ *
+ * FIRST CALL PER DEVICE.  The first call on each device looks up the device address of the fixed array
+ * (cudaGetSymbolAddress) and the SM count, under a lock, and keeps them.  Make that first call during start-up,
+ * before any stream capture begins on that device; later calls only launch.
+ *
+ * SHARED STATE.  Every call in the process on the same device uses the same array.  Calls enqueued on one stream run
+ * one after the other and are safe.  Two calls that can overlap on the GPU (different streams without an event
+ * between them, or two host threads on different streams) overwrite each other's partial sums: ordering them is the
+ * caller's job.  The array keeps whatever the last call left in it; that is harmless, because stage one rewrites every
+ * partial sum that stage two reads, so nothing has to start at zero.  Results are bitwise reproducible from call to
+ * call on the same device; they agree with sldg_density to rounding (the chunking of the v sum differs). */
+#define SLDG_DENSITY_STATIC_MAX_X (1 << 20)
+int sldg_density_static(const void* f, const double* Wv, long long X, long long V, int precision, double* rho,
+                        void* stream, int* cuda_error_host);
+long long sldg_density_static_max_x(void);
 
 /* Tuning knob (affects speed only, never results): see DESIGN.md section 5.  A fused pass whose launcher declines
  * a shape that the planner accepted is replaced by the separate sweeps (plus one device copy when the buffer

@@ -58,6 +58,8 @@ EXPORTS = {
     "sldg_cg_info": (C.c_int, [_vp, _ip, _dp]),
     "sldg_last_phi": (_vp, [_vp]),
     "sldg_sipg_matrices": (C.c_int, [C.c_int, C.c_double, _dp, _dp]),
+    "sldg_density_static": (C.c_int, [_vp, _vp, _ll, _ll, C.c_int, _vp, _vp, _ip]),
+    "sldg_density_static_max_x": (_ll, []),
     "sldg_plan_query": (C.c_int, [C.c_int, C.c_int, _ip, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                   C.POINTER(C.c_longlong)]),
 }
@@ -137,6 +139,36 @@ def gauss_legendre(degree):
     xi, w = np.empty(degree + 1), np.empty(degree + 1)
     _check(lib().sldg_gauss_legendre(int(degree), xi.ctypes.data_as(_dp), w.ctypes.data_as(_dp)))
     return xi, w
+
+
+def density_static_max_x():
+    return int(lib().sldg_density_static_max_x())
+
+
+def density_static(f, Wv, rho=None, stream=None):
+    """sldg_density_static: rho[x] = sum_v Wv[v] f[v, x] without a context, a workspace or any device allocation inside the
+    library (for callers that cannot allocate; the partial sums use a fixed 8 MiB array inside the library, so X is limited to
+    density_static_max_x() and calls that overlap on the GPU must be ordered by the caller).  f: contiguous CUDA tensor, float64
+    or float32, whose leading dimensions are the v axes and whose trailing dimensions are the x axes; Wv: float64 CUDA tensor
+    with one weight per v row (its size fixes V, X = f.numel() / V).  Passing rho avoids the one torch allocation made here."""
+    import torch
+    assert f.is_cuda and f.is_contiguous() and f.dtype in (torch.float64, torch.float32)
+    assert Wv.is_cuda and Wv.is_contiguous() and Wv.dtype == torch.float64
+    V = Wv.numel()
+    assert V > 0 and f.numel() % V == 0
+    X = f.numel() // V
+    if rho is None:
+        rho = torch.empty(X, dtype=torch.float64, device=f.device)
+    assert rho.is_cuda and rho.is_contiguous() and rho.dtype == torch.float64 and rho.numel() == X
+    st = stream if stream is not None else torch.cuda.current_stream(f.device)
+    err = C.c_int(0)
+    with torch.cuda.device(f.device):
+        code = lib().sldg_density_static(C.c_void_p(f.data_ptr()), C.c_void_p(Wv.data_ptr()), X, V,
+                                         1 if f.dtype == torch.float32 else 0, C.c_void_p(rho.data_ptr()),
+                                         C.c_void_p(st.cuda_stream), C.byref(err))
+    if code != 0:
+        raise SldgError(f"sldg error {code}: {lib().sldg_strerror(code).decode()}" + (f" [cudaError {err.value}]" if code == -3 else ""))
+    return rho
 
 
 class Sldg:

@@ -1241,6 +1241,7 @@ extern "C" const char* sldg_strerror(int code)
     case SLDG_ENOMEM: return "out of memory";
     case SLDG_ECUDA: return "CUDA runtime error (see sldg_last_cuda_error); no CPU fallback exists";
     case SLDG_ENOWORKSPACE: return "workspace missing or too small";
+    case SLDG_ETOOLARGE: return "x grid exceeds SLDG_DENSITY_STATIC_MAX_X nodes: sldg_density_static has a fixed scratch array; use sldg_density";
     }
     return "unknown error";
 }
