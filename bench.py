@@ -280,7 +280,8 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
     passes = {k: v for k, v in kinds.items() if k.startswith(SWEEP_KINDS_PREFIX) and v[0]}
     n_pass = sum(n for n, _ in passes.values())
     n_rho = kinds.get("rho", (0, 0.0))[0]
-    phys_step = (n_pass * pass_bytes + n_rho * nf * ESIZE) / steps
+    n_copy = kinds.get("copies", (0, 0.0))[0]     # whole-array device copies of f (fallback plans only): |f| read + |f| written each
+    phys_step = ((n_pass + n_copy) * pass_bytes + n_rho * nf * ESIZE) / steps
     kernels = {}
     for k, (n, ms) in passes.items():
         gbs = pass_bytes / (ms / n * 1e-3) / 1e9
@@ -291,6 +292,11 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
         gbs = nf * ESIZE / (ms / n * 1e-3) / 1e9
         kernels["rho"] = {"launches": n, "avg_ms": ms / n, "physical_gbs": gbs, "frac_of_measured_peak": gbs / peak,
                           "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS, "bytes_per_launch": nf * ESIZE}
+    if n_copy:
+        n, ms = kinds["copies"]
+        gbs = pass_bytes / (ms / n * 1e-3) / 1e9
+        kernels["copies"] = {"launches": n, "avg_ms": ms / n, "physical_gbs": gbs, "frac_of_measured_peak": gbs / peak,
+                             "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS, "bytes_per_launch": pass_bytes}
     # EFFECTIVE per-axis figures (BASELINE.json's metric: 2*|f|*8 B per 1-D sweep / time): a fused or merged launch books
     # an equal share of its time on each sweep it performs, so these exceed the HBM peak by the fusion factor
     sweeps = {}
@@ -310,6 +316,17 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
                 "launches": kl, "avg_ms": kms / kl,
                 "timed_by": "CUDA events around every launch, K steps run right after the timed region",
                 "share_of_step": kms / sum(v[1] for v in kinds.values())}
+    # the kernel FURTHEST below the roofline among the launch kinds that move f (>= 2 % of the step), and every kind's fraction
+    total_ms = sum(v[1] for v in kinds.values())
+    big = {k: v for k, v in kernels.items() if v["avg_ms"] * v["launches"] >= 0.02 * total_ms} or kernels
+    wk = min(big, key=lambda k: big[k]["frac_of_measured_peak"])
+    roofline["worst"] = {"kernel": wk, "frac": kernels[wk]["frac_of_measured_peak"], "avg_ms": kernels[wk]["avg_ms"],
+                         "launches": kernels[wk]["launches"], "achieved": kernels[wk]["physical_gbs"],
+                         "share_of_step": kernels[wk]["avg_ms"] * kernels[wk]["launches"] / total_ms}
+    roofline["parts_frac"] = {k: round(v["frac_of_measured_peak"], 4) for k, v in kernels.items()}
+    roofline["parts_ms_per_step"] = {k: round(v["avg_ms"] * v["launches"] / steps, 4) for k, v in kernels.items()}
+    roofline["peak_is"] = ("device-to-device copy rate (read + write): kernels that mostly read, or stream with TMA, "
+                           "can exceed it (frac up to ~1.08 measured)")
     parts = {k: {"launches": n, "ms_per_step": ms / steps} for k, (n, ms) in kinds.items() if n}
     res = {"workload": cfg["name"], "values": nf, "bytes_f": nf * ESIZE, "ms_per_step": ms_step,
            "single_step_ms": ms_single_calls,
@@ -323,6 +340,7 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
 
 
 def run_ours(args, cfg, rank, world, local):
+    global ESIZE
     import torch
     import workloads as W
 
@@ -414,7 +432,7 @@ def run_ours(args, cfg, rank, world, local):
                                       "physical_bytes_per_step": r["physical_bytes_per_step"],
                                       "physical_gbs": r["physical_gbs"], "physical_frac": r["physical_frac"],
                                       "roofline": {"kernel": rf["kernel"], "frac": rf["frac"], "avg_ms": rf["avg_ms"],
-                                                   "achieved": rf["achieved"]},
+                                                   "achieved": rf["achieved"], "worst": rf["worst"]},
                                       "kernels": {k: {"avg_ms": v["avg_ms"], "frac_of_measured_peak": v["frac_of_measured_peak"],
                                                       "launches": v["launches"]} for k, v in r["kernels"].items()},
                                       "clocks": r["clocks"], "steps": r["steps"],
@@ -422,6 +440,48 @@ def run_ours(args, cfg, rank, world, local):
             except Exception as ex:
                 others[oc["name"]] = {"error": str(ex)[:200]}
         line["configs"] = others
+        # NEXT rows, driver-measured: the paper's default order (k = 3) on the two bump-on-tail workloads, and the
+        # headline config in single precision (Tables 3-4)
+        import argparse as _ap
+        nxt = {c["name"]: c for c in W.NEXT_CONFIGS}
+        legs = [("bot_6d_k3_9", nxt.get("bot_6d_k3_9"), "f64"), ("bot_5d_k3_16", nxt.get("bot_5d_k3_16"), "f64"),
+                (cfg["name"] + "_f32", cfg, "f32")]
+        f32 = {}
+        for name, oc, prec in legs:
+            if oc is None or args.dtype != "f64":
+                continue
+            a2 = _ap.Namespace(**vars(args))
+            a2.dtype = prec
+            es0, ESIZE = ESIZE, (4 if prec == "f32" else 8)
+            try:
+                r, _, _, g2, f2 = measure_config(a2, oc, dev, local, min(args.steps, 10), 3, False)
+                g2.close()
+                del g2, f2
+                torch.cuda.empty_cache()
+                blk = {"ms_per_step": r["ms_per_step"], "single_step_ms": r["single_step_ms"], "dtype": prec,
+                       "passes_per_step": r["passes_per_step"], "physical_gbs": r["physical_gbs"],
+                       "physical_frac": r["physical_frac"], "effective_gbs_per_sweep": r["effective_gbs_per_sweep"],
+                       "worst": r["roofline"]["worst"], "parts_frac": r["roofline"]["parts_frac"],
+                       "parts_ms_per_step": r["roofline"]["parts_ms_per_step"], "steps": r["steps"]}
+            except Exception as ex:
+                blk = {"error": str(ex)[:200]}
+            finally:
+                ESIZE = es0
+            if prec == "f32":
+                f32[name] = blk
+            else:
+                others[name] = blk
+        if f32:
+            line["f32"] = f32
+        # one compact row per config INSIDE the roofline block (the driver's record keeps that block whole):
+        # [ms_per_step, passes_per_step, physical_frac, worst kernel, its frac]
+        def row(r):
+            w = r.get("worst") or (r.get("roofline") or {}).get("worst") or {}
+            return [round(r["ms_per_step"], 4), r["passes_per_step"], round(r["physical_frac"], 4), w.get("kernel"),
+                    round(w.get("frac", 0.0), 4)] if "ms_per_step" in r else [r.get("error")]
+        line["roofline"]["by_config"] = {n: row(r) for n, r in list(others.items()) + list(f32.items())}
+        line["roofline"]["by_config_columns"] = "ms_per_step, passes_per_step, physical_frac, worst kernel, worst frac"
+        line["roofline"]["previous_round_headline"] = "cfg5_6d_twostream_24x20_k1 (round 2: 72.29 ms; round 1 headline was cfg2)"
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         r = time_oracle(cfg, steps=1000, warmup=1, budget_s=12.0)

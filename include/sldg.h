@@ -54,6 +54,13 @@ extern "C" {
 
 typedef struct sldg_ctx sldg_ctx;
 
+/* ABI version.  Bumped whenever the signature of an existing symbol changes (round 2 inserted `fuse_v3` in the middle of
+ * sldg_plan_query's argument list: a caller built against the older header passes x_double in its place without any
+ * diagnostic).  From version 3 on, new parameters are only ever appended or the symbol gets a new name; a C caller should
+ * compare sldg_abi_version() with the SLDG_ABI_VERSION it was compiled against before its first call. */
+#define SLDG_ABI_VERSION 3
+int sldg_abi_version(void);
+
 /* ---- lifetime --------------------------------------------------------------------------
  * sldg_create: problem statement of P:50-58.  dim_x in 1..3, dim_x <= dim_v <= 3 (the paper
  * uses 2x2v, 2x3v, 3x3v; 1x1v and 1x2v are accepted as cheap test vehicles).
@@ -192,14 +199,16 @@ int sldg_advect_axis(sldg_ctx* ctx, double* f, int axis, const double* delta_hos
 /* ---- instrumentation --------------------------------------------------------------------
  * With timing on, every kernel launch is bracketed by CUDA events on the context's stream.
  * Kinds: 0 = sweep along axis 0 (TMA/SMEM kernel), 1 = sweep along a slow axis, 2 = rho,
- * 3 = Poisson/E, 4 = shift tables, 5 = copies, 6 = fused x pass (x_1+x_2, or x_1+x_2+x_3 for dim_x = 3, in one
+ * 3 = Poisson/E, 4 = shift tables (device-side v-table kernel), 5 = whole-array device copies of f (|f| read + |f| written
+ * each; only fallback plans make any), 6 = fused x pass (x_1+x_2, or x_1+x_2+x_3 for dim_x = 3, in one
  * launch), 7 = fused v_1+v_2 pass (one launch), 8 = double x half step (x_1+x_2 applied twice in one launch, inside
  * sldg_steps), 9 = fused v_1+v_2+v_3 pass (one launch, dim_x = 3), 10 = double x half step for dim_x = 3
- * (x_1+x_2+x_3 applied twice in one launch, inside sldg_steps); the per-axis figures of sldg_timing_axis book an equal share of a
+ * (x_1+x_2+x_3 applied twice in one launch, inside sldg_steps), 11 = host-to-device uploads of rebuilt x-sweep shift tables
+ * (O(D) bytes; until ABI version 2 these were booked under kind 5); the per-axis figures of sldg_timing_axis book an equal share of a
  * fused launch's time on each of its axes.  sldg_timing_read synchronises, adds the elapsed
  * times of all events recorded since the last read, and returns per kind the number of launches
  * and the total milliseconds (arrays of SLDG_NKINDS entries, host). */
-#define SLDG_NKINDS 11
+#define SLDG_NKINDS 12
 int sldg_timing_enable(sldg_ctx* ctx, int on);
 /* SLDG_ECUDA (and no figures) if an event could not be created since the last read: launches went unrecorded. */
 int sldg_timing_read(sldg_ctx* ctx, long long* launches, double* ms);
@@ -217,15 +226,6 @@ int sldg_timing_axis(const sldg_ctx* ctx, long long* launches, double* ms);
  * by sldg_launch_count.  A fused or merged launch is ONE pass.  Returns 0 or a negative code. */
 int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
                     int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts);
-
-/* Diagnostic (no part of the hot path): the rate at which the SMs can pull the strided row tiles the fused v passes
- * gather -- pieces [rows][wx] of a row-major [R][X] fp64 device array `src` -- with no arithmetic and no stores.
- * mode 0: 2-d TMA tensor copies into a ring of `depth` shared-memory slots; mode 1: 1-d TMA bulk copies, one per
- * row piece; mode 2: plain 128-bit global loads by all threads (depth 2 or 4 boxes in flight per thread).
- * `threads` per block (multiple of 32, <= 256), every block handles `chunks_per_block` consecutive boxes of one x tile.
- * Runs one untimed and `reps` timed launches; *ms_out (host) = elapsed ms of the timed ones.  Synchronises. */
-int sldg_probe_load_rate(sldg_ctx* ctx, const double* src, long long X, long long R, int mode, int wx, int rows,
-                         int depth, int threads, int chunks_per_block, int reps, double* ms_out);
 
 /* ---- rho for callers that cannot allocate device memory -----------------------------------
  * Same operation as sldg_density (a3): rho[x] = sum_v Wv[v] f[v][x], f seen as a row-major [V][X]

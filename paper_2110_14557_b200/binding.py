@@ -9,15 +9,17 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = "libsldg_b200.so"
 
-NKINDS = 11
+NKINDS = 12
+ABI_VERSION = 3          # SLDG_ABI_VERSION of the include/sldg.h these argument lists were written against
 MAX_DIM = 6
-KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x", "sweep_fused_v", "sweep_fused_x_double", "sweep_fused_v3", "sweep_fused_x3_double"]
+KIND_NAMES = ["sweep_axis0_tma", "sweep_slow_axis", "rho", "poisson", "shift_tables", "copies", "sweep_fused_x", "sweep_fused_v", "sweep_fused_x_double", "sweep_fused_v3", "sweep_fused_x3_double", "table_uploads"]
 
 _vp, _dp, _ip, _ll = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_longlong
 _llp = C.POINTER(C.c_longlong)
 
 # name -> (restype, argtypes); every symbol include/sldg.h declares
 EXPORTS = {
+    "sldg_abi_version": (C.c_int, []),
     "sldg_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, _ip, C.c_int, _dp]),
     "sldg_create_prec": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, _ip, C.c_int, _dp, C.c_int]),
     "sldg_precision": (C.c_int, [_vp]),
@@ -51,7 +53,6 @@ EXPORTS = {
     "sldg_launch_count": (_ll, [_vp]),
     "sldg_timing_axis": (C.c_int, [_vp, _llp, _dp]),
     "sldg_set_option": (C.c_int, [_vp, C.c_char_p, _ll]),
-    "sldg_probe_load_rate": (C.c_int, [_vp, _vp, _ll, _ll, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _dp]),
     "sldg_poisson_cg": (C.c_int, [_vp, _vp, _vp, C.c_double, C.c_int]),
     "sldg_set_poisson_solver": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, C.c_double]),
     "sldg_cg_reset": (C.c_int, [_vp]),
@@ -87,6 +88,8 @@ def lib():
         for name, (res, args) in EXPORTS.items():
             fn = getattr(L, name)
             fn.restype, fn.argtypes = res, args
+        if L.sldg_abi_version() != ABI_VERSION:
+            raise SldgError(f"{path} has ABI version {L.sldg_abi_version()}, this binding was written for {ABI_VERSION}: rebuild")
         _lib = L
     return _lib
 
@@ -344,14 +347,6 @@ class Sldg:
 
     def launch_count(self):
         return int(lib().sldg_launch_count(self._h))
-
-    def probe_load_rate(self, src, X, R, mode, wx, rows, depth, threads, chunks_per_block, reps=3):
-        """sldg_probe_load_rate -> GB/s of the timed launches (bytes = the boxes' bytes)"""
-        ms = C.c_double()
-        _check(lib().sldg_probe_load_rate(self._h, _ptr(src), int(X), int(R), int(mode), int(wx), int(rows), int(depth),
-                                          int(threads), int(chunks_per_block), int(reps), C.byref(ms)), self._h)
-        nbytes = (X // wx) * wx * (R // rows) * rows * 8
-        return reps * nbytes / (ms.value * 1e-3) / 1e9
 
     def set_option(self, name, value):
         _check(lib().sldg_set_option(self._h, name.encode(), int(value)))

@@ -11,7 +11,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsldg_b200.so")
-SOURCES = ["sldg_api.cu", "sldg_sweep_walk.cu", "sldg_sweep_tma.cu", "sldg_sweep_line.cu", "sldg_sweep_fused.cu", "sldg_sweep_fused_cell.cu", "sldg_sweep_fused3.cu", "sldg_sweep_fused3d.cu", "sldg_sweep_fusedv.cu", "sldg_sweep_fusedv3.cu", "sldg_field.cu", "sldg_density_static.cu", "sldg_probe.cu", "sldg_cgdg.cu", "sldg_tables.cpp"]
+SOURCES = ["sldg_api.cu", "sldg_sweep_walk.cu", "sldg_sweep_tma.cu", "sldg_sweep_line.cu", "sldg_sweep_fused.cu", "sldg_sweep_fused_cell.cu", "sldg_sweep_fused3.cu", "sldg_sweep_fused3d.cu", "sldg_sweep_fusedv.cu", "sldg_sweep_fusedv3.cu", "sldg_field.cu", "sldg_density_static.cu", "sldg_cgdg.cu", "sldg_tables.cpp"]
 DUAL = ["sldg_sweep_walk.cu", "sldg_sweep_line.cu", "sldg_sweep_fused_cell.cu", "sldg_sweep_fused3.cu", "sldg_sweep_fused3d.cu", "sldg_sweep_fusedv.cu", "sldg_sweep_fusedv3.cu"]
 HEADERS = [os.path.join(CSRC, "sldg_real.h"), os.path.join(CSRC, "sldg_internal.h"), os.path.join(CSRC, "sldg_async.h"), os.path.join(CSRC, "sldg_tmap.h"), os.path.join(HERE, "..", "include", "sldg.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

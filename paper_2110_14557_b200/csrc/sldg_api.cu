@@ -337,7 +337,7 @@ static int upload_table(sldg_ctx* c, const double* delta, long long n, int N, in
         for (size_t i = 0; i < h4.size(); i++) h4[i] = (float)c->hAB[i];
         memcpy(c->hAB, h4.data(), h4.size() * 4);
     }
-    sldg_ev_begin(c, KIND_COPY, -1);
+    sldg_ev_begin(c, KIND_UPLOAD, -1);
     CK(cudaMemcpyAsync(dS, c->hS, (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(dAB, c->hAB, (size_t)n * NN2 * c->esize, cudaMemcpyHostToDevice, c->stream));
     sldg_ev_end(c);
@@ -1233,6 +1233,7 @@ extern "C" int sldg_mass(sldg_ctx* c, const double* f, double* host_out)
     if (!c->ws_ready) return SLDG_ENOWORKSPACE;
     return scalar_out(c, sldg_launch_mass(c, f, c->dScalar), host_out);
 }
+extern "C" int sldg_abi_version(void) { return SLDG_ABI_VERSION; }
 extern "C" const char* sldg_strerror(int code)
 {
     switch (code) {

@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(128) rho_partial_kernel(const T* __restrict__ 
 }
 
 // rho by TMA (large problems): f seen as [V][X]; a block owns a tile of 32 x values and a chunk of v rows and streams boxes
-// of 32 x RHO_ROWS values (2-d tensor copies into a full/empty mbarrier ring; tests/test_gpu_probe.py: this path streams at
+// of 32 x RHO_ROWS values (2-d tensor copies into a full/empty mbarrier ring; profiles/r2_probe_load_rate.md: this path streams at
 // 1.05-1.1 of the device-copy rate, the plain-load kernel above at 0.95).  Lane = two x values, warp w sums rows w, w + 8, ... of
 // every box in ascending v with fma(W_v, f, acc); the eight warps' sums are added in warp order: deterministic.
 constexpr int RHO_WX = 64, RHO_ROWS = 32, RHO_WARPS = 8;     // lane = TWO x values (one 16-byte / 8-byte load per row)

@@ -18,7 +18,7 @@
 #define SLDG_COPY_BIT (1 << 30)
 #define SLDG_S_MASK (SLDG_COPY_BIT - 1)
 
-enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5, KIND_FUSED = 6, KIND_FUSEDV = 7, KIND_FUSEDX2 = 8, KIND_FUSEDV3 = 9, KIND_FUSEDX3D = 10 };
+enum { KIND_SWEEP0 = 0, KIND_SWEEP = 1, KIND_RHO = 2, KIND_POISSON = 3, KIND_TABLE = 4, KIND_COPY = 5, KIND_FUSED = 6, KIND_FUSEDV = 7, KIND_FUSEDX2 = 8, KIND_FUSEDV3 = 9, KIND_FUSEDX3D = 10, KIND_UPLOAD = 11 };
 
 // Polynomial coefficients of A_jl(alpha), B_jl(alpha) in powers of (alpha - 1/2), ascending, row-major
 // [2][K1*K1][SLDG_MAXPOLY]; the fp64 copy is uploaded per context (dPoly) for the device-side table kernel.

@@ -347,8 +347,11 @@ bool shape(const sldg_ctx* c, FV3Shape* o)
     auto smem_of = [&](int st) { return (size_t)st * slot_bytes + 16 * (size_t)st + (size_t)wx * (4 * K1 * K1 + 2) * sizeof(real) + 128; };
     // ring depth: measured on B200 (cfg4, 20 KB boxes) 6 slots beat the 11 that fit by 4-10 % (the deeper ring lets the
     // strips of an x tile drift apart, and their shared halo cells stop hitting in L2)
+    // An explicit option value is honoured down to 2 slots (LAG = 1 in the kernel: tests/test_gpu_fusedv3.py runs 2 and 3);
+    // the 4-slot floor applies to the automatic choice only.
     int slots = c->opt_fv3_slots > 0 ? c->opt_fv3_slots : (int)((120 * 1024) / slot_bytes);
-    if (slots < 4) slots = 4;
+    if (c->opt_fv3_slots <= 0 && slots < 4) slots = 4;
+    if (slots < 2) slots = 2;
     while (slots > 2 && smem_of(slots) > 227 * 1024) slots--;
     if (smem_of(slots) > 227 * 1024) return false;
     if (o) { o->wx = wx; o->threads = (int)(((long long)wx * N1 + 31) / 32 * 32); o->S = S; o->nstrips = nstrips;

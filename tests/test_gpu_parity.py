@@ -549,17 +549,17 @@ def test_x_table_cache_holds_two_time_increments(P):
     g.timing_enable(True); g.timing_read()
     g.advect_x(f, 0.1); g.advect_x(f, 0.05)
     kinds, _ = g.timing_read()
-    assert kinds["copies"][0] == 2 * 2                       # two increments x two axes, one upload event each
+    assert kinds["table_uploads"][0] == 2 * 2                       # two increments x two axes, one upload event each
     for _ in range(3):
         g.advect_x(f, 0.1); g.advect_x(f, 0.05)
     kinds, _ = g.timing_read()
-    assert kinds["copies"][0] == 0                           # cached: no upload, no synchronisation
+    assert kinds["table_uploads"][0] == 0                           # cached: no upload, no synchronisation
     g.advect_x(f, 0.2); g.advect_x(f, 0.05); g.advect_x(f, 0.2)
     kinds, _ = g.timing_read()
-    assert kinds["copies"][0] == 2                           # 0.2 evicted 0.1 (least recently used); 0.05 stayed
+    assert kinds["table_uploads"][0] == 2                           # 0.2 evicted 0.1 (least recently used); 0.05 stayed
     g.advect_x(f, 0.1)
     kinds, _ = g.timing_read()
-    assert kinds["copies"][0] == 2
+    assert kinds["table_uploads"][0] == 2
     g.timing_enable(False)
 
 
@@ -651,4 +651,5 @@ def test_density_through_tensor_copies_matches_plain_loads_and_the_oracle(P, geo
     assert np.array_equal(outs[0], outs[2])                              # deterministic
     for name, r in (("tensor copies", outs[0]), ("plain loads", outs[1])):
         assert parity_report.add("density, " + name, "x".join(map(str, cells)) + f" k={k}", "rho", r, want, TOL_SWEEP, prec) <= TOL_SWEEP
-    assert not np.array_equal(outs[0], outs[1]) or prec == "f32" or True   # (the summation orders differ; equality is allowed)
+    # the two kernels chunk the v sum differently: they may differ, but only by the rounding of two fp64 sums of <= 1024 terms
+    assert rel_inf(outs[0], outs[1]) <= 1e-14

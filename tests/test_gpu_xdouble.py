@@ -187,7 +187,8 @@ def test_plan_query_counts_are_those_of_the_real_calls(P, geom, n, fuse_v, x_dou
     sweeps = sum(v[0] for name, v in kinds.items() if name.startswith("sweep"))
     assert sweeps == want["x_passes"] + want["v_passes"]
     assert kinds["sweep_fused_v"][0] + kinds["sweep_slow_axis"][0] >= want["v_passes"]
-    assert kinds["copies"][0] == dx                                # only the x shift-table uploads (one event per axis)
+    assert kinds["table_uploads"][0] == dx                         # the x shift-table uploads (one event per axis)
+    assert kinds["copies"][0] == want["copies"] == 0               # and no whole-array copy of f
     assert kinds["rho"][0] == max(1, n)
 
 

@@ -238,7 +238,7 @@ def test_p12_linear_landau_damping_rate():
     slope = np.polyfit(tp, lp, 1)[0]
     gamma = slope / 2
     omega = math.pi / np.mean(np.diff(tp))
-    assert abs(gamma - (-0.1533)) < 0.02 * 0.1533 * 2, gamma
+    assert abs(gamma - (-0.1533)) < 0.02 * 0.1533, gamma          # DESIGN.md reading M: +-2 % (measured 0.74 %)
     assert abs(omega - 1.4156) < 0.02 * 1.4156, omega
 
 
