@@ -142,7 +142,7 @@ static int create_impl(sldg_ctx** out, int dim_x, int dim_v, const int* cells, i
     c->opt_tile_bytes = 3584; c->opt_tile_stages = 2; c->opt_axis0_impl = 0; c->opt_walk_block = 128; c->opt_walk_vec = 0; c->opt_rho_vec = 0; c->opt_rho_tma = 1; c->opt_fuse_x = 1; c->opt_fused_threads = 256; c->opt_inplace_walk = 1; c->opt_rho_blocks = 8;
     c->opt_fused_impl = 0; c->opt_x_copy = 0; c->opt_fuse3 = 1; c->opt_f3_threads = 128; c->opt_f3_stages = 3; c->opt_f3d_threads = 128; c->opt_cell_threads = 64; c->opt_cell_rows = 0; c->opt_cell_bytes = 9216; c->opt_cell_stages = 2;
     c->opt_poisson_small = 1; c->opt_x_double = 1; c->opt_fuse_v = 1; c->opt_fv_wx = 0; c->opt_fv_stages = 0; c->opt_fv_inflight = 72 * 1024; c->opt_fv_ppb = 0; c->opt_fv_l2 = 2; c->opt_fv_cps = 1;
-    c->opt_decline = 0; c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0;
+    c->opt_decline = 0; c->opt_fuse_v3 = 1; c->opt_fv3_wx = 0; c->opt_fv3_strip = 0; c->opt_fv3_slots = 0; c->opt_fv3_pw = 1;
     for (int a = 0; a < SLDG_MAX_DIM; a++) { c->tab_safe[a] = false; c->tab_anycp[a] = true; c->dWx[a] = nullptr; }
     for (int a = 0; a < 3; a++) for (int i = 0; i < SLDG_XTAB_SLOTS; i++) { XTab& x = c->xtab[a][i]; x.dS = nullptr; x.dAB = nullptr; x.tau = 0.0; x.valid = x.anycp = x.safe = false; x.used = 0; }
     c->xtab_clock = 0; c->ev_failed = false;
@@ -1355,6 +1355,7 @@ extern "C" int sldg_set_option(sldg_ctx* c, const char* name, long long value)
     if (!strcmp(name, "fuse_v3")) { if (value < 0 || value > 2) return SLDG_EINVAL; c->opt_fuse_v3 = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv3_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv3_wx = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv3_strip")) { if (value < 0 || value > 5) return SLDG_EINVAL; c->opt_fv3_strip = (int)value; return SLDG_OK; }
+    if (!strcmp(name, "fv3_pw")) { if (value < 0 || value > 1) return SLDG_EINVAL; c->opt_fv3_pw = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv3_slots")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv3_slots = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_wx")) { if (value < 0 || value > 256) return SLDG_EINVAL; c->opt_fv_wx = (int)value; return SLDG_OK; }
     if (!strcmp(name, "fv_stages")) { if (value < 0 || value > 24) return SLDG_EINVAL; c->opt_fv_stages = (int)value; return SLDG_OK; }

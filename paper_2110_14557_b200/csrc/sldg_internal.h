@@ -172,6 +172,7 @@ struct sldg_ctx {
     int opt_fuse_v3;                // v_1, v_2 and v_3 sweeps in one pass (sldg_sweep_fusedv3.cu; dim_x = 3, degree <= 1): 0 never, 1 auto, 2 whenever the shape allows
     int opt_fv3_wx;                 // fused v_1v_2v_3 kernel: x nodes per tile (0 = auto)
     int opt_fv3_strip;              // fused v_1v_2v_3 kernel: v_2 donor pairs per strip (0 = auto: 4)
+    int opt_fv3_pw;                 // fused v_1v_2v_3 kernel: 1 = dedicated producer warp (an extra warp per block)
     int opt_fv3_slots;              // fused v_1v_2v_3 kernel: ring slots (0 = as many as shared memory holds)
     int opt_poisson_small;          // 1: x grids of up to 1024 nodes are solved by one single-block launch (FFT route)
     int opt_rho_tma;                // 1: large problems read f through TMA tensor copies (rho_tma_kernel), 0: plain loads only

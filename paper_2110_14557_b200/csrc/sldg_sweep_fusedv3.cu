@@ -40,6 +40,7 @@ struct FV3Params {
     real* fout;
     long long X;
     int N1, N2, N3, WX, S, nstrips, ntiles, slots;
+    int pw;                       // 1: the block's LAST warp is a dedicated producer (issues every tensor copy), the others only consume
     uint32_t slot_bytes;          // ring slot stride (>= (k+1)^2 * D_1 * WX * sizeof(real), multiple of 1024)
     ShiftTable t1, t2, t3;
 };
@@ -62,7 +63,7 @@ __device__ __forceinline__ void fv3_table(const ShiftTable& t, long long idx, re
 
 // WXT: x nodes per tile as a compile-time constant (shared-memory offsets become immediates), 0 = P.WX at run time
 template <int K1, int S, int WXT>
-__global__ void __launch_bounds__(FV3_MAXT)
+__global__ void __launch_bounds__(FV3_MAXT + 32)
     sweep_fusedv3_kernel(const __grid_constant__ CUtensorMap tmap, const FV3Params P)
 {
     constexpr int NN = K1 * K1, N3V = K1 * K1 * K1;
@@ -74,7 +75,8 @@ __global__ void __launch_bounds__(FV3_MAXT)
     const uint32_t empty_s = full_s + (uint32_t)ST * 8u;
 
     const int t = threadIdx.x;
-    const int NTR = (int)blockDim.x;                                    // whole warps
+    const bool PW = P.pw != 0;
+    const int NTR = (int)blockDim.x - (PW ? 32 : 0);                    // consumer threads (whole warps)
     const int LAG = ST >= 4 ? 2 : 1;                                    // the producer refills the slot of box i - LAG
     const int DEP = ST - LAG;                                           // boxes in flight ahead of the consumers
     const int strip = (int)(blockIdx.x % (unsigned)P.nstrips);          // neighbouring strips (shared halo) run together
@@ -105,8 +107,12 @@ __global__ void __launch_bounds__(FV3_MAXT)
         if (++pst == ST) { pst = 0; pn++; }
         pi++;
     };
-    if (t == 0)
+    if (PW) {                                                           // dedicated producer: the whole ring in flight at once
+        if (t == NTR)
+            for (int i = 0; i < ST; i++) produce();
+    } else if (t == 0) {
         for (int i = 0; i < DEP; i++) produce();
+    }
 
     // ---------------- consumers
     const int c = t / WX, x = t - c * WX;
@@ -146,6 +152,15 @@ __global__ void __launch_bounds__(FV3_MAXT)
         }
         __syncthreads();
     }
+    if (PW && t >= NTR) {
+        // Producer warp: lane 0 refills each slot as soon as every consumer warp has arrived on its empty barrier.  No consumer
+        // ever waits on an empty barrier or issues a copy, so a box is delayed only by the slowest warp's reads, not by warp 0's
+        // position in its own arithmetic.  The block's shared memory outlives this warp: the consumers wait for every full
+        // barrier before they finish.
+        if (t == NTR)
+            while (pi < total) produce();
+        return;
+    }
     // the alpha == 0 copy selects are compiled out for warps none of whose x nodes has the copy bit (the usual case)
     const bool anycp = __any_sync(0xffffffffu, cp1 || cp2 || cp3);
 
@@ -168,7 +183,7 @@ __global__ void __launch_bounds__(FV3_MAXT)
         constexpr bool CP = decltype(cpt)::value;
         // next box of the ring -> the v_1-swept (k+1)^3 block [j3][j2][j1] of this thread's v_1 cell
         auto swept_box = [&](real (&g)[N3V]) {
-            if (t == 0) produce();
+            if (!PW && t == 0) produce();
             mbar_wait(fbar, ph);
             real a[NN][K1], b[NN][K1];
             const real* pa = pa0 + soff;
@@ -302,7 +317,7 @@ cudaError_t launch(sldg_ctx* c, const CUtensorMap& tm, const FV3Params& P, int t
     if (e != cudaSuccess) return e;
     const long long grid = (long long)P.ntiles * P.nstrips;
     if (grid > 0x7fffffffLL) return cudaErrorNotSupported;
-    kern<<<(unsigned)grid, threads, smem, c->stream>>>(tm, P);
+    kern<<<(unsigned)grid, threads + (P.pw ? 32 : 0), smem, c->stream>>>(tm, P);
     return cudaGetLastError();
 }
 
@@ -337,7 +352,10 @@ bool shape(const sldg_ctx* c, FV3Shape* o)
     if (sizeof(real) == 4 && c->opt_fv3_wx <= 0) wx = 16;              // fp32: 64-byte rows (a 128-byte tile would need 2x the threads)
     while (wx * (int)sizeof(real) > 32 && (long long)wx * N1 > FV3_MAXT) wx /= 2;
     if ((long long)wx * N1 > FV3_MAXT || ((wx * (int)sizeof(real)) & 15) || wx > 256) return false;
-    int S = c->opt_fv3_strip > 0 ? c->opt_fv3_strip : 4;
+    // strip size: fp64 at degree 1 keeps a (k+1)^3 block per pair in registers; with 4 pairs ptxas spills at the 168-register cap
+    // of a 9..12-warp block (3 warps share a 16384-register sub-partition), with 3 it does not: measured on B200, cfg5, 28.1 -> 25.3 ms
+    // although 7 strips re-read more halo cells than 5 (profiles/r3_fusedv3.md)
+    int S = c->opt_fv3_strip > 0 ? c->opt_fv3_strip : ((sizeof(real) == 8 && K1 == 2) ? 3 : 4);
     if (S > FV3_MAXS) S = FV3_MAXS;
     if (S > N2) S = N2;
     int nstrips = (N2 + S - 1) / S;
@@ -379,7 +397,7 @@ cudaError_t SLDG_SFX(sldg_launch_sweep_fusedv3)(sldg_ctx* c, const void* fin, vo
     P.fout = static_cast<real*>(fout);
     P.X = c->X; P.N1 = c->cells[3]; P.N2 = c->cells[4]; P.N3 = c->cells[5]; P.WX = sh.wx;
     P.S = sh.S; P.nstrips = sh.nstrips; P.ntiles = (int)((c->X + sh.wx - 1) / sh.wx);
-    P.slots = sh.slots; P.slot_bytes = sh.slot_bytes;
+    P.slots = sh.slots; P.slot_bytes = sh.slot_bytes; P.pw = c->opt_fv3_pw ? 1 : 0;
     P.t1 = t1; P.t2 = t2; P.t3 = t3;
 
     CUtensorMap tm;

@@ -51,14 +51,43 @@ def halo_cells(geom, e_max, dt):
     return int(math.ceil(abs(e_max) * abs(dt) / h)) + 1
 
 
+class HaloTooNarrow(RuntimeError):
+    pass
+
+
+def cuda_interior_density(P, interior):
+    """-> callable(f_interior) for VShard(interior_density=...): rho of the interior slab through sldg_density_static, which
+    takes the slab (a contiguous sub-array of the extended array) and its velocity weights and needs neither a context nor a
+    workspace.  P is the binding module (paper_2110_14557_b200); the weights prod_d h_{v_d} w_{j_d} of the INTERIOR geometry
+    are built here once, on the host, and uploaded."""
+    import numpy as np
+    import torch
+    _, w = P.gauss_legendre(interior.degree)
+    Wv = np.ones(1)
+    for a in range(interior.dim_x, interior.d):
+        h = (interior.domain[2 * a + 1] - interior.domain[2 * a]) / interior.cells[a]
+        Wv = (np.tile(h * w, interior.cells[a])[:, None] * Wv[None, :]).reshape(-1)
+    Wv_dev = torch.from_numpy(np.ascontiguousarray(Wv)).cuda()
+    k1 = interior.degree + 1
+    xshape = tuple(reversed([c * k1 for c in interior.cells[:interior.dim_x]]))
+
+    def density(f_int):
+        return P.density_static(f_int, Wv_dev).reshape(xshape)
+    return density
+
+
 class VShard:
     """One rank's share of a v-sharded problem.
 
     make_engine(geometry) -> object with advect_x(f, tau), advect_v(f, E, tau), density(f) -> rho, poisson(rho) -> E acting
     on arrays of that geometry in place / by value (the CUDA binding's `Sldg` has exactly these calls).
-    `dist` is torch.distributed (already initialised) or None for a single rank."""
+    `dist` is torch.distributed (already initialised) or None for a single rank.
+    `interior_density` (optional): callable(f_interior) -> rho of the rank's interior cells.  Without it a SECOND engine is
+    built on the interior geometry just for rho; with the CUDA binding that engine is a full context whose workspace holds
+    another |f_interior| values of device memory.  `cuda_interior_density` below gives the CUDA path a density that needs no
+    context and no workspace (sldg_density_static), so the rank carries one workspace only."""
 
-    def __init__(self, geom, rank, world, halo, make_engine, dist=None):
+    def __init__(self, geom, rank, world, halo, make_engine, dist=None, interior_density=None):
         n = geom.cells[-1]
         if n % world:
             raise ValueError(f"cells of the cut axis ({n}) must divide evenly over {world} ranks")
@@ -73,8 +102,10 @@ class VShard:
         self.interior = geom.with_last_axis(self.n_loc, a, b)
         self.extended = geom.with_last_axis(self.n_loc + 2 * self.H, a - self.H * h, b + self.H * h)
         self.eng_ext = make_engine(self.extended)
-        self.eng_int = make_engine(self.interior) if self.H else self.eng_ext
+        self.interior_density = interior_density
+        self.eng_int = None if interior_density is not None else (make_engine(self.interior) if self.H else self.eng_ext)
         self.k1 = geom.degree + 1
+        self.h_cut = h
 
     # ---- views of the extended array (axis 0 of the array = slowest axis = the cut axis, in nodes)
     def interior_of(self, f_ext):
@@ -104,16 +135,31 @@ class VShard:
 
     def density(self, f_ext):
         """rho of the WHOLE problem: the rank's interior partial sum, all-reduced."""
-        rho = self.eng_int.density(self.interior_of(f_ext))
+        f_int = self.interior_of(f_ext)
+        rho = self.interior_density(f_int) if self.interior_density is not None else self.eng_int.density(f_int)
         if self.world > 1 and self.dist is not None:
             self.dist.all_reduce(rho, op=self.dist.ReduceOp.SUM)
         return rho
+
+    def check_halo(self, E, dt):
+        """The halo width was fixed at construction from an estimate of max|E|.  If the field has grown past it (two-stream
+        runs do), donors of interior cells would come from the periodic wrap of the widened slab: silently wrong.  So the
+        cut-axis component of the field just solved (X doubles, identical on every rank) is checked every step; the read-back
+        of its maximum synchronises the stream once per step."""
+        if not self.H:
+            return
+        emax = float(abs(E[-1]).max())
+        need = int(math.ceil(emax * abs(dt) / self.h_cut)) + 1
+        if need > self.H:
+            raise HaloTooNarrow(f"max|E| = {emax:.6g} on the cut axis needs a halo of {need} cells for dt = {dt:g}, "
+                                f"this shard was built with {self.H}: rebuild it with halo_cells(geom, e_max, dt) for a larger e_max")
 
     def step(self, f_ext, dt):
         """One Strang step on this rank's extended slab; returns (rho, E) of the step."""
         self.eng_ext.advect_x(f_ext, dt / 2.0)
         rho = self.density(f_ext)
         E = self.eng_ext.poisson(rho)                      # redundant on every rank
+        self.check_halo(E, dt)
         self.exchange_halos(f_ext)
         self.eng_ext.advect_v(f_ext, E, dt)
         self.eng_ext.advect_x(f_ext, dt / 2.0)

@@ -50,15 +50,17 @@ FV3_GEOMS = [
     ([3, 2, 2, 4, 3, 3], 2),          # degree 2: not fused (registers) -> planner falls back
 ]
 
-# (fuse_v3: 0 never / 2 whenever the shape allows, fv3_wx, fv3_strip, fv3_slots); plan 0 = three separate walks
-PLANS = ((0, 0, 0, 0), (2, 0, 0, 0), (2, 2, 1, 3), (2, 4, 2, 2), (2, 8, 3, 5), (2, 16, 5, 0), (2, 0, 4, 4), (1, 0, 0, 0))
+# (fuse_v3: 0 never / 2 whenever the shape allows, fv3_wx, fv3_strip, fv3_slots[, fv3_pw: dedicated producer warp]); plan 0 = three
+# separate walks; the last plan is the automatic rule
+PLANS = ((0, 0, 0, 0), (2, 0, 0, 0), (2, 2, 1, 3), (2, 4, 2, 2), (2, 8, 3, 5), (2, 16, 5, 0), (2, 0, 4, 4),
+         (2, 0, 0, 0, 1), (2, 8, 2, 2, 1), (2, 16, 5, 3, 1), (2, 4, 1, 5, 1), (1, 0, 0, 0))
 
 
 def run_plans(g, f0, E, dt, plans):
     outs = []
-    for fuse3, wx, strip, slots in plans:
+    for fuse3, wx, strip, slots, *rest in plans:
         g.set_option("fuse_v", 0); g.set_option("fuse_v3", fuse3); g.set_option("fv3_wx", wx)
-        g.set_option("fv3_strip", strip); g.set_option("fv3_slots", slots)
+        g.set_option("fv3_strip", strip); g.set_option("fv3_slots", slots); g.set_option("fv3_pw", rest[0] if rest else 0)
         fg = f0.to(g.device).contiguous()
         n0 = g.launch_count()
         g.advect_v(fg, E, dt)
@@ -192,9 +194,9 @@ def test_fused_v3_ring_under_drift_long_walks(P):
     want = f0.clone()
     g.advect_v(want, E, 0.1)
     g.set_option("fuse_v3", 2)
-    for slots, strip in ((2, 1), (3, 5), (4, 2), (0, 0)):
-        g.set_option("fv3_slots", slots); g.set_option("fv3_strip", strip)
+    for slots, strip, pw in ((2, 1, 0), (3, 5, 0), (4, 2, 0), (0, 0, 0), (2, 1, 1), (3, 5, 1), (0, 0, 1)):
+        g.set_option("fv3_slots", slots); g.set_option("fv3_strip", strip); g.set_option("fv3_pw", pw)
         for _ in range(3):
             got = f0.clone()
             g.advect_v(got, E, 0.1)
-            assert torch.equal(got, want), (slots, strip, int((got != want).sum()))
+            assert torch.equal(got, want), (slots, strip, pw, int((got != want).sum()))

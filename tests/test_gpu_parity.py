@@ -604,10 +604,12 @@ def test_declined_fused_passes_fall_back_to_the_same_bits(P, geom):
         assert np.array_equal(outs[0], x)
 
 
-def test_v_shard_plumbing_drives_the_cuda_context(P):
+@pytest.mark.parametrize("rho_by", ["second context", "density_static"])
+def test_v_shard_plumbing_drives_the_cuda_context(P, rho_by):
     """paper_2110_14557_b200/shard.py with the CUDA context as its engine (single rank: the halo exchange is the periodic
     wrap of the rank's own slab): a context on the widened sub-domain for the sweeps, one on the interior for rho.  The
-    interior must equal the plain single-domain steps (same sweeps; rho summed over the same values in another order)."""
+    interior must equal the plain single-domain steps (same sweeps; rho summed over the same values in another order).
+    "density_static": rho of the interior through the context-free entry point instead of a second context (and workspace)."""
     from paper_2110_14557_b200 import shard as S
     cfg = W.scaled(W.CONFIGS[0], [6, 4, 6, 8])
     g, o = pair_of_cfg(P, cfg)
@@ -617,7 +619,11 @@ def test_v_shard_plumbing_drives_the_cuda_context(P):
         g.step(ref, cfg["dt"])
     geom = S.Geometry(cfg["dim_x"], cfg["dim_v"], cfg["cells"], cfg["degree"], cfg["domain"])
     H = 2
-    sh = S.VShard(geom, 0, 1, H, lambda gm: P.Sldg(gm.dim_x, gm.dim_v, gm.cells, gm.degree, gm.domain))
+    make = lambda gm: P.Sldg(gm.dim_x, gm.dim_v, gm.cells, gm.degree, gm.domain)
+    sh = S.VShard(geom, 0, 1, H, make)
+    if rho_by == "density_static":
+        sh = S.VShard(geom, 0, 1, H, make, interior_density=S.cuda_interior_density(P, sh.interior))
+        assert sh.eng_int is None
     k1 = cfg["degree"] + 1
     f_ext = torch.zeros(tuple(reversed([c * k1 for c in sh.extended.cells])), dtype=torch.float64, device=g.device)
     sh.interior_of(f_ext).copy_(f0)

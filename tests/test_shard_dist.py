@@ -128,3 +128,39 @@ def test_halo_width_rule():
     assert S.halo_cells(g3, 100.0, 0.1) == 0                              # cut axis not advected
     with pytest.raises(ValueError):
         S.VShard(g, 0, 3, 1, lambda geom: None)                           # 8 cells do not divide over 3 ranks
+
+
+def test_step_refuses_a_field_that_outgrew_the_halo():
+    """VShard.step checks max|E| on the cut axis against the halo width it was built with (advisor finding, round 2): a field
+    that has grown past the construction-time estimate must raise, not wrap silently."""
+    import torch
+    from paper_2110_14557_b200 import shard as S
+
+    class FakeEngine:                       # plumbing only: a field of a chosen size, no arithmetic
+        emax = 0.5
+        def __init__(self, g):
+            self.g = g
+        def advect_x(self, f, tau): pass
+        def advect_v(self, f, E, tau): pass
+        def density(self, f): return torch.zeros(4)
+        def poisson(self, rho): return torch.full((2, 4), FakeEngine.emax, dtype=torch.float64)
+
+    geom = S.Geometry(2, 2, [2, 2, 8, 8], 1, [0, 1, 0, 1, -4, 4, -4, 4])          # h_v = 1
+    dt = 1.0
+    H = S.halo_cells(geom, 0.5, dt)                                               # ceil(0.5) + 1 = 2
+    assert H == 2
+    sh = S.VShard(geom, 0, 1, H, FakeEngine)
+    f_ext = torch.zeros(tuple(reversed([c * 2 for c in sh.extended.cells])), dtype=torch.float64)
+    sh.step(f_ext, dt)                                                            # |delta| = 0.5 <= H - 1: fine
+    FakeEngine.emax = 1.0
+    sh.step(f_ext, dt)                                                            # |delta| = 1.0 = H - 1: still fine
+    FakeEngine.emax = 1.25
+    with pytest.raises(S.HaloTooNarrow):
+        sh.step(f_ext, dt)                                                        # needs 3 cells
+    # the interior-density hook replaces the second engine
+    calls = []
+    sh2 = S.VShard(geom, 0, 1, H, FakeEngine, interior_density=lambda fi: calls.append(tuple(fi.shape)) or torch.zeros(4))
+    assert sh2.eng_int is None
+    FakeEngine.emax = 0.5
+    sh2.step(f_ext, dt)
+    assert calls == [tuple(sh2.interior_of(f_ext).shape)]
