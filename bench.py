@@ -264,6 +264,20 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
     s1.record(g.stream)
     torch.cuda.synchronize(dev)
     ms_single_calls = s0.elapsed_time(s1) / steps
+    # ---- and as K sldg_step_to calls ping-ponging between f and the workspace buffer: f(t_n) exists after every step too, at
+    # the pass budget of the merged plan (no third |f|-sized buffer)
+    wsf = g.workspace_field()
+    cur, oth = f, wsf
+    g.step_to(cur, oth, dt); cur, oth = oth, cur                # untimed: loads the kernels this plan uses
+    s0.record(g.stream)
+    for _ in range(steps):
+        g.step_to(cur, oth, dt)
+        cur, oth = oth, cur
+    s1.record(g.stream)
+    torch.cuda.synchronize(dev)
+    ms_step_to = s0.elapsed_time(s1) / steps
+    if cur is not f:
+        f.copy_(cur)
     # ---- the same K steps again with CUDA events around every launch (on the library's stream): per-kernel figures
     g.timing_enable(True)
     g.steps(f, dt, steps)                     # untimed, same plan: with events on, small problems leave the graph path (kernels load here)
@@ -329,7 +343,7 @@ def measure_config(args, cfg, dev, local, steps, warmup, headline):
                            "can exceed it (frac up to ~1.08 measured)")
     parts = {k: {"launches": n, "ms_per_step": ms / steps} for k, (n, ms) in kinds.items() if n}
     res = {"workload": cfg["name"], "values": nf, "bytes_f": nf * ESIZE, "ms_per_step": ms_step,
-           "single_step_ms": ms_single_calls,
+           "single_step_ms": ms_single_calls, "step_to_ms": ms_step_to,
            "effective_gbs_per_sweep": bytes_step / (ms_step * 1e-3) / 1e9,
            "passes_per_step": n_pass / steps, "rho_passes_per_step": n_rho / steps,
            "physical_bytes_per_step": phys_step, "physical_gbs": phys_step / (ms_step * 1e-3) / 1e9,
@@ -383,7 +397,9 @@ def run_ours(args, cfg, rank, world, local):
         "pct_of_measured_peak": 100 * value / world / peak, "pct_of_nominal_8TBs": 100 * value / world / NOMINAL_HBM_GBS,
         "physical_bytes_per_step": res["physical_bytes_per_step"], "physical_gbs": res["physical_gbs"],
         "physical_frac": res["physical_frac"], "passes_per_step": res["passes_per_step"],
-        "single_step_calls": {"ms_per_step": res["single_step_ms"], "note": "K separate sldg_step calls, each ending in the caller's buffer"},
+        "single_step_calls": {"ms_per_step": res["single_step_ms"], "note": "K separate sldg_step calls, each ending in the caller's buffer",
+                              "step_to_ms_per_step": res["step_to_ms"],
+                              "step_to_note": "K sldg_step_to calls ping-ponging between f and the workspace buffer: f(t_n) after every step"},
         "paper_style": paper_style,
         "kernels": res["kernels"], "sweeps_effective": res["sweeps_effective"], "parts": parts, "roofline": res["roofline"],
         "clocks": res["clocks"], "gpu_launches": res["gpu_launches"],
@@ -426,7 +442,7 @@ def run_ours(args, cfg, rank, world, local):
                 del g2, f2
                 torch.cuda.empty_cache()
                 rf = r["roofline"]
-                others[oc["name"]] = {"ms_per_step": r["ms_per_step"], "single_step_ms": r["single_step_ms"],
+                others[oc["name"]] = {"ms_per_step": r["ms_per_step"], "single_step_ms": r["single_step_ms"], "step_to_ms": r["step_to_ms"],
                                       "effective_gbs_per_sweep": r["effective_gbs_per_sweep"],
                                       "passes_per_step": r["passes_per_step"],
                                       "physical_bytes_per_step": r["physical_bytes_per_step"],
@@ -458,7 +474,7 @@ def run_ours(args, cfg, rank, world, local):
                 g2.close()
                 del g2, f2
                 torch.cuda.empty_cache()
-                blk = {"ms_per_step": r["ms_per_step"], "single_step_ms": r["single_step_ms"], "dtype": prec,
+                blk = {"ms_per_step": r["ms_per_step"], "single_step_ms": r["single_step_ms"], "step_to_ms": r["step_to_ms"], "dtype": prec,
                        "passes_per_step": r["passes_per_step"], "physical_gbs": r["physical_gbs"],
                        "physical_frac": r["physical_frac"], "effective_gbs_per_sweep": r["effective_gbs_per_sweep"],
                        "worst": r["roofline"]["worst"], "parts_frac": r["roofline"]["parts_frac"],
@@ -478,9 +494,10 @@ def run_ours(args, cfg, rank, world, local):
         def row(r):
             w = r.get("worst") or (r.get("roofline") or {}).get("worst") or {}
             return [round(r["ms_per_step"], 4), r["passes_per_step"], round(r["physical_frac"], 4), w.get("kernel"),
-                    round(w.get("frac", 0.0), 4)] if "ms_per_step" in r else [r.get("error")]
+                    round(w.get("frac", 0.0), 4), round(r["single_step_ms"], 4), round(r["step_to_ms"], 4)] if "ms_per_step" in r else [r.get("error")]
         line["roofline"]["by_config"] = {n: row(r) for n, r in list(others.items()) + list(f32.items())}
-        line["roofline"]["by_config_columns"] = "ms_per_step, passes_per_step, physical_frac, worst kernel, worst frac"
+        line["roofline"]["by_config_columns"] = "ms_per_step (sldg_steps), passes_per_step, physical_frac, worst kernel, worst frac, ms per sldg_step call, ms per sldg_step_to call"
+        line["roofline"]["headline_single_step_ms"] = [round(res["single_step_ms"], 4), round(res["step_to_ms"], 4)]
         line["roofline"]["previous_round_headline"] = "cfg5_6d_twostream_24x20_k1 (round 2: 72.29 ms; round 1 headline was cfg2)"
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -124,6 +124,19 @@ int sldg_poisson(sldg_ctx* ctx, const double* rho, double* E);
 /* a7, Strang splitting: advect_x(dt/2); density; poisson; advect_v(dt);
  * advect_x(dt/2).  rho and E of the step stay in the workspace (sldg_last_rho / sldg_last_E). */
 int sldg_step(sldg_ctx* ctx, double* f, double dt);
+/* a7 out of place: the same Strang step with the result in f_out.  f_in (|f| values, the state at t_n) is used as
+ * scratch and holds no meaningful data afterwards; f_out must not alias f_in or the workspace.  Why: sldg_step has to end in
+ * the buffer it was given, which forces an even number of buffer flips -- for dim_x = 3 the v advection then runs as two
+ * passes instead of one, for dim_x = 2 the fused v pass is not used.  A caller who needs f(t_n) after EVERY step (per-step
+ * diagnostics) and owns two buffers anyway ping-pongs between them with this call and gets the pass budget of sldg_steps
+ * (3 passes + rho for dim_x = 3).  Same 1-D sweeps in the same order as sldg_step: bit-identical result.
+ * end_of_step_field = 1 additionally evaluates rho and E of f(t_{n+1}) (the paper's second density/field evaluation per
+ * step, "This is done twice"): sldg_last_rho / sldg_last_E then belong to t_{n+1} instead of the half step.
+ * Always enqueues plain launches (no graph replay).  sldg_workspace_field returns the |f|-value buffer inside the workspace
+ * (NULL before sldg_set_workspace): it may serve as f_out / f_in of this call, so that f and the workspace ping-pong without
+ * a third buffer; every other sweep or step call overwrites it. */
+int sldg_step_to(sldg_ctx* ctx, double* f_in, double* f_out, double dt, int end_of_step_field);
+double* sldg_workspace_field(const sldg_ctx* ctx);
 /* Small problems (|f| <= 256 MB; option graph) replay a CUDA graph of the step, captured at the first call with a
  * given (f, dt).  1 if such a graph is instantiated right now (the next sldg_step with the same f, dt replays it). */
 int sldg_graph_active(const sldg_ctx* ctx);
@@ -226,6 +239,10 @@ int sldg_timing_axis(const sldg_ctx* ctx, long long* launches, double* ms);
  * by sldg_launch_count.  A fused or merged launch is ONE pass.  Returns 0 or a negative code. */
 int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
                     int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts);
+
+/* Host-only: the plan of one sldg_step_to call (same arguments and counts as sldg_plan_query; end_of_step_field as in the call). */
+int sldg_plan_query_step_to(int dim_x, int dim_v, const int* cells, int degree, int precision, int end_of_step_field,
+                            int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts);
 
 /* ---- rho for callers that cannot allocate device memory -----------------------------------
  * Same operation as sldg_density (a3): rho[x] = sum_v Wv[v] f[v][x], f seen as a row-major [V][X]

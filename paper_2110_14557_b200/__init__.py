@@ -4,4 +4,4 @@
 Argument marshalling only; every step of the path runs in the CUDA kernels under csrc/.
 There is no CPU fallback: if the library is missing or no CUDA device is present, calls raise.
 """
-from .binding import Sldg, SldgError, lib, library_path, EXPORTS, AB, gauss_legendre, sipg_matrices, plan_query, density_static, density_static_max_x  # noqa: F401
+from .binding import Sldg, SldgError, lib, library_path, EXPORTS, AB, gauss_legendre, sipg_matrices, plan_query, plan_query_step_to, density_static, density_static_max_x  # noqa: F401

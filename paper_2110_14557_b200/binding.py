@@ -33,6 +33,10 @@ EXPORTS = {
     "sldg_poisson": (C.c_int, [_vp, _vp, _vp]),
     "sldg_step": (C.c_int, [_vp, _vp, C.c_double]),
     "sldg_graph_active": (C.c_int, [_vp]),
+    "sldg_step_to": (C.c_int, [_vp, _vp, _vp, C.c_double, C.c_int]),
+    "sldg_workspace_field": (_vp, [_vp]),
+    "sldg_plan_query_step_to": (C.c_int, [C.c_int, C.c_int, _ip, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                          C.POINTER(C.c_longlong)]),
     "sldg_steps": (C.c_int, [_vp, _vp, C.c_double, C.c_int]),
     "sldg_step_host": (C.c_int, [_vp, _vp, _vp, _vp, C.c_double, C.c_int]),
     "sldg_field_elems": (_ll, [_vp]),
@@ -133,6 +137,17 @@ def plan_query(dim_x, dim_v, cells, degree, nsteps, precision="f64", shifts_belo
     out = (C.c_longlong * 6)()
     _check(lib().sldg_plan_query(int(dim_x), int(dim_v), cells_c, int(degree), 1 if precision == "f32" else 0, int(nsteps),
                                  1 if shifts_below_one else 0, int(fuse_v), int(fuse_v3), int(x_double), out))
+    return dict(zip(("x_passes", "v_passes", "rho_passes", "field_solves", "copies", "launches"), [int(v) for v in out]))
+
+
+def plan_query_step_to(dim_x, dim_v, cells, degree, precision="f64", end_of_step_field=False, shifts_below_one=True, fuse_v=1,
+                       x_double=1, fuse_v3=1):
+    """sldg_plan_query_step_to (host-only call): passes over f of one sldg_step_to call; same dict as plan_query."""
+    cells_c = (C.c_int * len(cells))(*[int(c) for c in cells])
+    out = (C.c_longlong * 6)()
+    _check(lib().sldg_plan_query_step_to(int(dim_x), int(dim_v), cells_c, int(degree), 1 if precision == "f32" else 0,
+                                         1 if end_of_step_field else 0, 1 if shifts_below_one else 0, int(fuse_v), int(fuse_v3),
+                                         int(x_double), out))
     return dict(zip(("x_passes", "v_passes", "rho_passes", "field_solves", "copies", "launches"), [int(v) for v in out]))
 
 
@@ -285,6 +300,16 @@ class Sldg:
 
     def step(self, f, dt):
         _check(lib().sldg_step(self._h, self._fp(f), float(dt)), self._h)
+
+    def step_to(self, f_in, f_out, dt, end_of_step_field=False):
+        _check(lib().sldg_step_to(self._h, self._fp(f_in), self._fp(f_out), float(dt), 1 if end_of_step_field else 0), self._h)
+
+    def workspace_field(self):
+        """The |f|-value buffer inside the workspace as a tensor VIEW (no copy): a valid f_out / f_in of step_to."""
+        ptr = lib().sldg_workspace_field(self._h)
+        off = ptr - self.workspace.data_ptr()
+        nbytes = self.nf * (4 if self.precision == "f32" else 8)
+        return self.workspace[off:off + nbytes].view(self.dtype).reshape(self.shape)
 
     def graph_active(self):
         return bool(lib().sldg_graph_active(self._h))

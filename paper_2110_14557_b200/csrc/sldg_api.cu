@@ -990,6 +990,26 @@ static int step_enqueue(sldg_ctx* c, double* f, double dt)
     return SLDG_OK;
 }
 
+// Out-of-place Strang step: the pair (f_in, f_out) takes the place of (f, workspace buffer) and the step is planned to END IN
+// THE OTHER BUFFER (flip_total = true), which is the cheapest parity for dim_x = 3 (one-pass x half steps + the one-flip
+// v_1v_2v_3 pass: 3 passes + rho) and lets dim_x = 2 use the fused v pass.
+extern "C" int sldg_step_to(sldg_ctx* c, double* f_in, double* f_out, double dt, int end_of_step_field)
+{
+    int r = check_f(c, f_in);
+    if (r) return r;
+    if ((r = check_f(c, f_out))) return r;
+    if (f_in == f_out) return SLDG_EINVAL;
+    double *cur = f_in, *oth = f_out;
+    if ((r = step_core(c, &cur, &oth, dt, true))) return r;
+    if (cur != f_out && (r = copy_back(c, f_out, cur))) return r;              // unreachable by construction
+    if (end_of_step_field) {                                                    // rho, E of f(t_{n+1}) for the diagnostics
+        if ((r = sldg_density(c, f_out, c->rho))) return r;
+        if ((r = c->poisson_solver == 1 ? sldg_poisson_cg(c, c->rho, c->E, c->cg_tol, 0) : sldg_poisson(c, c->rho, c->E))) return r;
+    }
+    return SLDG_OK;
+}
+extern "C" double* sldg_workspace_field(const sldg_ctx* c) { return (c && c->ws_ready) ? c->f2 : nullptr; }
+
 void sldg_graph_drop(sldg_ctx* c)
 {
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
@@ -1115,8 +1135,8 @@ extern "C" int sldg_steps(sldg_ctx* c, double* f, double dt, int nsteps)
 // Host-only: run the planning code of sldg_step (nsteps == 0) or sldg_steps(nsteps) on a context without a device and
 // count what it would launch.  The same functions plan and launch (c->dry only replaces the launches), so the counts
 // are those of the real calls.
-extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
-                               int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts)
+static int plan_query_impl(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
+                           int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts, bool step_to)
 {
     if (!counts || nsteps < 0 || fuse_v < 0 || fuse_v > 2 || fuse_v3 < 0 || fuse_v3 > 2 || x_double < 0 || x_double > 2) return SLDG_EINVAL;
     if (precision != SLDG_F64 && precision != SLDG_F32) return SLDG_EINVAL;
@@ -1132,11 +1152,24 @@ extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degre
     double* f = reinterpret_cast<double*>((uintptr_t)0x10000);
     c->f2 = reinterpret_cast<double*>((uintptr_t)0x20000);
     c->rho = c->E = reinterpret_cast<double*>((uintptr_t)0x30000);
-    r = nsteps == 0 ? sldg_step(c, f, 0.1) : sldg_steps(c, f, 0.1, nsteps);
+    if (step_to) r = sldg_step_to(c, f, reinterpret_cast<double*>((uintptr_t)0x40000), 0.1, nsteps);   // nsteps carries end_of_step_field
+    else r = nsteps == 0 ? sldg_step(c, f, 0.1) : sldg_steps(c, f, 0.1, nsteps);
     counts[0] = c->dry_x; counts[1] = c->dry_v; counts[2] = c->dry_rho; counts[3] = c->dry_field; counts[4] = c->dry_copies;
     counts[5] = c->launches;
     delete c;
     return r;
+}
+
+extern "C" int sldg_plan_query(int dim_x, int dim_v, const int* cells, int degree, int precision, int nsteps,
+                               int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts)
+{
+    return plan_query_impl(dim_x, dim_v, cells, degree, precision, nsteps, shifts_below_one, fuse_v, fuse_v3, x_double, counts, false);
+}
+extern "C" int sldg_plan_query_step_to(int dim_x, int dim_v, const int* cells, int degree, int precision, int end_of_step_field,
+                                       int shifts_below_one, int fuse_v, int fuse_v3, int x_double, long long* counts)
+{
+    if (end_of_step_field < 0 || end_of_step_field > 1) return SLDG_EINVAL;
+    return plan_query_impl(dim_x, dim_v, cells, degree, precision, end_of_step_field, shifts_below_one, fuse_v, fuse_v3, x_double, counts, true);
 }
 
 extern "C" int sldg_step_host(sldg_ctx* c, double* f_host, double* f_dev, double* E_host, double dt, int nsteps)

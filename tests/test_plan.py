@@ -85,3 +85,20 @@ def test_every_plan_ends_in_the_callers_buffer_without_a_copy(dx, dv, k):
         # never more passes than one per 1-D sweep, never fewer than the merged minimum
         assert r["x_passes"] <= 2 * dx * steps and r["v_passes"] <= dx * steps
         assert r["x_passes"] >= steps + 1 and r["v_passes"] >= steps
+
+
+def test_out_of_place_step_has_the_pass_budget_of_merged_steps():
+    """sldg_step_to (result in the other buffer) may flip the buffers an odd number of times: one step of the 3x3v
+    configs is 3 passes + rho (sldg_step: 4), of the dim_x = 2 configs 3 passes (sldg_step: 4); the end-of-step field evaluation
+    of PAPER.md:199 adds exactly one rho pass and one field solve; never a whole-array copy."""
+    import paper_2110_14557_b200 as P
+    for dx, dv, cells, k in [(3, 3, [24, 24, 24, 20, 20, 20], 1), (3, 3, [20] * 6, 1), (2, 2, [64] * 4, 2), (2, 3, [32] * 5, 1)]:
+        one = P.plan_query(dx, dv, cells, k, 0)
+        to = P.plan_query_step_to(dx, dv, cells, k)
+        diag = P.plan_query_step_to(dx, dv, cells, k, end_of_step_field=True)
+        assert one["x_passes"] + one["v_passes"] == 4
+        assert (to["x_passes"], to["v_passes"], to["rho_passes"], to["field_solves"], to["copies"]) == (2, 1, 1, 1, 0)
+        assert (diag["x_passes"], diag["v_passes"], diag["rho_passes"], diag["field_solves"], diag["copies"]) == (2, 1, 2, 2, 0)
+    # degree 3 (no one-pass 3x3v sweeps yet): no worse than sldg_step
+    one, to = P.plan_query(3, 3, [9] * 6, 3, 0), P.plan_query_step_to(3, 3, [9] * 6, 3)
+    assert to["x_passes"] + to["v_passes"] <= one["x_passes"] + one["v_passes"] and to["copies"] == 0
