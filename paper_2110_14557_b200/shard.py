@@ -4,7 +4,8 @@ reduced.  Every arithmetic step stays in the engine the caller supplies (the CUD
 drive the same plumbing over CPU buffers with gloo).  BASELINE.json fixes ONE GPU for this build ("replicas only",
 DESIGN.md section 9), so nothing in bench.py uses this module; it is the design of the next row, kept testable.
 
-Decomposition.  The SLOWEST velocity axis (axis d-1) is cut into `world` contiguous slabs of n_loc cells.  A rank stores
+Decomposition.  The SLOWEST velocity axis (axis d-1) is cut into `world` contiguous slabs of n_loc cells (slabs differ by at
+most one cell when the cell count is not a multiple of `world`; `start` is a slab's first cell).  A rank stores
 its slab plus H halo cells on either side, f_ext = [n_loc + 2H cells of v_last][...all other axes...], i.e. one contiguous
 array in the library's layout whose last axis has n_loc + 2H cells and whose domain on that axis is widened by H cells.
 
@@ -89,16 +90,20 @@ class VShard:
 
     def __init__(self, geom, rank, world, halo, make_engine, dist=None, interior_density=None):
         n = geom.cells[-1]
-        if n % world:
-            raise ValueError(f"cells of the cut axis ({n}) must divide evenly over {world} ranks")
         self.geom, self.rank, self.world, self.H, self.dist = geom, int(rank), int(world), int(halo), dist
-        self.n_loc = n // world
-        if self.H > self.n_loc:
-            raise ValueError("halo wider than a slab: use fewer ranks or a smaller time step")
+        if not 0 <= self.rank < self.world or self.world > n:
+            raise ValueError(f"{world} ranks for {n} cells on the cut axis")
+        # Slabs need not be equal: the first n % world ranks own one cell more (20 cells of cfg4/cfg5 over 8 ranks: 3,3,3,3,2,2,2,2).
+        # Nothing else depends on equal slabs -- a halo is H cells whatever the neighbour's size, rho is an all-reduce.
+        q, rem = divmod(n, self.world)
+        self.n_loc = q + (1 if self.rank < rem else 0)
+        self.start = self.rank * q + min(self.rank, rem)          # first cell of the slab on the cut axis
+        if self.H > q:
+            raise ValueError("halo wider than the smallest slab: use fewer ranks or a smaller time step")
         lo, hi = geom.domain[-2], geom.domain[-1]
         h = (hi - lo) / n
-        a = lo + self.rank * self.n_loc * h
-        b = lo + (self.rank + 1) * self.n_loc * h
+        a = lo + self.start * h
+        b = lo + (self.start + self.n_loc) * h
         self.interior = geom.with_last_axis(self.n_loc, a, b)
         self.extended = geom.with_last_axis(self.n_loc + 2 * self.H, a - self.H * h, b + self.H * h)
         self.eng_ext = make_engine(self.extended)

@@ -56,7 +56,7 @@ H = S.halo_cells(geom, 1.05 * emax, dt)
 sh = S.VShard(geom, rank, world, H, OracleEngine, dist if world > 1 else None)
 # this rank's extended slab of the initial data (halo cells start as garbage: the first exchange fills them)
 k1 = cfg["degree"] + 1
-r0 = rank * sh.n_loc * k1
+r0 = sh.start * k1
 f_ext = torch.full(tuple(reversed([c * k1 for c in sh.extended.cells])), float("nan"), dtype=torch.float64)
 sh.interior_of(f_ext).copy_(torch.from_numpy(f_full[r0:r0 + sh.n_loc * k1]))
 if H:
@@ -111,6 +111,31 @@ def test_two_rank_sharded_steps_equal_the_single_domain_steps(tmp_path, ci):
         assert res[0]["H"] == 0                               # 2x3v: nothing to exchange
 
 
+def test_three_ranks_with_uneven_slabs(tmp_path):
+    """8 cells of the cut axis over 3 ranks: slabs of 3, 3 and 2 cells (the 20 v_3 cells of cfg4 / cfg5 do not divide by 8 either)."""
+    res = run_ranks(tmp_path, CASES[1], 3, 29661)
+    assert sorted(d["n_loc"] for d in res) == [2, 3, 3]
+    for d in res:
+        assert d["finite"] and d["err"] <= 1e-13 and d["err_rho"] <= 1e-13 and d["err_E"] <= 1e-11, d
+
+
+def test_slab_bounds_of_uneven_cuts():
+    sys.path.insert(0, ROOT)
+    from paper_2110_14557_b200 import shard as S
+
+    class Nothing:
+        def __init__(self, g): self.g = g
+    geom = S.Geometry(3, 3, [2, 2, 2, 2, 2, 20], 1, [0, 1] * 5 + [-6, 6])
+    sl = [S.VShard(geom, r, 8, 2, Nothing) for r in range(8)]
+    assert [s.n_loc for s in sl] == [3, 3, 3, 3, 2, 2, 2, 2] and [s.start for s in sl] == [0, 3, 6, 9, 12, 14, 16, 18]
+    for a, b in zip(sl, sl[1:]):
+        assert a.interior.domain[-1] == pytest.approx(b.interior.domain[-2], abs=1e-15)
+    assert sl[0].interior.domain[-2] == -6 and sl[-1].interior.domain[-1] == pytest.approx(6)
+    assert sl[4].extended.cells[-1] == 2 + 4
+    with pytest.raises(ValueError):
+        S.VShard(geom, 0, 8, 3, Nothing)                      # halo wider than the smallest slab
+
+
 def test_single_rank_shard_is_the_periodic_problem(tmp_path):
     """world = 1: the halo exchange degenerates to the periodic wrap of the rank's own slab."""
     res = run_ranks(tmp_path, CASES[1], 1, 29651)
@@ -126,8 +151,9 @@ def test_halo_width_rule():
     assert S.halo_cells(g, 31.0, 0.1) == 4                                # |delta| = 2.07 cells
     g3 = S.Geometry(2, 3, [4, 4, 4, 4, 6], 1, [0, 1] * 2 + [-6, 6] * 3)
     assert S.halo_cells(g3, 100.0, 0.1) == 0                              # cut axis not advected
+    assert S.VShard(g, 0, 3, 1, lambda geom: None).n_loc == 3             # 8 cells over 3 ranks: uneven slabs (3, 3, 2) are allowed
     with pytest.raises(ValueError):
-        S.VShard(g, 0, 3, 1, lambda geom: None)                           # 8 cells do not divide over 3 ranks
+        S.VShard(g, 0, 9, 1, lambda geom: None)                           # more ranks than cells
 
 
 def test_step_refuses_a_field_that_outgrew_the_halo():
